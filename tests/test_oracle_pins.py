@@ -1,0 +1,528 @@
+"""Pins of the CPU oracle against what the paper and the mathematics fix.
+
+None of these compares the oracle with itself through the same formula: each
+uses a closed form the paper prints (Eq. 6-8, W_RP = 9 S0^2 W), an invariant
+(uniform field, translation, rotation, L2 == L3 on periodic lattices), brute
+force (central finite differences of the total energy) or a special case that
+reduces to a textbook result (plane-wave response of the 7-point Laplacian,
+velocity Verlet on a harmonic oscillator).  Citations: PAPER.md:<line>.
+"""
+import math
+import os
+
+import numpy as np
+import pytest
+
+from paper_1911_07045_b200 import workloads as wl
+
+A, B, Cc, L1 = wl.A_5CB, wl.B_5CB, wl.C_5CB, wl.L1_5CB
+GOLD = os.path.join(os.path.dirname(__file__), "golden")
+
+
+def _golden(name):
+    vals = {}
+    with open(os.path.join(GOLD, name)) as f:
+        for line in f:
+            line = line.split("#")[0].strip()
+            if line:
+                k, v = line.split("=")
+                vals[k.strip()] = float(v)
+    return vals
+
+
+def full_tensor(q):
+    """[N,3,3] from [5][N]"""
+    xx, xy, xz, yy, yz = q
+    Q = np.empty((q.shape[1], 3, 3))
+    Q[:, 0, 0], Q[:, 0, 1], Q[:, 0, 2] = xx, xy, xz
+    Q[:, 1, 0], Q[:, 1, 1], Q[:, 1, 2] = xy, yy, yz
+    Q[:, 2, 0], Q[:, 2, 1], Q[:, 2, 2] = xz, yz, -xx - yy
+    return Q
+
+
+def five(Q):
+    return np.stack([Q[:, 0, 0], Q[:, 0, 1], Q[:, 0, 2], Q[:, 1, 1], Q[:, 1, 2]])
+
+
+def make(oracle_mod, c, **over):
+    kw = dict(L1=c["L1"], L2=c["L2"], L3=c["L3"], mask=c["mask"], kind=c["kind"], W=c["W"], axis=c["axis"])
+    kw.update(over)
+    return oracle_mod.Oracle(c["Lx"], c["Ly"], c["Lz"], c["A"], c["B"], c["C"], kw.pop("L1"), kw.pop("L2"),
+                             kw.pop("L3"), **kw)
+
+
+# ---------------------------------------------------------------- P1: bulk
+
+def test_S0_matches_paper_value(oracle_mod):
+    """PAPER.md:171 prints 'S0 ~ 0.53' for the 5CB constants; Eq. 7."""
+    g = _golden("paper_constants.txt")
+    S0 = oracle_mod.S0_of(A, B, Cc)
+    assert abs(S0 - g["S0_printed"]) < 0.005          # the paper's two printed digits
+    assert abs(oracle_mod.q0_of(A, B, Cc) - wl.Q0_5CB) < 2e-16
+    # S0 is a stationary point of Eq. 6: f'(S) = 3/2 A S + 3/4 B S^2 + 9/4 C S^3
+    assert abs(1.5 * A * S0 + 0.75 * B * S0 ** 2 + 2.25 * Cc * S0 ** 3) < 1e-15
+    # K = L1 * 9 S0^2 / 2 = 1e-11 N and dx = sqrt(L1_phys / (L1~ |A|)) ~ 4.5 nm
+    L1_phys = 1e-11 / (4.5 * S0 ** 2)
+    dx = math.sqrt(L1_phys / (L1 * abs(A) * 1e6))
+    assert abs(dx * 1e9 - g["dx_nm_printed"]) < 0.1
+
+
+@pytest.mark.parametrize("variant", [0, 1])
+def test_bulk_energy_is_eq6_on_uniaxial(oracle_mod, variant):
+    """Eq. 5 on Q = 3/2 S (nn - I/3) equals the polynomial Eq. 6, any S, any n."""
+    rng = np.random.default_rng(1)
+    o = oracle_mod.Oracle(4, 4, 4, A, B, Cc, 0.0)
+    for S in (0.1, 0.3, oracle_mod.S0_of(A, B, Cc), 0.9, -0.2):
+        n = rng.standard_normal(3)
+        n /= np.linalg.norm(n)
+        q = wl.uniaxial_q(np.repeat(n[:, None], 64, axis=1), 1.5 * S)
+        e, terms = o.energy(q, variant, terms=True)
+        eq6 = 0.75 * A * S ** 2 + 0.25 * B * S ** 3 + 9.0 / 16.0 * Cc * S ** 4
+        assert abs(e - 64 * eq6) < 1e-13
+        assert terms[1] == 0.0 and terms[2] == 0.0
+
+
+@pytest.mark.parametrize("variant", [0, 1])
+def test_uniform_S0_has_zero_force_and_f0(oracle_mod, variant):
+    """S = S0 minimises Eq. 6: zero force, energy density f0."""
+    S0 = oracle_mod.S0_of(A, B, Cc)
+    f0 = 0.75 * A * S0 ** 2 + 0.25 * B * S0 ** 3 + 9.0 / 16.0 * Cc * S0 ** 4
+    o = oracle_mod.Oracle(5, 4, 6, A, B, Cc, L1, 1.0, 0.5)
+    n = np.array([0.3, -0.5, 0.81])
+    n /= np.linalg.norm(n)
+    q = wl.uniaxial_q(np.repeat(n[:, None], 120, axis=1), wl.Q0_5CB)
+    assert abs(o.energy(q, variant) - 120 * f0) < 1e-13
+    assert np.abs(o.forces(q, variant)).max() < 1e-14
+
+
+# ---------------------------------------------------- P2: uniform field, masks
+
+@pytest.mark.parametrize("variant", [0, 1])
+def test_uniform_field_no_elastic_energy_or_force_on_any_mask(oracle_mod, variant):
+    c = wl.random_masked_problem(7, 6, 5, 4, obj_frac=0.3)
+    o = oracle_mod.Oracle(6, 5, 4, 0.0, 0.0, 1.0, 2.32, 1.0, 0.5, mask=c["mask"])
+    q = np.repeat(np.array([0.2, -0.1, 0.3, 0.15, -0.25])[:, None], c["N"], axis=1)
+    e, terms = o.energy(q, variant, terms=True)
+    assert terms[1] == 0.0
+    o2 = oracle_mod.Oracle(6, 5, 4, 0.0, 0.0, 0.0, 2.32, 1.0, 0.5, mask=c["mask"])
+    assert np.abs(o2.forces(q, variant)).max() == 0.0
+
+
+# ------------------------------------- P3: force = -central FD of total energy
+
+def _fd_force(o, q, variant, h=1e-5):
+    F = np.zeros_like(q)
+    qq = q.copy()
+    for c in range(5):
+        for s in range(q.shape[1]):
+            old = qq[c, s]
+            qq[c, s] = old + h
+            ep = o.energy(qq, variant)
+            qq[c, s] = old - h
+            em = o.energy(qq, variant)
+            qq[c, s] = old
+            F[c, s] = -(ep - em) / (2 * h)
+    return F
+
+
+@pytest.mark.parametrize("dims,seed,L2,L3", [((4, 4, 4), 11, 0.0, 0.0), ((4, 4, 4), 12, 0.7, 0.4),
+                                             ((5, 4, 6), 13, 1.0, 0.5), ((6, 6, 6), 14, 0.0, 0.9)])
+@pytest.mark.parametrize("variant", [0, 1])
+def test_force_is_minus_gradient_of_energy(oracle_mod, dims, seed, L2, L3, variant):
+    """forces come from explicit differentiation of the discretised F for bulk and
+    boundary sites alike -> brute-force central differences of the total energy must agree."""
+    c = wl.random_masked_problem(seed, *dims, obj_frac=0.25, L2=L2, L3=L3)
+    o = make(oracle_mod, c)
+    F = o.forces(c["q"], variant)
+    Ffd = _fd_force(o, c["q"], variant)
+    sim = c["mask"] == 0
+    assert np.abs(F[:, ~sim]).max() == 0.0
+    assert np.abs(Ffd[:, ~sim]).max() == 0.0          # object-site values do not enter the energy
+    scale = np.abs(F).max()
+    assert np.abs(F - Ffd).max() < 2e-8 * scale
+    # single-site evaluation agrees with the field
+    rng = np.random.default_rng(seed)
+    for s in rng.integers(0, c["N"], size=20):
+        x, y, z = s % dims[0], (s // dims[0]) % dims[1], s // (dims[0] * dims[1])
+        assert np.abs(o.force_at(c["q"], x, y, z, variant) - F[:, s]).max() < 1e-12 * scale
+
+
+def test_force_fd_periodic_object_free(oracle_mod):
+    c = wl.bulk_quench(4, 5)
+    o = oracle_mod.Oracle(4, 4, 4, A, B, Cc, L1, 1.0, 0.5)
+    q = c["q"] + 0.05 * np.random.default_rng(3).standard_normal(c["q"].shape)
+    for variant in (0, 1):
+        F = o.forces(q, variant)
+        assert np.abs(F - _fd_force(o, q, variant)).max() < 2e-8 * np.abs(F).max()
+
+
+# ---------------------------------------------- P4: literal == factorised
+
+@pytest.mark.parametrize("seed", [21, 22, 23])
+def test_literal_equals_factorised(oracle_mod, seed):
+    c = wl.random_masked_problem(seed, 7, 5, 6, obj_frac=0.3, L2=1.0, L3=0.5)
+    o = make(oracle_mod, c)
+    e0, t0 = o.energy(c["q"], 0, terms=True)
+    e1, t1 = o.energy(c["q"], 1, terms=True)
+    assert abs(e0 - e1) < 1e-13 * max(1.0, abs(e0))
+    assert np.abs(t0 - t1).max() < 1e-12 * np.abs(t0).max()
+    F0, F1 = o.forces(c["q"], 0), o.forces(c["q"], 1)
+    assert np.abs(F0 - F1).max() < 1e-13 * np.abs(F0).max()
+
+
+def test_factorised_openmp_colouring_all_Lz_remainders(oracle_mod):
+    """the z-plane 3-colouring of the scatter must not depend on Lz mod 3 or the thread count"""
+    for Lz in (4, 5, 6, 7, 8):
+        c = wl.random_masked_problem(30 + Lz, 5, 4, Lz, obj_frac=0.15)
+        o = make(oracle_mod, c)
+        F0 = o.forces(c["q"], 0)
+        for nt in (1, 3, 8):
+            oracle_mod.set_num_threads(nt)
+            assert np.abs(o.forces(c["q"], 1) - F0).max() < 1e-13 * np.abs(F0).max()
+    oracle_mod.set_num_threads(os.cpu_count() or 1)
+
+
+# ------------------------------------------ P5: L2 == L3 on periodic lattices
+
+def test_L2_equals_L3_periodic_but_not_with_objects(oracle_mod):
+    """On an object-free periodic lattice the L2 and L3 sums are related by a discrete
+    integration by parts (centred differences commute), so only L2+L3 matters; next to
+    objects the one-sided differences break this."""
+    rng = np.random.default_rng(5)
+    q = 0.3 * rng.standard_normal((5, 6 * 5 * 4))
+    a, b = 0.8, 0.45
+    oa = oracle_mod.Oracle(6, 5, 4, A, B, Cc, L1, a, b)
+    ob = oracle_mod.Oracle(6, 5, 4, A, B, Cc, L1, a + b, 0.0)
+    for v in (0, 1):
+        assert abs(oa.energy(q, v) - ob.energy(q, v)) < 1e-12
+        assert np.abs(oa.forces(q, v) - ob.forces(q, v)).max() < 1e-12
+    c = wl.random_masked_problem(6, 6, 5, 4, obj_frac=0.2)
+    oa = oracle_mod.Oracle(6, 5, 4, A, B, Cc, L1, a, b, mask=c["mask"])
+    ob = oracle_mod.Oracle(6, 5, 4, A, B, Cc, L1, a + b, 0.0, mask=c["mask"])
+    assert abs(oa.energy(q, 0) - ob.energy(q, 0)) > 1e-4
+
+
+# ------------------------------------------------ P6: plane-wave response
+
+M5 = np.array([[2, 0, 0, 1, 0], [0, 2, 0, 0, 0], [0, 0, 2, 0, 0], [1, 0, 0, 2, 0], [0, 0, 0, 0, 2.0]])
+
+
+@pytest.mark.parametrize("kvec", [(1, 0, 0), (0, 2, 0), (1, 1, 3), (4, 3, 2)])
+@pytest.mark.parametrize("variant", [0, 1])
+def test_plane_wave_response_one_constant(oracle_mod, kvec, variant):
+    """Averaged forward/backward differences give the nearest-neighbour bond energy
+    (PAPER.md:183), i.e. the 7-point Laplacian: a plane wave dq cos(k.x) on a uniform
+    background feels  F_el = -L1 * lambda(k) * M dq cos(k.x),  lambda = sum_k 4 sin^2(k_k/2),
+    M = metric of tr(dQ^2) in the 5 variables.  (kvec = (4,3,2) on 8x6x4 is the checkerboard,
+    lambda = 12: no lattice doubling.)"""
+    Lx, Ly, Lz = 8, 6, 4
+    o = oracle_mod.Oracle(Lx, Ly, Lz, 0.0, 0.0, 0.0, L1)
+    z, y, x = np.meshgrid(np.arange(Lz), np.arange(Ly), np.arange(Lx), indexing="ij")
+    k = 2 * np.pi * np.array(kvec) / np.array([Lx, Ly, Lz])
+    phase = np.cos(k[0] * x + k[1] * y + k[2] * z).reshape(-1)
+    dq = np.array([0.01, -0.02, 0.03, 0.015, -0.005])
+    q0 = np.array([0.2, -0.1, 0.3, 0.15, -0.25])
+    q = q0[:, None] + dq[:, None] * phase[None, :]
+    lam = float(np.sum(4 * np.sin(k / 2) ** 2))
+    F_expected = -L1 * lam * (M5 @ dq)[:, None] * phase[None, :]
+    F = o.forces(q, variant)
+    assert np.abs(F - F_expected).max() < 1e-14
+    if kvec == (4, 3, 2):
+        assert abs(lam - 12.0) < 1e-12 and np.abs(F).max() > 0.1
+
+
+def test_one_constant_energy_is_bond_sum(oracle_mod):
+    """periodic, object-free: E_el = (L1/2) * sum over nearest-neighbour bonds |Q(x+k)-Q(x)|_F^2"""
+    rng = np.random.default_rng(9)
+    Lx, Ly, Lz = 5, 4, 6
+    q = 0.3 * rng.standard_normal((5, Lx * Ly * Lz))
+    Q = full_tensor(q).reshape(Lz, Ly, Lx, 3, 3)
+    bonds = sum(((np.roll(Q, -1, axis=ax) - Q) ** 2).sum() for ax in range(3))
+    o = oracle_mod.Oracle(Lx, Ly, Lz, A, B, Cc, L1)
+    for v in (0, 1):
+        assert abs(o.energy(q, v, terms=True)[1][1] - 0.5 * L1 * bonds) < 1e-11
+
+
+# ------------------------------------------------- P7: lattice symmetries
+
+def test_translation_invariance(oracle_mod):
+    c = wl.random_masked_problem(41, 6, 5, 4, obj_frac=0.2)
+    o = make(oracle_mod, c)
+    e, F = o.energy(c["q"], 1), o.forces(c["q"], 1)
+    sh = (1, 2, 3)  # shift in (z, y, x)
+
+    def roll(a):
+        lead = a.shape[:-1]
+        return np.roll(a.reshape(*lead, 4, 5, 6), sh, axis=(-3, -2, -1)).reshape(*lead, -1)
+
+    c2 = dict(c, mask=roll(c["mask"]), kind=roll(c["kind"]), W=roll(c["W"]), axis=roll(c["axis"]))
+    o2 = make(oracle_mod, c2)
+    assert abs(o2.energy(roll(c["q"]), 1) - e) < 1e-12 * abs(e)
+    assert np.abs(o2.forces(roll(c["q"]), 1) - roll(F)).max() < 1e-12 * np.abs(F).max()
+
+
+def _rotate_field(q, L, R):
+    """site x -> R x (about the lattice origin, mod L), tensor Q -> R Q R^T."""
+    Q = full_tensor(q).reshape(L, L, L, 3, 3)            # [z][y][x]
+    out = np.empty_like(Q)
+    idx = np.arange(L)
+    Z, Y, X = np.meshgrid(idx, idx, idx, indexing="ij")
+    pos = np.stack([X, Y, Z], axis=-1)                    # (x,y,z) of each site
+    new = np.einsum("ab,zyxb->zyxa", R, pos) % L
+    Qr = np.einsum("ia,zyxab,jb->zyxij", R, Q, R)
+    out[new[..., 2], new[..., 1], new[..., 0]] = Qr
+    return five(out.reshape(-1, 3, 3))
+
+
+def test_rotation_invariance(oracle_mod):
+    """Eq. 5 and Eq. 10 are scalars: energy invariant under the cubic group on a periodic lattice
+    (all of L1, L2, L3); for rotations about z the 5-variable force is covariant too."""
+    L = 5
+    rng = np.random.default_rng(77)
+    q = 0.3 * rng.standard_normal((5, L ** 3))
+    o = oracle_mod.Oracle(L, L, L, A, B, Cc, L1, 1.0, 0.5)
+    Rz = np.array([[0, -1, 0], [1, 0, 0], [0, 0, 1]])
+    Rx = np.array([[1, 0, 0], [0, 0, -1], [0, 1, 0]])
+    e = o.energy(q, 0)
+    for R in (Rz, Rx, Rz @ Rx, Rx @ Rx @ Rz):
+        for v in (0, 1):
+            assert abs(o.energy(_rotate_field(q, L, R), v) - e) < 1e-11 * abs(e)
+    F = o.forces(q, 0)
+    Fr = o.forces(_rotate_field(q, L, Rz), 0)
+    # rotate F as a 5-vector field: for Rz the map on (xx,xy,xz,yy,yz) is a signed permutation,
+    # so F transforms like q itself
+    assert np.abs(Fr - _rotate_field(F, L, Rz)).max() < 1e-12 * np.abs(F).max()
+
+
+# ------------------------------------------------ P8: anchoring closed forms
+
+@pytest.mark.parametrize("variant", [0, 1])
+def test_anchoring_closed_forms(oracle_mod, variant):
+    """Uniaxial Q at S0 tilted by theta from the axis.  Eq. 14: W tr((Q-Q0)^2) =
+    (9/2) S0^2 W sin^2(theta) = (W_RP/2) sin^2(theta) -> the Rapini-Papoular form with
+    W_RP = 9 S0^2 W_ND printed at PAPER.md:149.  Eq. 15 with Qt_perp = P Qt P:
+    (9/4) S0^2 W (2 cos^2 - cos^4)."""
+    S0 = oracle_mod.S0_of(A, B, Cc)
+    Lx = Ly = 4
+    Lz = 5
+    N = Lx * Ly * Lz
+    mask = np.zeros((Lz, Ly, Lx), np.uint8)
+    mask[0] = 1                                        # one wall; z=1 and z=4 are boundary layers
+    Wv = 1.7
+    nu = np.array([0.0, 0.0, 1.0])
+    for kind_id in (1, 2):
+        for theta in (0.0, 0.3, 1.1, np.pi / 2):
+            n = np.array([np.sin(theta) * np.cos(0.4), np.sin(theta) * np.sin(0.4), np.cos(theta)])
+            q = wl.uniaxial_q(np.repeat(n[:, None], N, axis=1), 1.5 * S0)
+            kind = np.zeros((Lz, Ly, Lx), np.uint8)
+            kind[1] = kind_id
+            W = np.full(N, Wv)
+            axis = np.repeat(nu[:, None], N, axis=1)
+            o = oracle_mod.Oracle(Lx, Ly, Lz, A, B, Cc, L1, mask=mask, kind=kind, W=W, axis=axis)
+            _, terms = o.energy(q, variant, terms=True)
+            ct, st = np.cos(theta), np.sin(theta)
+            if kind_id == 1:
+                W_RP = 9 * S0 ** 2 * Wv
+                expect = 0.5 * W_RP * st ** 2
+            else:
+                expect = 2.25 * S0 ** 2 * Wv * (2 * ct ** 2 - ct ** 4)
+            assert abs(terms[2] - 16 * expect) < 1e-12
+            assert abs(terms[1]) < 1e-28             # uniform field
+
+
+def test_anchoring_ignored_off_boundary(oracle_mod):
+    """only boundary-class sites carry an anchoring term: kind on a bulk site still counts only
+    if the caller put it there -- the library's rule (R9) is class==boundary && kind!=0;
+    the oracle takes kind as given, so workloads must only set kind on boundary sites."""
+    c = wl.make_replica("5")
+    f = make(oracle_mod, c).classify()
+    assert np.all((c["kind"] != 0) <= ((f & 3) == 1))
+
+
+# ------------------------------------------------------- P11: classification
+
+def test_classification_bits_small(oracle_mod):
+    mask = np.zeros((4, 4, 4), np.uint8)
+    mask[0, 0, 0] = 1
+    f = oracle_mod.Oracle(4, 4, 4, A, B, Cc, L1, mask=mask).classify().reshape(4, 4, 4)
+    assert f[0, 0, 0] & 3 == 2 and f[0, 0, 0] >> 2 == 0b111111
+    assert f[0, 0, 1] == (1 | (0b111101 << 2))      # -x neighbour is the object: bit 3 clear
+    assert f[0, 0, 3] == (1 | (0b111110 << 2))      # +x neighbour (periodic) is the object: bit 2 clear
+    assert f[0, 1, 0] == (1 | (0b110111 << 2))      # -y
+    assert f[3, 0, 0] == (1 | (0b101111 << 2))      # +z (periodic)
+    assert f[1, 0, 0] == (1 | (0b011111 << 2))      # -z
+    assert f[2, 2, 2] == (0b111111 << 2)
+    assert np.sum((f & 3) == 1) == 6 and np.sum((f & 3) == 2) == 1
+
+
+def test_classification_counts_configs(oracle_mod):
+    """integer geometry rules of DESIGN.md section 4 (counts by inclusion-exclusion / lattice-point count)"""
+    c = wl.make_config("2")
+    f = make(oracle_mod, c).classify()
+    assert np.sum((f & 3) == 2) == 20000 and np.sum((f & 3) == 1) == 20000
+    c = wl.make_replica("3")
+    f = make(oracle_mod, c).classify()
+    L = 64
+    n_wall = L ** 3 - (L - 2) ** 3
+    idx = np.arange(-L // 2, L // 2)
+    n_sph = int(np.sum(idx[:, None, None] ** 2 + idx[None, :, None] ** 2 + idx[None, None, :] ** 2 <= 36))
+    assert np.sum((f & 3) == 2) == n_wall + n_sph
+    n_wall_adj = (L - 2) ** 3 - (L - 4) ** 3
+    assert np.sum(((f & 3) == 1) & (c["W"] == 0.5)) == n_wall_adj
+    c = wl.make_replica("5")
+    f = make(oracle_mod, c).classify()
+    assert np.sum((f & 3) == 2) == 2 * 100 * 100 and np.sum((f & 3) == 1) == 2 * 100 * 100
+
+
+# ------------------------------------------------------------- P10: FIRE
+
+def _harmonic(oracle_mod, q0vec, A_h=0.8):
+    """A>0, B=C=0, no elastic: E = A/2 tr Q^2 = A (xx^2+yy^2+xx yy+xy^2+xz^2+yz^2): a harmonic
+    well; uniform field stays uniform so each site is the same 5-dof oscillator."""
+    o = oracle_mod.Oracle(4, 4, 4, A_h, 0.0, 0.0, 0.0)
+    q = np.repeat(np.asarray(q0vec, float)[:, None], 64, axis=1)
+    return o, q
+
+
+def test_fire_schedule_and_verlet_on_1dof_harmonic(oracle_mod):
+    """Only Qxy excited: 1 dof, k = 2A.  While P > 0 the mixing is a no-op (F parallel to v), so
+    FIRE is velocity Verlet with the closed-form schedule dt_n = dt0 * finc^max(0, n-Nmin) (capped),
+    alpha_n = alpha0 * falpha^max(0, n-Nmin) (Alg. 1; strict '>' per DESIGN.md R13).
+    First step closed form: x1 = x0 (1 - k dt0^2 / 2)."""
+    A_h = 0.8
+    k = 2 * A_h
+    fp = dict(wl.FIRE_PARAMS)
+    o, q = _harmonic(oracle_mod, [0, 0.3, 0, 0, 0], A_h)
+    qf, rep, tr = o.fire(q, 40, 0.0, fp, variant=0, trace=True)
+    q1, _ = o.fire(q, 1, 0.0, fp, variant=0)
+    assert abs(q1[1, 0] - 0.3 * (1 - k * fp["dt0"] ** 2 / 2)) < 1e-16
+    # independent recurrence: kick-drift-kick with the schedule applied between steps
+    x, v, dt, al, npos = 0.3, 0.0, fp["dt0"], fp["alpha0"], 0
+    for n in range(1, 41):
+        v += 0.5 * dt * (-k * x)
+        x += dt * v
+        v += 0.5 * dt * (-k * x)
+        P = -k * x * v
+        assert P > 0                                   # still falling into the well
+        npos += 1
+        if npos > fp["Nmin"]:
+            dt = min(dt * fp["finc"], fp["dtmax"])
+            al *= fp["falpha"]
+        assert abs(tr[n - 1, 0] - fp["dt0"] * fp["finc"] ** max(0, n - 5)) < 1e-15 or dt == fp["dtmax"]
+        assert abs(tr[n - 1, 0] - dt) < 1e-16 and abs(tr[n - 1, 1] - al) < 1e-15
+        assert tr[n - 1, 2] == npos
+        assert abs(tr[n - 1, 3] - 64 * P) < 1e-12 * abs(64 * P)
+    assert abs(qf[1, 0] - x) < 1e-14
+    assert tr[30, 0] == fp["dtmax"]                    # 1.1^25 > 10: capped from step 30 on
+
+
+def test_fire_uphill_reset(oracle_mod):
+    """run the 1-dof oscillator past the minimum: the first P <= 0 step halves dt, zeroes v,
+    resets alpha and Npos (Alg. 1 'else' branch)."""
+    fp = dict(wl.FIRE_PARAMS, dt0=0.05, dtmax=0.5)
+    o, q = _harmonic(oracle_mod, [0, 0.3, 0, 0, 0])
+    qf, rep, v, tr = o.fire(q, 60, 0.0, fp, variant=0, trace=True, return_v=True)
+    neg = np.where(tr[:, 3] <= 0)[0]
+    assert len(neg) > 0
+    n = neg[0]
+    assert tr[n, 2] == 0 and tr[n, 1] == fp["alpha0"]
+    assert abs(tr[n, 0] - 0.5 * tr[n - 1, 0]) < 1e-16
+    # v was zeroed at step n, so a run of exactly n+1 steps ends with v == 0
+    _, _, v_at, _ = o.fire(q, int(n) + 1, 0.0, fp, variant=0, trace=True, return_v=True)
+    assert np.abs(v_at).max() == 0.0
+
+
+def test_fire_mixing_two_modes_against_numpy(oracle_mod):
+    """Two modes of different stiffness (xy: k=2A; xx-yy: k=A) make F not parallel to v, so the
+    mixing v <- (1-a) v + a |v| F/|F| (FIRE, ref. [81] of the paper; PAPER.md:198 'rescale velocity')
+    acts.  Independent numpy restatement on the 5-vector of one site."""
+    A_h = 0.8
+    fp = dict(wl.FIRE_PARAMS, dt0=0.05, dtmax=0.2)
+    x0 = np.array([0.2, 0.3, 0.0, -0.2, 0.1])
+    o, q = _harmonic(oracle_mod, x0, A_h)
+    K = A_h * M5                                        # F = -K x
+    x, v, dt, al, npos = x0.copy(), np.zeros(5), fp["dt0"], fp["alpha0"], 0
+    nsteps = 25
+    for n in range(nsteps):
+        F = -K @ x
+        v = v + 0.5 * dt * F
+        x = x + dt * v
+        F = -K @ x
+        v = v + 0.5 * dt * F
+        P, FF, vv = F @ v, F @ F, v @ v
+        v = (1 - al) * v + al * np.sqrt(vv / FF) * F
+        if P > 0:
+            npos += 1
+            if npos > fp["Nmin"]:
+                dt = min(dt * fp["finc"], fp["dtmax"])
+                al *= fp["falpha"]
+        else:
+            npos, dt, al, v = 0, dt * fp["fdec"], fp["alpha0"], np.zeros(5)
+    qf, rep, vf = o.fire(q, nsteps, 0.0, fp, variant=1, return_v=True)
+    assert np.abs(qf[:, 0] - x).max() < 1e-14
+    assert np.abs(vf[:, 7] - v).max() < 1e-14
+    assert abs(rep["dt"] - dt) < 1e-16 and abs(rep["alpha"] - al) < 1e-16
+
+
+def test_fire_converges_to_uniform_ground_state(oracle_mod):
+    """Fig. 2: random quench in a periodic box relaxes to the uniform nematic,
+    F - F_min -> 0 with F_min = N f0 (Eq. 8).  8^3 lattice, BASELINE.json's FIRE parameters."""
+    c = wl.bulk_quench(8, 12345)
+    o = make(oracle_mod, c)
+    S0 = oracle_mod.S0_of(A, B, Cc)
+    f0 = 0.75 * A * S0 ** 2 + 0.25 * B * S0 ** 3 + 9.0 / 16.0 * Cc * S0 ** 4
+    e0 = o.energy(c["q"], 1)
+    qf, rep, tr = o.fire(c["q"], 4000, 1e-9, c["fire"], variant=1, trace=True, trace_energy=True)
+    assert rep["converged"] == 1 and rep["Fmax"] < 1e-9
+    assert abs(rep["energy"] - 512 * f0) < 1e-9
+    assert rep["energy"] < e0
+    # DESIGN.md R18: inertial, so not monotone step to step; monotone on a 100-step stride
+    E = tr[:, 7]
+    assert np.all(np.diff(E[99::100]) <= 1e-12)
+    # masked sites never move
+    c2 = wl.random_masked_problem(3, 6, 6, 6)
+    o2 = make(oracle_mod, c2)
+    q2, _ = o2.fire(c2["q"], 20, 0.0, c2["fire"], variant=1)
+    obj = c2["mask"] == 1
+    assert np.array_equal(q2[:, obj], c2["q"][:, obj])
+    assert o2.energy(q2, 1) < o2.energy(c2["q"], 1)
+
+
+def test_fire_variants_agree(oracle_mod):
+    c = wl.random_masked_problem(8, 6, 5, 7)
+    o = make(oracle_mod, c)
+    qa, ra = o.fire(c["q"], 30, 0.0, c["fire"], variant=0)
+    qb, rb = o.fire(c["q"], 30, 0.0, c["fire"], variant=1)
+    assert np.abs(qa - qb).max() < 1e-12
+    assert abs(ra["energy"] - rb["energy"]) < 1e-11 * abs(ra["energy"])
+
+
+# ------------------------------ P12: Frank-Oseen limit (the paper's L <-> K map)
+
+@pytest.mark.parametrize("L2,L3", [(0.0, 0.0), (1.0, 0.5), (0.3, -0.2)])
+def test_frank_oseen_limit_matches_printed_L_to_K_map(oracle_mod, L2, L3):
+    """Eq. 10 reduces in the uniaxial limit to Frank-Oseen with
+    L1 = 2/(27 S^2)(K3-K1+3K2), L2 = 4/(9S^2)(K1-K24), L3 = 4/(9S^2)(K24-K2), L6=0 -> K3=K1; i.e.
+    K2 = (9 S^2/2) L1 (the printed K = L1 9 S0^2/2) and K1 = K3 = (9 S^2/2)(L1+(L2+L3)/2).
+    A long-wavelength in-plane director n = (cos t, sin t, 0) varying along z is pure twist
+    (K2/2 t'^2); varying along x or y it is splay+bend (K1/2 t'^2).  Lattice error O((2 pi/L)^2)."""
+    S0 = oracle_mod.S0_of(A, B, Cc)
+    L = 64
+    K2 = 4.5 * S0 ** 2 * L1
+    K1 = 4.5 * S0 ** 2 * (L1 + 0.5 * (L2 + L3))
+    dth = 0.4 * 2 * np.pi / L * np.cos(2 * np.pi * np.arange(L) / L)
+    for ax, dims, K in (("z", (4, 4, L), K2), ("x", (L, 4, 4), K1), ("y", (4, L, 4), K1)):
+        Lx, Ly, Lz = dims
+        zz, yy, xx = np.meshgrid(np.arange(Lz), np.arange(Ly), np.arange(Lx), indexing="ij")
+        coord = {"z": zz, "x": xx, "y": yy}[ax].reshape(-1)
+        th = 0.4 * np.sin(2 * np.pi * coord / L)
+        q = wl.uniaxial_q(np.stack([np.cos(th), np.sin(th), 0 * th]), 1.5 * S0)
+        o = oracle_mod.Oracle(Lx, Ly, Lz, A, B, Cc, L1, L2, L3)
+        for v in (0, 1):
+            e_el = o.energy(q, v, terms=True)[1][1]
+            assert abs(e_el / (16 * np.sum(0.5 * K * dth ** 2)) - 1) < 3e-3
+        if ax == "z":
+            # exact lattice value for twist: each bond carries L1 q0^2 sin^2(dtheta)
+            t1 = 0.4 * np.sin(2 * np.pi * np.arange(L) / L)
+            exact = 16 * np.sum(L1 * (1.5 * S0) ** 2 * np.sin(np.roll(t1, -1) - t1) ** 2)
+            assert abs(o.energy(q, 0, terms=True)[1][1] - exact) < 1e-12

@@ -1,0 +1,159 @@
+/*
+ * lq.h -- C ABI of liblq.so: the B200 (sm_100a) hot path of lattice Landau-de Gennes
+ * Q-tensor minimisation with FIRE (arXiv:1911.07045, Sussman & Beller, "openQmin").
+ *
+ * Citations: "PAPER.md:<line>" = /root/reference/PAPER.md with the section / equation
+ * the line falls in; "DESIGN.md Rn" = reading n of a silent or garbled passage.
+ *
+ * Conventions (all calls)
+ *   - Lattice: Lx x Ly x Lz cubic lattice, spacing 1, site index s = x + Lx*(y + Ly*z),
+ *     N = Lx*Ly*Lz.  Index arithmetic is periodic in x, y and z; walls are layers of
+ *     object sites supplied through lq_set_sites (R14).
+ *   - Fields: fp64, structure of arrays [5][N], component order (xx, xy, xz, yy, yz)
+ *     (PAPER.md:173); Qzz = -Qxx - Qyy is implied.  Everything is in the paper's lattice
+ *     units (energy density / |A|-scale, lengths / lattice spacing).
+ *   - `where` says where the CALLER's buffer lives: LQ_HOST (pageable or pinned host
+ *     memory) or LQ_DEVICE (a device pointer on the context's GPU, e.g. a torch tensor's
+ *     data_ptr()).  set_* copy in, get_* / lq_forces copy out; the library never keeps a
+ *     caller pointer after the call returns.  Copies and kernels are enqueued on the
+ *     context's stream (lq_set_stream; default: the legacy default stream) and every call
+ *     that returns data to the host synchronises that stream before returning.
+ *   - Ownership: the library owns the context and every internal device buffer; the
+ *     caller owns every pointer it passes.
+ *   - Errors: every int-returning call returns LQ_OK or a negative LQ_ERR_*; nothing
+ *     throws or aborts across the ABI.  lq_last_error gives a message for the last
+ *     failing call on that context.  There is NO CPU fallback: without a usable CUDA
+ *     device lq_create fails with LQ_ERR_CUDA.
+ */
+#ifndef LQ_H
+#define LQ_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct lq_ctx lq_ctx; /* opaque; owned by the library */
+
+enum { LQ_OK = 0, LQ_ERR_ARG = -1, LQ_ERR_STATE = -2, LQ_ERR_CUDA = -3, LQ_ERR_NOMEM = -4 };
+enum { LQ_HOST = 0, LQ_DEVICE = 1 };
+enum { LQ_SITE_LC = 0, LQ_SITE_OBJECT = 1 }; /* values of the input mask */
+enum { LQ_ANCH_NONE = 0, LQ_ANCH_ORIENTED = 1 /* Eq. 14 */, LQ_ANCH_DEGENERATE_PLANAR = 2 /* Eq. 15 */ };
+
+/* packed site byte returned by lq_get_flags ("integer type"; R8):
+ *   bits 0-1: class  0 bulk, 1 boundary (simulated, >= 1 of its 6 face neighbours is an
+ *             object), 2 object (not simulated)
+ *   bit 2: site +x is simulated   bit 3: -x   bit 4: +y   bit 5: -y   bit 6: +z   bit 7: -z
+ *   (neighbour bits are set the same way at object sites). */
+enum { LQ_CLASS_BULK = 0, LQ_CLASS_BOUNDARY = 1, LQ_CLASS_OBJECT = 2 };
+
+/* Create a context for an Lx x Ly x Lz lattice with the bulk constants A, B, C of Eq. 5
+ * and the distortion constants L1, L2, L3 of Eq. 10 (L4 = L6 = 0;
+ * L2 = L3 = 0 selects the one-constant form Eq. 11).  All sites start as bulk
+ * liquid crystal with no anchoring and Q undefined.  The context computes
+ * S0 = (-B + sqrt(B^2 - 24 A C)) / (6 C) (Eq. 7) for the anchoring terms.
+ * Errors: LQ_ERR_ARG if any L < 4 or N > 2^31-1 padded sites, C <= 0 or B^2 - 24AC < 0
+ * (no nematic minimum), or out == NULL; LQ_ERR_CUDA if there is no usable sm_100 device;
+ * LQ_ERR_NOMEM if device memory cannot be allocated.  *out is set only on LQ_OK. */
+int lq_create(int Lx, int Ly, int Lz, double A, double B, double C,
+              double L1, double L2, double L3, lq_ctx **out);
+
+/* Free the context and all device memory it owns.  NULL is allowed. */
+void lq_destroy(lq_ctx *ctx);
+
+/* Use `cuda_stream` (a cudaStream_t / CUstream passed as void*, e.g.
+ * torch.cuda.current_stream().cuda_stream) for all later work.  NULL = legacy default stream. */
+int lq_set_stream(lq_ctx *ctx, void *cuda_stream);
+
+/* Geometry and anchoring: mask[N] in {LQ_SITE_LC, LQ_SITE_OBJECT};
+ * anch_kind[N] in LQ_ANCH_* (NULL = none anywhere); W[N] = the coefficient W of Eq. 14 / 15
+ * (NOT the Rapini-Papoular W_RP = 9 S0^2 W);
+ * axis[3][N] SoA unit vectors: the preferred director n0 (kind 1) or the surface normal nu
+ * (kind 2).  W and axis are read only where anch_kind != 0 and may be NULL iff anch_kind is.
+ * The library classifies every site (bulk / boundary / object + 6 neighbour bits) on the GPU.
+ * An anchoring term is applied at a site iff its class is boundary and its kind != 0, one term
+ * per site (R9).  mask == NULL resets to "all bulk".  May be called again at any time;
+ * it does not touch Q.  Errors: LQ_ERR_ARG on bad pointers / where / values > 1 in mask or > 2 in kind. */
+int lq_set_sites(lq_ctx *ctx, const uint8_t *mask, const uint8_t *anch_kind,
+                 const double *W, const double *axis, int where);
+
+/* Copy the packed class/neighbour byte of every site into flags[N] (bit-exact parity gate). */
+int lq_get_flags(lq_ctx *ctx, uint8_t *flags, int where);
+
+/* Set / read the Q field, [5][N] fp64 SoA.  lq_set_Q also resets the FIRE velocities to 0.
+ * Values at object sites are stored and returned unchanged and never enter any result
+ * (R17).  lq_get_Q before lq_set_Q: LQ_ERR_STATE. */
+int lq_set_Q(lq_ctx *ctx, const double *q, int where);
+int lq_get_Q(lq_ctx *ctx, double *q, int where);
+
+/* FIRE velocities after the last lq_fire_minimize ([5][N]; zeros after lq_set_Q). */
+int lq_get_velocity(lq_ctx *ctx, double *v, int where);
+
+/* Total free energy F = sum over simulated sites of f_bulk + f_distortion + f_anchoring
+ * (PAPER.md:175): Eq. 5; Eq. 10 averaged over the forward/backward differences allowed by the
+ * geometry; Eq. 14 / 15 at boundary sites.  *E is a HOST double.
+ * lq_energy_terms writes (bulk, distortion, anchoring) to the host array terms[3]. */
+int lq_energy(lq_ctx *ctx, double *E);
+int lq_energy_terms(lq_ctx *ctx, double *terms);
+
+/* Force F_a(x) = -dF/dq_a(x) in the five stored variables, [5][N], exactly 0 at
+ * object sites. */
+int lq_forces(lq_ctx *ctx, double *F, int where);
+
+/* FIRE parameters (Algorithm 1).  integrator must be 0 (velocity Verlet,
+ * kick-drift-kick; R4).  report_energy != 0 fills lq_fire_report.energy (one extra pass). */
+typedef struct {
+    double dt0, dtmax, alpha0, finc, fdec, falpha;
+    int Nmin;
+    int integrator;
+    int report_energy;
+} lq_fire_params;
+
+/* steps = FIRE steps taken; converged = 1 iff max|F_a| < force_tol was reached (then Q is the state
+ * that force was computed on); Fmax = max over simulated sites and components of |F_a|;
+ * Frms = sqrt(sum F^2 / N_simulated); P = F.v of the last step; dt, alpha = schedule state after the
+ * last step; energy = total energy of the final Q (0 unless report_energy);
+ * launches = kernels this call launched; sweep_launches = launches of the fused force+FIRE sweep
+ * kernel among them; gpu_ms = device time of the minimisation loop (CUDA events on the stream). */
+typedef struct {
+    long steps;
+    int converged;
+    double Fmax, Frms, P, dt, alpha, energy;
+    long launches, sweep_launches;
+    double gpu_ms;
+} lq_fire_report;
+
+/* Run FIRE from the current Q with v = 0, dt = dt0, alpha = alpha0 (state restarts every call,
+ * DESIGN.md R13) until max|F_a| < force_tol or max_steps steps.  Per step: v += dt/2 F; q += dt v;
+ * F = force(q); v += dt/2 F; P = F.v, |F|^2, |v|^2, max|F| over the simulated dofs;
+ * v <- (1-alpha) v + alpha |v| F/|F|; P > 0: after more than Nmin such steps dt <- min(dt finc, dtmax),
+ * alpha <- alpha falpha; else dt <- dt fdec, v <- 0, alpha <- alpha0 (R3).
+ * The whole loop runs on the device; the host only polls a flag.  force_tol = 0 runs exactly
+ * max_steps steps.  Errors: LQ_ERR_STATE before lq_set_Q; LQ_ERR_ARG on bad parameters
+ * (dt0 <= 0, dtmax < dt0, alpha0 outside [0,1], finc < 1, fdec or falpha outside (0,1], Nmin < 0,
+ * integrator != 0, max_steps < 0, NULL pointers). */
+int lq_fire_minimize(lq_ctx *ctx, long max_steps, double force_tol,
+                     const lq_fire_params *params, lq_fire_report *out);
+
+/* S0 of Eq. 7 for the context's A, B, C (host double). */
+int lq_get_S0(lq_ctx *ctx, double *S0);
+
+/* Tuning / introspection, not part of the method.  Keys:
+ *   "fire_path" (set): 0 = fused one-sweep-per-step kernel (default), 1 = unfused four-kernel path
+ *   "sweep_bytes_per_site" (get): algorithmic HBM bytes one sweep moves per site
+ *   "n_simulated" (get), "n_boundary" (get), "n_object" (get)
+ * Unknown key: LQ_ERR_ARG. */
+int lq_set_option(lq_ctx *ctx, const char *key, double value);
+int lq_get_info(lq_ctx *ctx, const char *key, double *value);
+
+/* Message for the last error on this context ("" if none); valid until the next call. */
+const char *lq_last_error(lq_ctx *ctx);
+
+/* Library version string, e.g. "lq 0.1 sm_100a". */
+const char *lq_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LQ_H */

@@ -1,0 +1,243 @@
+"""Thin ctypes binding of csrc/liblq.so -- the same names as include/lq.h.
+
+Argument marshalling only: every function forwards to the C ABI entry point of
+the same name; no step of the method runs in Python.  Arrays may be numpy
+arrays (host, ``LQ_HOST``) or CUDA torch tensors (``LQ_DEVICE``); they must be
+contiguous, fp64 (uint8 for mask / kind / flags).  There is no CPU fallback:
+if the library cannot be loaded or there is no B200, calls raise ``LqError``.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+LQ_OK, LQ_ERR_ARG, LQ_ERR_STATE, LQ_ERR_CUDA, LQ_ERR_NOMEM = 0, -1, -2, -3, -4
+LQ_HOST, LQ_DEVICE = 0, 1
+LQ_SITE_LC, LQ_SITE_OBJECT = 0, 1
+LQ_ANCH_NONE, LQ_ANCH_ORIENTED, LQ_ANCH_DEGENERATE_PLANAR = 0, 1, 2
+
+_LIB_PATH = os.path.join(os.path.dirname(os.path.abspath(__file__)), "csrc", "liblq.so")
+_lib = None
+
+# every symbol include/lq.h declares (checked by tests/test_abi.py against the header)
+SYMBOLS = ["lq_create", "lq_destroy", "lq_set_stream", "lq_set_sites", "lq_get_flags", "lq_set_Q", "lq_get_Q",
+           "lq_get_velocity", "lq_energy", "lq_energy_terms", "lq_forces", "lq_fire_minimize", "lq_get_S0",
+           "lq_set_option", "lq_get_info", "lq_last_error", "lq_version"]
+
+
+class LqError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__("lq error %d: %s" % (code, msg))
+        self.code = code
+
+
+class lq_fire_params(C.Structure):
+    _fields_ = [("dt0", C.c_double), ("dtmax", C.c_double), ("alpha0", C.c_double), ("finc", C.c_double),
+                ("fdec", C.c_double), ("falpha", C.c_double), ("Nmin", C.c_int), ("integrator", C.c_int),
+                ("report_energy", C.c_int)]
+
+
+class lq_fire_report(C.Structure):
+    _fields_ = [("steps", C.c_long), ("converged", C.c_int), ("Fmax", C.c_double), ("Frms", C.c_double),
+                ("P", C.c_double), ("dt", C.c_double), ("alpha", C.c_double), ("energy", C.c_double),
+                ("launches", C.c_long), ("sweep_launches", C.c_long), ("gpu_ms", C.c_double)]
+
+
+def lib_path() -> str:
+    return _LIB_PATH
+
+
+def load():
+    """dlopen liblq.so and declare the prototypes.  Raises LqError if it is missing (no fallback)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(_LIB_PATH):
+        raise LqError(LQ_ERR_CUDA, "CUDA library %s is not built (python -m paper_1911_07045_b200.build); "
+                      "there is no CPU fallback" % _LIB_PATH)
+    L = C.CDLL(_LIB_PATH)
+    vp, dp, ip = C.c_void_p, C.POINTER(C.c_double), C.c_int
+    L.lq_create.argtypes = [ip, ip, ip] + [C.c_double] * 6 + [C.POINTER(vp)]
+    L.lq_destroy.argtypes = [vp]
+    L.lq_destroy.restype = None
+    L.lq_set_stream.argtypes = [vp, vp]
+    L.lq_set_sites.argtypes = [vp, vp, vp, vp, vp, ip]
+    L.lq_get_flags.argtypes = [vp, vp, ip]
+    L.lq_set_Q.argtypes = [vp, vp, ip]
+    L.lq_get_Q.argtypes = [vp, vp, ip]
+    L.lq_get_velocity.argtypes = [vp, vp, ip]
+    L.lq_energy.argtypes = [vp, dp]
+    L.lq_energy_terms.argtypes = [vp, dp]
+    L.lq_forces.argtypes = [vp, vp, ip]
+    L.lq_fire_minimize.argtypes = [vp, C.c_long, C.c_double, C.POINTER(lq_fire_params), C.POINTER(lq_fire_report)]
+    L.lq_get_S0.argtypes = [vp, dp]
+    L.lq_set_option.argtypes = [vp, C.c_char_p, C.c_double]
+    L.lq_get_info.argtypes = [vp, C.c_char_p, dp]
+    L.lq_last_error.argtypes = [vp]
+    L.lq_last_error.restype = C.c_char_p
+    L.lq_version.restype = C.c_char_p
+    for name in SYMBOLS:
+        getattr(L, name)
+    _lib = L
+    return L
+
+
+def _buf(a, dtype, count):
+    """(pointer, where) of a numpy array or CUDA torch tensor; checks dtype, size, contiguity."""
+    if a is None:
+        return None, None
+    if isinstance(a, np.ndarray):
+        if a.dtype != dtype or not a.flags["C_CONTIGUOUS"] or a.size != count:
+            raise LqError(LQ_ERR_ARG, "array must be C-contiguous %s with %d elements" % (np.dtype(dtype).name, count))
+        return C.c_void_p(a.ctypes.data), LQ_HOST
+    # torch tensor (duck-typed so that torch is not imported for host-only use)
+    if hasattr(a, "data_ptr") and hasattr(a, "is_cuda"):
+        import torch
+        tdt = {np.dtype(np.float64): torch.float64, np.dtype(np.uint8): torch.uint8}[np.dtype(dtype)]
+        if a.dtype != tdt or not a.is_contiguous() or a.numel() != count:
+            raise LqError(LQ_ERR_ARG, "tensor must be contiguous %s with %d elements" % (tdt, count))
+        if a.is_cuda:
+            return C.c_void_p(a.data_ptr()), LQ_DEVICE
+        return C.c_void_p(a.data_ptr()), LQ_HOST      # CPU (possibly pinned) tensor
+    raise LqError(LQ_ERR_ARG, "unsupported buffer type %r" % type(a))
+
+
+def _check(ctx, rc):
+    if rc != LQ_OK:
+        raise LqError(rc, load().lq_last_error(ctx).decode())
+
+
+class lq_ctx:
+    """Opaque handle; destroyed by lq_destroy or garbage collection."""
+
+    def __init__(self, handle, dims):
+        self.handle = handle
+        self.Lx, self.Ly, self.Lz = dims
+        self.N = dims[0] * dims[1] * dims[2]
+
+    def __del__(self):
+        try:
+            lq_destroy(self)
+        except Exception:
+            pass
+
+
+def lq_version() -> str:
+    return load().lq_version().decode()
+
+
+def lq_create(Lx, Ly, Lz, A, B, Cc, L1, L2=0.0, L3=0.0) -> lq_ctx:
+    h = C.c_void_p()
+    rc = load().lq_create(int(Lx), int(Ly), int(Lz), A, B, Cc, L1, L2, L3, C.byref(h))
+    _check(None, rc)
+    return lq_ctx(h, (int(Lx), int(Ly), int(Lz)))
+
+
+def lq_destroy(ctx: lq_ctx) -> None:
+    if ctx.handle is not None and _lib is not None:
+        _lib.lq_destroy(ctx.handle)
+    ctx.handle = None
+
+
+def lq_set_stream(ctx, cuda_stream) -> None:
+    """cuda_stream: integer handle (e.g. torch.cuda.current_stream().cuda_stream) or None."""
+    _check(ctx.handle, load().lq_set_stream(ctx.handle, C.c_void_p(cuda_stream or 0)))
+
+
+def lq_set_sites(ctx, mask, anch_kind=None, W=None, axis=None) -> None:
+    N = ctx.N
+    pm, wm = _buf(mask, np.uint8, N)
+    pk, wk = _buf(anch_kind, np.uint8, N)
+    pw, ww = _buf(W, np.float64, N)
+    pa, wa = _buf(axis, np.float64, 3 * N)
+    wheres = {w for w in (wm, wk, ww, wa) if w is not None}
+    if len(wheres) > 1:
+        raise LqError(LQ_ERR_ARG, "lq_set_sites: all arrays must live in the same place")
+    where = wheres.pop() if wheres else LQ_HOST
+    _check(ctx.handle, load().lq_set_sites(ctx.handle, pm, pk, pw, pa, where))
+
+
+def lq_get_flags(ctx, out=None):
+    if out is None:
+        out = np.empty(ctx.N, dtype=np.uint8)
+    p, w = _buf(out, np.uint8, ctx.N)
+    _check(ctx.handle, load().lq_get_flags(ctx.handle, p, w))
+    return out
+
+
+def lq_set_Q(ctx, q) -> None:
+    p, w = _buf(q, np.float64, 5 * ctx.N)
+    _check(ctx.handle, load().lq_set_Q(ctx.handle, p, w))
+
+
+def _get5(fn, ctx, out):
+    if out is None:
+        out = np.empty((5, ctx.N), dtype=np.float64)
+    p, w = _buf(out, np.float64, 5 * ctx.N)
+    _check(ctx.handle, fn(ctx.handle, p, w))
+    return out
+
+
+def lq_get_Q(ctx, out=None):
+    return _get5(load().lq_get_Q, ctx, out)
+
+
+def lq_get_velocity(ctx, out=None):
+    return _get5(load().lq_get_velocity, ctx, out)
+
+
+def lq_forces(ctx, out=None):
+    return _get5(load().lq_forces, ctx, out)
+
+
+def lq_energy(ctx) -> float:
+    e = C.c_double()
+    _check(ctx.handle, load().lq_energy(ctx.handle, C.byref(e)))
+    return e.value
+
+
+def lq_energy_terms(ctx):
+    t = (C.c_double * 3)()
+    _check(ctx.handle, load().lq_energy_terms(ctx.handle, t))
+    return np.array(t[:])
+
+
+def lq_get_S0(ctx) -> float:
+    s = C.c_double()
+    _check(ctx.handle, load().lq_get_S0(ctx.handle, C.byref(s)))
+    return s.value
+
+
+def lq_set_option(ctx, key: str, value: float) -> None:
+    _check(ctx.handle, load().lq_set_option(ctx.handle, key.encode(), float(value)))
+
+
+def lq_get_info(ctx, key: str) -> float:
+    v = C.c_double()
+    _check(ctx.handle, load().lq_get_info(ctx.handle, key.encode(), C.byref(v)))
+    return v.value
+
+
+def lq_fire_minimize(ctx, max_steps, force_tol, params: dict, report_energy=False) -> dict:
+    """params: dict with dt0, dtmax, alpha0, finc, fdec, falpha, Nmin.  Returns the report as a dict."""
+    fp = lq_fire_params(params["dt0"], params["dtmax"], params["alpha0"], params["finc"], params["fdec"],
+                        params["falpha"], int(params["Nmin"]), int(params.get("integrator", 0)),
+                        int(bool(report_energy)))
+    rep = lq_fire_report()
+    _check(ctx.handle, load().lq_fire_minimize(ctx.handle, int(max_steps), float(force_tol), C.byref(fp), C.byref(rep)))
+    return {k: getattr(rep, k) for k, _ in lq_fire_report._fields_}
+
+
+def lq_last_error(ctx) -> str:
+    return load().lq_last_error(ctx.handle if ctx else None).decode()
+
+
+def create_from_config(c: dict) -> lq_ctx:
+    """Convenience for tests / bench: context + sites + Q from a workloads.* config dict (host arrays)."""
+    ctx = lq_create(c["Lx"], c["Ly"], c["Lz"], c["A"], c["B"], c["C"], c["L1"], c["L2"], c["L3"])
+    if c.get("mask") is not None:
+        lq_set_sites(ctx, c["mask"], c.get("kind"), c.get("W"), c.get("axis"))
+    lq_set_Q(ctx, np.ascontiguousarray(c["q"]))
+    return ctx

@@ -1,0 +1,425 @@
+// lq_api.cu -- the C ABI of liblq.so (include/lq.h): argument checking, device buffers,
+// host<->device marshalling and the FIRE driver loop.  No arithmetic of the method runs on
+// the host: every step of the path is a kernel in lq_kernels.cu / lq_sweep.cu.
+#include "../../include/lq.h"
+#include "lq_internal.cuh"
+#include "lq_sweep.cuh"
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+
+struct lq_ctx {
+    LqGeom g{};
+    LqPhys ph{};
+    int device = 0;
+    cudaStream_t stream = nullptr;
+    // state, padded SoA; [cur] is the live buffer, [cur^1] the sweep's output buffer
+    double *q[2] = {nullptr, nullptr}, *v[2] = {nullptr, nullptr}, *F[2] = {nullptr, nullptr};
+    int cur = 0;
+    uint8_t *maskp = nullptr, *flags = nullptr, *kind = nullptr;
+    double *W = nullptr, *axis = nullptr;
+    bool flags_active = false, anch_active = false, has_Q = false;
+    unsigned long long n_class[3] = {0, 0, 0};
+    double *partials = nullptr;
+    size_t partials_len = 0;
+    double *dscal3 = nullptr;            // 3 doubles of energy output
+    LqFireScalars *dsc = nullptr;        // 2 slots
+    unsigned long long *dcounts = nullptr;
+    int *dbad = nullptr;
+    LqSweepPlan *sweep = nullptr;
+    int fire_path = 1;
+    std::string err;
+};
+
+namespace {
+
+thread_local std::string g_noctx_err;
+
+int fail(lq_ctx *c, int code, const std::string &msg) {
+    if (c) c->err = msg;
+    else g_noctx_err = msg;
+    return code;
+}
+#define LQ_CUDA(c, call)                                                                             \
+    do {                                                                                             \
+        cudaError_t e_ = (call);                                                                     \
+        if (e_ != cudaSuccess)                                                                       \
+            return fail((c), e_ == cudaErrorMemoryAllocation ? LQ_ERR_NOMEM : LQ_ERR_CUDA,           \
+                        std::string(#call) + ": " + cudaGetErrorString(e_));                         \
+    } while (0)
+
+LqFields fields_of(const lq_ctx *c) {
+    LqFields f;
+    f.flags = c->flags_active ? c->flags : nullptr;
+    f.kind = (c->flags_active && c->anch_active) ? c->kind : nullptr;
+    f.W = c->W;
+    f.axis = c->axis;
+    return f;
+}
+
+// copy between a caller's dense [ncomp][Lz][Ly][Lx] array and a padded device array
+cudaError_t copy_box(const LqGeom &g, void *padded, const void *user, size_t elem, int ncomp, bool to_padded,
+                     cudaStream_t st) {
+    for (int c = 0; c < ncomp; ++c) {
+        cudaMemcpy3DParms p;
+        memset(&p, 0, sizeof(p));
+        cudaPitchedPtr up = make_cudaPitchedPtr((char *)user + (size_t)c * g.N * elem, g.Lx * elem, g.Lx * elem, g.Ly);
+        cudaPitchedPtr pp = make_cudaPitchedPtr((char *)padded + (size_t)c * g.NP * elem, g.Px * elem, g.Px * elem, g.Py);
+        cudaPos ppos = make_cudaPos(LQ_XO * elem, LQ_GH, LQ_GH), upos = make_cudaPos(0, 0, 0);
+        if (to_padded) { p.srcPtr = up; p.srcPos = upos; p.dstPtr = pp; p.dstPos = ppos; }
+        else           { p.srcPtr = pp; p.srcPos = ppos; p.dstPtr = up; p.dstPos = upos; }
+        p.extent = make_cudaExtent(g.Lx * elem, g.Ly, g.Lz);
+        p.kind = cudaMemcpyDefault;
+        cudaError_t e = cudaMemcpy3DAsync(&p, st);
+        if (e != cudaSuccess) return e;
+    }
+    return cudaSuccess;
+}
+
+int ensure_partials(lq_ctx *c, size_t n) {
+    if (c->partials_len >= n) return LQ_OK;
+    if (c->partials) cudaFree(c->partials);
+    c->partials = nullptr; c->partials_len = 0;
+    LQ_CUDA(c, cudaMalloc(&c->partials, n * sizeof(double)));
+    c->partials_len = n;
+    return LQ_OK;
+}
+
+int ensure_field(lq_ctx *c, double **p) {
+    if (*p) return LQ_OK;
+    LQ_CUDA(c, cudaMalloc(p, (size_t)5 * c->g.NP * sizeof(double)));
+    LQ_CUDA(c, cudaMemsetAsync(*p, 0, (size_t)5 * c->g.NP * sizeof(double), c->stream));
+    return LQ_OK;
+}
+
+bool bad_where(int w) { return w != LQ_HOST && w != LQ_DEVICE; }
+
+}  // namespace
+
+extern "C" {
+
+const char *lq_version(void) { return "lq 0.1 sm_100a"; }
+
+const char *lq_last_error(lq_ctx *ctx) { return ctx ? ctx->err.c_str() : g_noctx_err.c_str(); }
+
+int lq_create(int Lx, int Ly, int Lz, double A, double B, double C, double L1, double L2, double L3, lq_ctx **out) {
+    if (!out) return fail(nullptr, LQ_ERR_ARG, "lq_create: out is NULL");
+    *out = nullptr;
+    if (Lx < 4 || Ly < 4 || Lz < 4) return fail(nullptr, LQ_ERR_ARG, "lq_create: every lattice dimension must be >= 4");
+    if (!(C > 0.0) || !(B * B - 24.0 * A * C >= 0.0))
+        return fail(nullptr, LQ_ERR_ARG, "lq_create: need C > 0 and B^2 - 24AC >= 0 (Eq. 7 has no nematic minimum)");
+    if (!std::isfinite(A) || !std::isfinite(B) || !std::isfinite(L1) || !std::isfinite(L2) || !std::isfinite(L3))
+        return fail(nullptr, LQ_ERR_ARG, "lq_create: non-finite constant");
+    int ndev = 0;
+    cudaError_t e = cudaGetDeviceCount(&ndev);
+    if (e != cudaSuccess || ndev == 0)
+        return fail(nullptr, LQ_ERR_CUDA, std::string("lq_create: no CUDA device (there is no CPU fallback): ") +
+                                              cudaGetErrorString(e));
+    int dev = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceProp prop;
+    if (cudaGetDeviceProperties(&prop, dev) != cudaSuccess || prop.major != 10)
+        return fail(nullptr, LQ_ERR_CUDA, "lq_create: device is not sm_100 (this library is built for sm_100a only)");
+
+    lq_ctx *c = new (std::nothrow) lq_ctx();
+    if (!c) return fail(nullptr, LQ_ERR_NOMEM, "lq_create: out of host memory");
+    c->device = dev;
+    LqGeom &g = c->g;
+    g.Lx = Lx; g.Ly = Ly; g.Lz = Lz;
+    g.Px = ((LQ_XO + Lx + LQ_GH + 15) / 16) * 16;
+    g.Py = Ly + 2 * LQ_GH; g.Pz = Lz + 2 * LQ_GH;
+    g.sy = g.Px; g.sz = (long long)g.Px * g.Py;
+    g.NP = g.sz * g.Pz; g.N = (long long)Lx * Ly * Lz;
+    if (g.NP > 2147483647LL) { delete c; return fail(nullptr, LQ_ERR_ARG, "lq_create: lattice too large (padded sites > 2^31-1)"); }
+    c->ph = LqPhys{A, B, C, L1, L2, L3, (-B + sqrt(B * B - 24.0 * A * C)) / (6.0 * C)};
+    int rc = LQ_OK;
+    do {
+        if ((rc = ensure_field(c, &c->q[0])) != LQ_OK) break;
+        if (cudaMalloc(&c->dscal3, 3 * sizeof(double)) != cudaSuccess ||
+            cudaMalloc(&c->dsc, 2 * sizeof(LqFireScalars)) != cudaSuccess ||
+            cudaMalloc(&c->dcounts, 3 * sizeof(unsigned long long)) != cudaSuccess ||
+            cudaMalloc(&c->dbad, sizeof(int)) != cudaSuccess) {
+            rc = fail(nullptr, LQ_ERR_NOMEM, "lq_create: cudaMalloc failed");
+            break;
+        }
+    } while (0);
+    if (rc != LQ_OK) { std::string m = c->err.empty() ? g_noctx_err : c->err; lq_destroy(c); return fail(nullptr, rc, m); }
+    *out = c;
+    return LQ_OK;
+}
+
+void lq_destroy(lq_ctx *c) {
+    if (!c) return;
+    for (int i = 0; i < 2; ++i) { cudaFree(c->q[i]); cudaFree(c->v[i]); cudaFree(c->F[i]); }
+    cudaFree(c->maskp); cudaFree(c->flags); cudaFree(c->kind); cudaFree(c->W); cudaFree(c->axis);
+    cudaFree(c->partials); cudaFree(c->dscal3); cudaFree(c->dsc); cudaFree(c->dcounts); cudaFree(c->dbad);
+    lq_sweep_destroy(c->sweep);
+    delete c;
+}
+
+int lq_set_stream(lq_ctx *c, void *s) {
+    if (!c) return LQ_ERR_ARG;
+    c->stream = (cudaStream_t)s;
+    return LQ_OK;
+}
+
+int lq_set_sites(lq_ctx *c, const uint8_t *mask, const uint8_t *anch_kind, const double *W, const double *axis,
+                 int where) {
+    if (!c) return LQ_ERR_ARG;
+    if (bad_where(where)) return fail(c, LQ_ERR_ARG, "lq_set_sites: bad `where`");
+    if (anch_kind && (!W || !axis)) return fail(c, LQ_ERR_ARG, "lq_set_sites: anch_kind given without W / axis");
+    const LqGeom &g = c->g;
+    cudaStream_t st = c->stream;
+    lq_sweep_invalidate(c->sweep);
+    if (!mask) {
+        c->flags_active = false; c->anch_active = false;
+        c->n_class[0] = (unsigned long long)g.N; c->n_class[1] = c->n_class[2] = 0;
+        return LQ_OK;
+    }
+    if (!c->maskp) LQ_CUDA(c, cudaMalloc(&c->maskp, (size_t)g.NP));
+    if (!c->flags) LQ_CUDA(c, cudaMalloc(&c->flags, (size_t)g.NP));
+    LQ_CUDA(c, cudaMemsetAsync(c->maskp, 0, (size_t)g.NP, st));
+    LQ_CUDA(c, cudaMemsetAsync(c->flags, 0xFC, (size_t)g.NP, st));
+    LQ_CUDA(c, copy_box(g, c->maskp, mask, 1, 1, true, st));
+    LQ_CUDA(c, cudaMemsetAsync(c->dbad, 0, sizeof(int), st));
+    lq_launch_check_u8_max(g, c->maskp, 1, c->dbad, st);
+    lq_launch_fill_ghosts_u8(g, c->maskp, st);
+    lq_launch_classify(g, c->maskp, c->flags, st);
+    lq_launch_fill_ghosts_u8(g, c->flags, st);
+    LQ_CUDA(c, cudaMemsetAsync(c->dcounts, 0, 3 * sizeof(unsigned long long), st));
+    lq_launch_count_classes(g, c->flags, c->dcounts, st);
+    int bad_kind = 0;
+    if (anch_kind) {
+        if (!c->kind) LQ_CUDA(c, cudaMalloc(&c->kind, (size_t)g.NP));
+        if (!c->W) LQ_CUDA(c, cudaMalloc(&c->W, (size_t)g.NP * sizeof(double)));
+        if (!c->axis) LQ_CUDA(c, cudaMalloc(&c->axis, (size_t)3 * g.NP * sizeof(double)));
+        LQ_CUDA(c, cudaMemsetAsync(c->kind, 0, (size_t)g.NP, st));
+        LQ_CUDA(c, cudaMemsetAsync(c->W, 0, (size_t)g.NP * sizeof(double), st));
+        LQ_CUDA(c, cudaMemsetAsync(c->axis, 0, (size_t)3 * g.NP * sizeof(double), st));
+        LQ_CUDA(c, copy_box(g, c->kind, anch_kind, 1, 1, true, st));
+        LQ_CUDA(c, copy_box(g, c->W, W, sizeof(double), 1, true, st));
+        LQ_CUDA(c, copy_box(g, c->axis, axis, sizeof(double), 3, true, st));
+        int *dbad2 = c->dbad;  // reuse after reading the first result
+        int bad_mask = 0;
+        LQ_CUDA(c, cudaMemcpyAsync(&bad_mask, c->dbad, sizeof(int), cudaMemcpyDeviceToHost, st));
+        LQ_CUDA(c, cudaStreamSynchronize(st));
+        if (bad_mask) { c->flags_active = false; return fail(c, LQ_ERR_ARG, "lq_set_sites: mask value > 1"); }
+        LQ_CUDA(c, cudaMemsetAsync(dbad2, 0, sizeof(int), st));
+        lq_launch_check_u8_max(g, c->kind, 2, dbad2, st);
+        LQ_CUDA(c, cudaMemcpyAsync(&bad_kind, dbad2, sizeof(int), cudaMemcpyDeviceToHost, st));
+    } else {
+        int bad_mask = 0;
+        LQ_CUDA(c, cudaMemcpyAsync(&bad_mask, c->dbad, sizeof(int), cudaMemcpyDeviceToHost, st));
+        LQ_CUDA(c, cudaStreamSynchronize(st));
+        if (bad_mask) { c->flags_active = false; return fail(c, LQ_ERR_ARG, "lq_set_sites: mask value > 1"); }
+    }
+    LQ_CUDA(c, cudaMemcpyAsync(c->n_class, c->dcounts, 3 * sizeof(unsigned long long), cudaMemcpyDeviceToHost, st));
+    LQ_CUDA(c, cudaStreamSynchronize(st));
+    LQ_CUDA(c, cudaGetLastError());
+    if (bad_kind) { c->anch_active = false; return fail(c, LQ_ERR_ARG, "lq_set_sites: anch_kind value > 2"); }
+    c->flags_active = c->n_class[2] > 0;
+    c->anch_active = anch_kind != nullptr && c->n_class[1] > 0;
+    return LQ_OK;
+}
+
+int lq_get_flags(lq_ctx *c, uint8_t *flags, int where) {
+    if (!c) return LQ_ERR_ARG;
+    if (!flags || bad_where(where)) return fail(c, LQ_ERR_ARG, "lq_get_flags: bad argument");
+    if (!c->flags_active) {
+        if (where == LQ_HOST) memset(flags, 0xFC, (size_t)c->g.N);
+        else LQ_CUDA(c, cudaMemsetAsync(flags, 0xFC, (size_t)c->g.N, c->stream));
+    } else {
+        LQ_CUDA(c, copy_box(c->g, c->flags, flags, 1, 1, false, c->stream));
+    }
+    LQ_CUDA(c, cudaStreamSynchronize(c->stream));
+    return LQ_OK;
+}
+
+int lq_set_Q(lq_ctx *c, const double *q, int where) {
+    if (!c) return LQ_ERR_ARG;
+    if (!q || bad_where(where)) return fail(c, LQ_ERR_ARG, "lq_set_Q: bad argument");
+    LQ_CUDA(c, copy_box(c->g, c->q[c->cur], q, sizeof(double), 5, true, c->stream));
+    lq_launch_fill_ghosts_f64(c->g, c->q[c->cur], 5, c->stream);
+    if (c->v[c->cur]) LQ_CUDA(c, cudaMemsetAsync(c->v[c->cur], 0, (size_t)5 * c->g.NP * sizeof(double), c->stream));
+    LQ_CUDA(c, cudaStreamSynchronize(c->stream));
+    LQ_CUDA(c, cudaGetLastError());
+    c->has_Q = true;
+    return LQ_OK;
+}
+
+int lq_get_Q(lq_ctx *c, double *q, int where) {
+    if (!c) return LQ_ERR_ARG;
+    if (!q || bad_where(where)) return fail(c, LQ_ERR_ARG, "lq_get_Q: bad argument");
+    if (!c->has_Q) return fail(c, LQ_ERR_STATE, "lq_get_Q: no Q has been set");
+    LQ_CUDA(c, copy_box(c->g, c->q[c->cur], q, sizeof(double), 5, false, c->stream));
+    LQ_CUDA(c, cudaStreamSynchronize(c->stream));
+    return LQ_OK;
+}
+
+int lq_get_velocity(lq_ctx *c, double *v, int where) {
+    if (!c) return LQ_ERR_ARG;
+    if (!v || bad_where(where)) return fail(c, LQ_ERR_ARG, "lq_get_velocity: bad argument");
+    if (!c->has_Q) return fail(c, LQ_ERR_STATE, "lq_get_velocity: no Q has been set");
+    int rc = ensure_field(c, &c->v[c->cur]);
+    if (rc != LQ_OK) return rc;
+    LQ_CUDA(c, copy_box(c->g, c->v[c->cur], v, sizeof(double), 5, false, c->stream));
+    LQ_CUDA(c, cudaStreamSynchronize(c->stream));
+    return LQ_OK;
+}
+
+int lq_energy_terms(lq_ctx *c, double *terms) {
+    if (!c) return LQ_ERR_ARG;
+    if (!terms) return fail(c, LQ_ERR_ARG, "lq_energy_terms: terms is NULL");
+    if (!c->has_Q) return fail(c, LQ_ERR_STATE, "lq_energy: no Q has been set");
+    int rc = ensure_partials(c, (size_t)3 * lq_energy_num_blocks(c->g));
+    if (rc != LQ_OK) return rc;
+    lq_launch_energy(c->g, c->ph, fields_of(c), c->q[c->cur], c->partials, c->dscal3, c->stream);
+    LQ_CUDA(c, cudaMemcpyAsync(terms, c->dscal3, 3 * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    LQ_CUDA(c, cudaStreamSynchronize(c->stream));
+    LQ_CUDA(c, cudaGetLastError());
+    return LQ_OK;
+}
+
+int lq_energy(lq_ctx *c, double *E) {
+    if (!c) return LQ_ERR_ARG;
+    if (!E) return fail(c, LQ_ERR_ARG, "lq_energy: E is NULL");
+    double t[3];
+    int rc = lq_energy_terms(c, t);
+    if (rc != LQ_OK) return rc;
+    *E = t[0] + t[1] + t[2];
+    return LQ_OK;
+}
+
+int lq_forces(lq_ctx *c, double *F, int where) {
+    if (!c) return LQ_ERR_ARG;
+    if (!F || bad_where(where)) return fail(c, LQ_ERR_ARG, "lq_forces: bad argument");
+    if (!c->has_Q) return fail(c, LQ_ERR_STATE, "lq_forces: no Q has been set");
+    int rc = ensure_field(c, &c->F[c->cur]);
+    if (rc != LQ_OK) return rc;
+    lq_launch_forces(c->g, c->ph, fields_of(c), c->q[c->cur], c->F[c->cur], c->stream);
+    LQ_CUDA(c, copy_box(c->g, c->F[c->cur], F, sizeof(double), 5, false, c->stream));
+    LQ_CUDA(c, cudaStreamSynchronize(c->stream));
+    LQ_CUDA(c, cudaGetLastError());
+    return LQ_OK;
+}
+
+int lq_get_S0(lq_ctx *c, double *S0) {
+    if (!c || !S0) return LQ_ERR_ARG;
+    *S0 = c->ph.S0;
+    return LQ_OK;
+}
+
+int lq_set_option(lq_ctx *c, const char *key, double value) {
+    if (!c || !key) return LQ_ERR_ARG;
+    if (!strcmp(key, "fire_path")) {
+        if (value != 0.0 && value != 1.0) return fail(c, LQ_ERR_ARG, "fire_path must be 0 or 1");
+        c->fire_path = (int)value;
+        return LQ_OK;
+    }
+    return fail(c, LQ_ERR_ARG, std::string("lq_set_option: unknown key ") + key);
+}
+
+int lq_get_info(lq_ctx *c, const char *key, double *value) {
+    if (!c || !key || !value) return LQ_ERR_ARG;
+    const double nsim = (double)(c->flags_active ? c->n_class[0] + c->n_class[1] : (unsigned long long)c->g.N);
+    if (!strcmp(key, "n_simulated")) { *value = nsim; return LQ_OK; }
+    if (!strcmp(key, "n_boundary")) { *value = c->flags_active ? (double)c->n_class[1] : 0.0; return LQ_OK; }
+    if (!strcmp(key, "n_object")) { *value = c->flags_active ? (double)c->n_class[2] : 0.0; return LQ_OK; }
+    if (!strcmp(key, "sweep_bytes_per_site")) {
+        // fused sweep: read q, v, F and write q, v, F (5 fp64 each) + the flag byte where objects exist
+        *value = c->fire_path == 0 ? 240.0 + (c->flags_active ? 1.0 : 0.0) : 0.0;
+        return LQ_OK;
+    }
+    return fail(c, LQ_ERR_ARG, std::string("lq_get_info: unknown key ") + key);
+}
+
+int lq_fire_minimize(lq_ctx *c, long max_steps, double force_tol, const lq_fire_params *fp, lq_fire_report *out) {
+    if (!c) return LQ_ERR_ARG;
+    if (!fp || !out) return fail(c, LQ_ERR_ARG, "lq_fire_minimize: NULL params / report");
+    if (!c->has_Q) return fail(c, LQ_ERR_STATE, "lq_fire_minimize: no Q has been set");
+    if (!(fp->dt0 > 0.0) || !(fp->dtmax >= fp->dt0) || !(fp->alpha0 >= 0.0 && fp->alpha0 <= 1.0) ||
+        !(fp->finc >= 1.0) || !(fp->fdec > 0.0 && fp->fdec <= 1.0) || !(fp->falpha > 0.0 && fp->falpha <= 1.0) ||
+        fp->Nmin < 0 || fp->integrator != 0 || max_steps < 0 || !(force_tol >= 0.0))
+        return fail(c, LQ_ERR_ARG, "lq_fire_minimize: bad FIRE parameter");
+    memset(out, 0, sizeof(*out));
+    const LqGeom &g = c->g;
+    cudaStream_t st = c->stream;
+    int rc;
+    if ((rc = ensure_field(c, &c->v[c->cur])) != LQ_OK) return rc;
+    if ((rc = ensure_field(c, &c->F[c->cur])) != LQ_OK) return rc;
+    const bool fused = c->fire_path == 0;
+    if (fused) {
+        if ((rc = ensure_field(c, &c->q[c->cur ^ 1])) != LQ_OK) return rc;
+        if ((rc = ensure_field(c, &c->v[c->cur ^ 1])) != LQ_OK) return rc;
+        if ((rc = ensure_field(c, &c->F[c->cur ^ 1])) != LQ_OK) return rc;
+    }
+    const int nb1 = lq_fire1_num_blocks(g);
+    if ((rc = ensure_partials(c, (size_t)4 * nb1)) != LQ_OK) return rc;
+
+    LqFireConsts fc{fp->dt0, fp->dtmax, fp->alpha0, fp->finc, fp->fdec, fp->falpha, force_tol, fp->Nmin, (long long)max_steps};
+    LqFireScalars h;
+    memset(&h, 0, sizeof(h));
+    h.dt = 0.0; h.alpha = fp->alpha0; h.mix_a = 1.0; h.mix_b = 0.0;
+    LQ_CUDA(c, cudaMemcpyAsync(&c->dsc[0], &h, sizeof(h), cudaMemcpyHostToDevice, st));
+    LQ_CUDA(c, cudaMemsetAsync(c->v[c->cur], 0, (size_t)5 * g.NP * sizeof(double), st));
+    const LqFields f = fields_of(c);
+    long launches = 0, sweeps = 0;
+
+    cudaEvent_t ev0, ev1;
+    LQ_CUDA(c, cudaEventCreate(&ev0));
+    LQ_CUDA(c, cudaEventCreate(&ev1));
+    LQ_CUDA(c, cudaEventRecord(ev0, st));
+
+    // step 0: F = force(q), convergence test on the initial state (dt = 0: no kick)
+    lq_launch_fire1_force(g, c->ph, f, c->q[c->cur], c->v[c->cur], c->F[c->cur], &c->dsc[0], c->partials, st);
+    lq_launch_fire_update(c->partials, nb1, &c->dsc[0], fc, 1, st);
+    launches += 2;
+
+    long done = 0;
+    if (fused) {
+        rc = lq_sweep_run(&c->sweep, g, c->ph, f, c->q, c->v, c->F, &c->cur, c->dsc, fc, max_steps, st, &launches,
+                          &sweeps, &h, c->err);
+        if (rc != LQ_OK) { cudaEventDestroy(ev0); cudaEventDestroy(ev1); return rc; }
+    } else {
+        const long chunk = force_tol > 0.0 ? 64 : 1024;
+        while (done < max_steps) {
+            const long n = (max_steps - done) < chunk ? (max_steps - done) : chunk;
+            for (long i = 0; i < n; ++i) {
+                lq_launch_fire1_drift(g, f, c->q[c->cur], c->v[c->cur], c->F[c->cur], &c->dsc[0], st);
+                lq_launch_fill_ghosts_f64(g, c->q[c->cur], 5, st);
+                lq_launch_fire1_force(g, c->ph, f, c->q[c->cur], c->v[c->cur], c->F[c->cur], &c->dsc[0], c->partials, st);
+                lq_launch_fire_update(c->partials, nb1, &c->dsc[0], fc, 0, st);
+            }
+            launches += 4 * n;
+            done += n;
+            if (force_tol > 0.0) {
+                LQ_CUDA(c, cudaMemcpyAsync(&h, &c->dsc[0], sizeof(h), cudaMemcpyDeviceToHost, st));
+                LQ_CUDA(c, cudaStreamSynchronize(st));
+                if (h.converged) break;
+            }
+        }
+        LQ_CUDA(c, cudaMemcpyAsync(&h, &c->dsc[0], sizeof(h), cudaMemcpyDeviceToHost, st));
+    }
+    LQ_CUDA(c, cudaEventRecord(ev1, st));
+    LQ_CUDA(c, cudaStreamSynchronize(st));
+    LQ_CUDA(c, cudaGetLastError());
+    float ms = 0.f;
+    cudaEventElapsedTime(&ms, ev0, ev1);
+    cudaEventDestroy(ev0); cudaEventDestroy(ev1);
+
+    const double nsim = (double)(c->flags_active ? c->n_class[0] + c->n_class[1] : (unsigned long long)g.N);
+    out->steps = (long)h.step; out->converged = h.converged;
+    out->Fmax = h.Fmax; out->Frms = nsim > 0 ? sqrt(h.FF / nsim) : 0.0;
+    out->P = h.P; out->dt = h.dt; out->alpha = h.alpha;
+    out->launches = launches; out->sweep_launches = sweeps; out->gpu_ms = ms;
+    if (fp->report_energy) {
+        rc = lq_energy(c, &out->energy);
+        if (rc != LQ_OK) return rc;
+    }
+    return LQ_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,79 @@
+// lq_internal.cuh -- shared declarations of the CUDA library (not part of the ABI).
+//
+// HBM layout.  Every per-site array lives in a PADDED box with a
+// ghost shell of width LQ_GH that mirrors the periodic images, so no kernel does modular
+// index arithmetic and TMA boxes with halos never wrap:
+//     p(x,y,z) = (x + LQ_XO) + Px * ((y + LQ_GH) + Py * (z + LQ_GH))
+// Px = roundup(LQ_XO + Lx + LQ_GH, 16): row starts and the first interior element of each
+// row are 128-byte aligned; the low-x ghosts sit in the LQ_GH elements before it.
+// Fields are SoA: component c of a 5-component field starts at c * NP.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+constexpr int LQ_GH = 2;   // ghost width in x, y and z
+constexpr int LQ_XO = 16;  // element offset of x = 0 inside a padded row (128 B for fp64)
+
+struct LqGeom {
+    int Lx, Ly, Lz;
+    int Px, Py, Pz;
+    long long sy, sz;  // strides (elements) of +y and +z in the padded box
+    long long NP;      // padded sites per component
+    long long N;       // Lx*Ly*Lz
+    __host__ __device__ inline long long pidx(int x, int y, int z) const {
+        return (long long)(x + LQ_XO) + sy * (long long)(y + LQ_GH) + sz * (long long)(z + LQ_GH);
+    }
+};
+
+struct LqPhys {
+    double A, B, C, L1, L2, L3, S0;
+};
+
+// FIRE state that lives on the device (Algorithm 1).
+// mix_a, mix_b: the velocity rescale of the step just reduced, v <- mix_a*v + mix_b*F
+// (mix_a = 1-alpha, mix_b = alpha*|v|/|F|; both 0 after a P <= 0 reset), applied lazily
+// by the next sweep.  dt is the step size of the NEXT step.
+struct LqFireScalars {
+    double dt, alpha;
+    double mix_a, mix_b;
+    double P, FF, vv, Fmax;
+    long long step;  // steps completed
+    int npos;
+    int converged;
+};
+
+struct LqFireConsts {
+    double dt0, dtmax, alpha0, finc, fdec, falpha, force_tol;
+    int Nmin;
+    long long max_steps;
+};
+
+struct LqFields {
+    // padded device arrays; any of flags/kind/W/axis may be null (no objects / no anchoring)
+    const uint8_t *flags;
+    const uint8_t *kind;
+    const double *W;
+    const double *axis;  // [3][NP]
+};
+
+// ---- generic kernels (lq_kernels.cu) ----------------------------------------------------
+void lq_launch_fill_ghosts_f64(const LqGeom &g, double *field, int ncomp, cudaStream_t st);
+void lq_launch_fill_ghosts_u8(const LqGeom &g, uint8_t *field, cudaStream_t st);
+void lq_launch_classify(const LqGeom &g, const uint8_t *mask_p, uint8_t *flags_p, cudaStream_t st);
+void lq_launch_count_classes(const LqGeom &g, const uint8_t *flags_p, unsigned long long *counts3, cudaStream_t st);
+void lq_launch_check_u8_max(const LqGeom &g, const uint8_t *arr_p, int maxval, int *bad, cudaStream_t st);
+void lq_launch_forces(const LqGeom &g, const LqPhys &ph, const LqFields &f, const double *q, double *F, cudaStream_t st);
+// energy: partial sums per block into partials (3 per block) then final reduce into out3 (device)
+int lq_energy_num_blocks(const LqGeom &g);
+void lq_launch_energy(const LqGeom &g, const LqPhys &ph, const LqFields &f, const double *q,
+                      double *partials, double *out3, cudaStream_t st);
+
+// unfused FIRE path (fire_path = 1): 4 launches per step
+int lq_fire1_num_blocks(const LqGeom &g);
+void lq_launch_fire1_drift(const LqGeom &g, const LqFields &f, double *q, double *v, const double *F,
+                           const LqFireScalars *sc, cudaStream_t st);
+void lq_launch_fire1_force(const LqGeom &g, const LqPhys &ph, const LqFields &f, const double *q, double *v,
+                           double *F, const LqFireScalars *sc, double *partials, cudaStream_t st);
+void lq_launch_fire_update(const double *partials, int nblocks, LqFireScalars *sc_in_out, LqFireConsts fc,
+                           int first, cudaStream_t st);
+void lq_launch_zero_object_sites(const LqGeom &g, const uint8_t *flags, double *field, cudaStream_t st);

@@ -1,0 +1,342 @@
+// lq_kernels.cu -- generic kernels: ghost refresh, site classification, force field,
+// energy, and the unfused FIRE path (fire_path = 1).  One thread per lattice site, global
+// loads through L1/L2.  These serve lq_set_sites / lq_forces / lq_energy and are the
+// cross-check for the fused sweep (lq_sweep.cu), which is the product's hot path.
+#include "lq_internal.cuh"
+#include "lq_site.cuh"
+
+namespace {
+
+constexpr int BX = 64, BY = 4;      // block shape for per-site kernels
+constexpr int ZPER = 8;             // z planes per block
+
+__device__ __forceinline__ int wrap(int i, int L) { return i < 0 ? i + L : (i >= L ? i - L : i); }
+
+// ---- ghost shell refresh: every padded cell outside the interior copies its periodic image
+template <typename T>
+__global__ void k_fill_ghosts(LqGeom g, T *field, int ncomp) {
+    const int px = blockIdx.x * blockDim.x + threadIdx.x;  // 0 .. Lx+2GH-1 -> x = px - GH
+    const int py = blockIdx.y * blockDim.y + threadIdx.y;
+    const int pz = blockIdx.z;
+    if (px >= g.Lx + 2 * LQ_GH || py >= g.Py) return;
+    const int x = px - LQ_GH, y = py - LQ_GH, z = pz - LQ_GH;
+    if (x >= 0 && x < g.Lx && y >= 0 && y < g.Ly && z >= 0 && z < g.Lz) return;
+    const long long dst = g.pidx(x, y, z);
+    const long long src = g.pidx(wrap(x, g.Lx), wrap(y, g.Ly), wrap(z, g.Lz));
+    for (int c = 0; c < ncomp; ++c) field[c * g.NP + dst] = field[c * g.NP + src];
+}
+
+// ---- classification (R8).  mask_p has its ghost shell filled.
+__global__ void k_classify(LqGeom g, const uint8_t *__restrict__ mask_p, uint8_t *__restrict__ flags_p) {
+    const int x = blockIdx.x * blockDim.x + threadIdx.x;
+    const int y = blockIdx.y * blockDim.y + threadIdx.y;
+    const int z = blockIdx.z;
+    if (x >= g.Lx || y >= g.Ly) return;
+    const long long p = g.pidx(x, y, z);
+    const long long off[6] = {1, -1, g.sy, -g.sy, g.sz, -g.sz};
+    unsigned f = 0, any_obj = 0;
+#pragma unroll
+    for (int b = 0; b < 6; ++b) {
+        const unsigned sim = mask_p[p + off[b]] == 0;
+        f |= sim << (2 + b);
+        any_obj |= !sim;
+    }
+    const unsigned cls = mask_p[p] != 0 ? 2u : (any_obj ? 1u : 0u);
+    flags_p[p] = (uint8_t)(f | cls);
+}
+
+__global__ void k_count_classes(LqGeom g, const uint8_t *__restrict__ flags_p, unsigned long long *counts) {
+    const int x = blockIdx.x * blockDim.x + threadIdx.x;
+    const int y = blockIdx.y * blockDim.y + threadIdx.y;
+    const int z = blockIdx.z;
+    __shared__ unsigned c[3];
+    const int tid = threadIdx.y * blockDim.x + threadIdx.x;
+    if (tid < 3) c[tid] = 0;
+    __syncthreads();
+    if (x < g.Lx && y < g.Ly) atomicAdd(&c[flags_p[g.pidx(x, y, z)] & 3u], 1u);
+    __syncthreads();
+    if (tid < 3 && c[tid]) atomicAdd(&counts[tid], (unsigned long long)c[tid]);
+}
+
+__global__ void k_check_u8_max(LqGeom g, const uint8_t *__restrict__ a, int maxval, int *bad) {
+    const int x = blockIdx.x * blockDim.x + threadIdx.x;
+    const int y = blockIdx.y * blockDim.y + threadIdx.y;
+    const int z = blockIdx.z;
+    if (x < g.Lx && y < g.Ly && a[g.pidx(x, y, z)] > maxval) *bad = 1;
+}
+
+__device__ __forceinline__ void load_anchor(const LqFields &f, long long NP, long long p, unsigned fl, int &kind,
+                                            double &W, double n[3]) {
+    kind = 0; W = 0.0; n[0] = n[1] = n[2] = 0.0;
+    if (f.kind != nullptr && (fl & 3u) == 1u) {
+        kind = f.kind[p];
+        if (kind != 0) { W = f.W[p]; n[0] = f.axis[p]; n[1] = f.axis[NP + p]; n[2] = f.axis[2 * NP + p]; }
+    }
+}
+
+// ---- force field (lq_forces)
+template <bool THREE>
+__global__ void __launch_bounds__(BX * BY) k_forces(LqGeom g, LqPhys ph, LqFields f, const double *__restrict__ q,
+                                                    double *__restrict__ F) {
+    const int x = blockIdx.x * BX + threadIdx.x;
+    const int y = blockIdx.y * BY + threadIdx.y;
+    if (x >= g.Lx || y >= g.Ly) return;
+    for (int z = blockIdx.z * ZPER; z < min(g.Lz, (int)(blockIdx.z + 1) * ZPER); ++z) {
+        const long long p = g.pidx(x, y, z);
+        const unsigned fl = f.flags ? f.flags[p] : 0xFCu;
+        double Fs[5] = {0, 0, 0, 0, 0};
+        if ((fl & 3u) != 2u) {
+            int kind; double W, n[3];
+            load_anchor(f, g.NP, p, fl, kind, W, n);
+            lqs::GlobalAcc acc{q, f.flags, g.NP, g.sy, g.sz, p};
+            lqs::site_force<THREE>(ph, acc, fl, kind, W, n, Fs);
+        }
+#pragma unroll
+        for (int c = 0; c < 5; ++c) F[c * g.NP + p] = Fs[c];
+    }
+}
+
+// ---- block reduction helpers (fixed order -> bitwise reproducible)
+__device__ __forceinline__ double warp_sum(double v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+    return v;
+}
+__device__ __forceinline__ double warp_max(double v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v = fmax(v, __shfl_down_sync(0xffffffffu, v, o));
+    return v;
+}
+
+template <int NV, int NT>
+__device__ __forceinline__ void block_reduce(double (&val)[NV], int nsum, double *out) {
+    // first nsum entries are summed, the rest are max-reduced; result written by thread 0
+    __shared__ double sm[NV][NT / 32];
+    const int tid = threadIdx.y * blockDim.x + threadIdx.x;
+    const int lane = tid & 31, wid = tid >> 5;
+#pragma unroll
+    for (int i = 0; i < NV; ++i) {
+        const double r = i < nsum ? warp_sum(val[i]) : warp_max(val[i]);
+        if (lane == 0) sm[i][wid] = r;
+    }
+    __syncthreads();
+    if (tid == 0) {
+#pragma unroll
+        for (int i = 0; i < NV; ++i) {
+            double r = sm[i][0];
+            for (int w = 1; w < NT / 32; ++w) r = i < nsum ? r + sm[i][w] : fmax(r, sm[i][w]);
+            out[i] = r;
+        }
+    }
+}
+
+// ---- energy
+template <bool THREE>
+__global__ void __launch_bounds__(BX * BY) k_energy(LqGeom g, LqPhys ph, LqFields f, const double *__restrict__ q,
+                                                    double *__restrict__ partials) {
+    const int x = blockIdx.x * BX + threadIdx.x;
+    const int y = blockIdx.y * BY + threadIdx.y;
+    double acc3[3] = {0, 0, 0};
+    if (x < g.Lx && y < g.Ly) {
+        for (int z = blockIdx.z * ZPER; z < min(g.Lz, (int)(blockIdx.z + 1) * ZPER); ++z) {
+            const long long p = g.pidx(x, y, z);
+            const unsigned fl = f.flags ? f.flags[p] : 0xFCu;
+            if ((fl & 3u) == 2u) continue;
+            int kind; double W, n[3], t[3];
+            load_anchor(f, g.NP, p, fl, kind, W, n);
+            lqs::GlobalAcc acc{q, f.flags, g.NP, g.sy, g.sz, p};
+            lqs::site_energy<THREE>(ph, acc, fl, kind, W, n, t);
+            acc3[0] += t[0]; acc3[1] += t[1]; acc3[2] += t[2];
+        }
+    }
+    const long long b = blockIdx.x + (long long)gridDim.x * (blockIdx.y + (long long)gridDim.y * blockIdx.z);
+    block_reduce<3, BX * BY>(acc3, 3, partials + 3 * b);
+}
+
+// final reduce: one block, fixed order, Neumaier-compensated per thread then tree
+template <int NV>
+__global__ void __launch_bounds__(256) k_final_sum(const double *__restrict__ partials, long long nblocks,
+                                                   double *__restrict__ out) {
+    double s[NV], c[NV];
+#pragma unroll
+    for (int i = 0; i < NV; ++i) { s[i] = 0.0; c[i] = 0.0; }
+    for (long long b = threadIdx.x; b < nblocks; b += 256) {
+#pragma unroll
+        for (int i = 0; i < NV; ++i) {
+            const double v = partials[NV * b + i];
+            const double t = s[i] + v;
+            c[i] += fabs(s[i]) >= fabs(v) ? (s[i] - t) + v : (v - t) + s[i];
+            s[i] = t;
+        }
+    }
+#pragma unroll
+    for (int i = 0; i < NV; ++i) s[i] += c[i];
+    block_reduce<NV, 256>(s, NV, out);
+}
+
+// ---- unfused FIRE (fire_path = 1)  Algorithm 1
+// drift: v <- mix_a v + mix_b F (the rescale decided by the previous step's reductions);
+//        v += dt/2 F; q += dt v          (simulated sites only)
+__global__ void __launch_bounds__(BX * BY) k_fire1_drift(LqGeom g, LqFields f, double *__restrict__ q,
+                                                         double *__restrict__ v, const double *__restrict__ F,
+                                                         const LqFireScalars *__restrict__ sc) {
+    if (sc->converged) return;
+    const int x = blockIdx.x * BX + threadIdx.x;
+    const int y = blockIdx.y * BY + threadIdx.y;
+    if (x >= g.Lx || y >= g.Ly) return;
+    const double dt = sc->dt, ma = sc->mix_a, mb = sc->mix_b;
+    for (int z = blockIdx.z * ZPER; z < min(g.Lz, (int)(blockIdx.z + 1) * ZPER); ++z) {
+        const long long p = g.pidx(x, y, z);
+        if (f.flags && (f.flags[p] & 3u) == 2u) continue;
+#pragma unroll
+        for (int c = 0; c < 5; ++c) {
+            const long long i = c * g.NP + p;
+            const double Fc = F[i];
+            double vc = ma * v[i] + mb * Fc;
+            vc += 0.5 * dt * Fc;
+            v[i] = vc;
+            q[i] += dt * vc;
+        }
+    }
+}
+
+// force + second half kick + partial reductions of P = F.v, |F|^2, |v|^2, max|F_a|
+template <bool THREE>
+__global__ void __launch_bounds__(BX * BY) k_fire1_force(LqGeom g, LqPhys ph, LqFields f,
+                                                         const double *__restrict__ q, double *__restrict__ v,
+                                                         double *__restrict__ F, const LqFireScalars *__restrict__ sc,
+                                                         double *__restrict__ partials) {
+    if (sc->converged) return;
+    const int x = blockIdx.x * BX + threadIdx.x;
+    const int y = blockIdx.y * BY + threadIdx.y;
+    const double hdt = 0.5 * sc->dt;
+    double r[4] = {0, 0, 0, 0};
+    if (x < g.Lx && y < g.Ly) {
+        for (int z = blockIdx.z * ZPER; z < min(g.Lz, (int)(blockIdx.z + 1) * ZPER); ++z) {
+            const long long p = g.pidx(x, y, z);
+            const unsigned fl = f.flags ? f.flags[p] : 0xFCu;
+            double Fs[5] = {0, 0, 0, 0, 0};
+            const bool sim = (fl & 3u) != 2u;
+            if (sim) {
+                int kind; double W, n[3];
+                load_anchor(f, g.NP, p, fl, kind, W, n);
+                lqs::GlobalAcc acc{q, f.flags, g.NP, g.sy, g.sz, p};
+                lqs::site_force<THREE>(ph, acc, fl, kind, W, n, Fs);
+            }
+#pragma unroll
+            for (int c = 0; c < 5; ++c) {
+                const long long i = c * g.NP + p;
+                F[i] = Fs[c];
+                if (sim) {
+                    const double vc = v[i] + hdt * Fs[c];
+                    v[i] = vc;
+                    r[0] += Fs[c] * vc; r[1] += Fs[c] * Fs[c]; r[2] += vc * vc; r[3] = fmax(r[3], fabs(Fs[c]));
+                }
+            }
+        }
+    }
+    const long long b = blockIdx.x + (long long)gridDim.x * (blockIdx.y + (long long)gridDim.y * blockIdx.z);
+    block_reduce<4, BX * BY>(r, 3, partials + 4 * b);
+}
+
+// One block: reduce the per-block partials in a fixed order, then advance the FIRE schedule.
+// first != 0: this is the initial force evaluation (step 0): only the convergence test applies.
+__global__ void __launch_bounds__(256) k_fire_update(const double *__restrict__ partials, int nblocks,
+                                                     LqFireScalars *sc, LqFireConsts fc, int first) {
+    if (sc->converged) return;
+    double s[4] = {0, 0, 0, 0};
+    for (int b = threadIdx.x; b < nblocks; b += 256) {
+        s[0] += partials[4 * b]; s[1] += partials[4 * b + 1]; s[2] += partials[4 * b + 2];
+        s[3] = fmax(s[3], partials[4 * b + 3]);
+    }
+    __shared__ double tot[4];
+    block_reduce<4, 256>(s, 3, tot);
+    __syncthreads();
+    if (threadIdx.x != 0) return;
+    LqFireScalars t = *sc;
+    t.P = tot[0]; t.FF = tot[1]; t.vv = tot[2]; t.Fmax = tot[3];
+    if (first) t.dt = fc.dt0;   // the initial force evaluation ran with dt = 0 (no kick)
+    else t.step += 1;
+    if (t.Fmax < fc.force_tol) {
+        t.converged = 1;
+    } else if (!first) {
+        if (t.FF > 0.0) { t.mix_a = 1.0 - t.alpha; t.mix_b = t.alpha * sqrt(t.vv / t.FF); }
+        else { t.mix_a = 1.0; t.mix_b = 0.0; }
+        if (t.P > 0.0) {
+            t.npos += 1;
+            if (t.npos > fc.Nmin) { t.dt = fmin(t.dt * fc.finc, fc.dtmax); t.alpha *= fc.falpha; }
+        } else {
+            t.npos = 0; t.dt *= fc.fdec; t.alpha = fc.alpha0; t.mix_a = 0.0; t.mix_b = 0.0;
+        }
+    }
+    *sc = t;
+}
+
+__global__ void k_zero_object_sites(LqGeom g, const uint8_t *__restrict__ flags, double *__restrict__ field) {
+    const int x = blockIdx.x * blockDim.x + threadIdx.x;
+    const int y = blockIdx.y * blockDim.y + threadIdx.y;
+    const int z = blockIdx.z;
+    if (x >= g.Lx || y >= g.Ly) return;
+    const long long p = g.pidx(x, y, z);
+    if ((flags[p] & 3u) == 2u)
+        for (int c = 0; c < 5; ++c) field[c * g.NP + p] = 0.0;
+}
+
+inline dim3 site_grid(const LqGeom &g) {
+    return dim3((g.Lx + BX - 1) / BX, (g.Ly + BY - 1) / BY, (g.Lz + ZPER - 1) / ZPER);
+}
+inline dim3 plane_grid(const LqGeom &g) { return dim3((g.Lx + BX - 1) / BX, (g.Ly + BY - 1) / BY, g.Lz); }
+
+}  // namespace
+
+void lq_launch_fill_ghosts_f64(const LqGeom &g, double *field, int ncomp, cudaStream_t st) {
+    dim3 b(64, 4), gr((g.Lx + 2 * LQ_GH + 63) / 64, (g.Py + 3) / 4, g.Pz);
+    k_fill_ghosts<double><<<gr, b, 0, st>>>(g, field, ncomp);
+}
+void lq_launch_fill_ghosts_u8(const LqGeom &g, uint8_t *field, cudaStream_t st) {
+    dim3 b(64, 4), gr((g.Lx + 2 * LQ_GH + 63) / 64, (g.Py + 3) / 4, g.Pz);
+    k_fill_ghosts<uint8_t><<<gr, b, 0, st>>>(g, field, 1);
+}
+void lq_launch_classify(const LqGeom &g, const uint8_t *mask_p, uint8_t *flags_p, cudaStream_t st) {
+    k_classify<<<plane_grid(g), dim3(BX, BY), 0, st>>>(g, mask_p, flags_p);
+}
+void lq_launch_count_classes(const LqGeom &g, const uint8_t *flags_p, unsigned long long *counts3, cudaStream_t st) {
+    k_count_classes<<<plane_grid(g), dim3(BX, BY), 0, st>>>(g, flags_p, counts3);
+}
+void lq_launch_check_u8_max(const LqGeom &g, const uint8_t *arr_p, int maxval, int *bad, cudaStream_t st) {
+    k_check_u8_max<<<plane_grid(g), dim3(BX, BY), 0, st>>>(g, arr_p, maxval, bad);
+}
+void lq_launch_forces(const LqGeom &g, const LqPhys &ph, const LqFields &f, const double *q, double *F,
+                      cudaStream_t st) {
+    if (ph.L2 != 0.0 || ph.L3 != 0.0) k_forces<true><<<site_grid(g), dim3(BX, BY), 0, st>>>(g, ph, f, q, F);
+    else k_forces<false><<<site_grid(g), dim3(BX, BY), 0, st>>>(g, ph, f, q, F);
+}
+int lq_energy_num_blocks(const LqGeom &g) {
+    dim3 gr = site_grid(g);
+    return (int)(gr.x * gr.y * gr.z);
+}
+void lq_launch_energy(const LqGeom &g, const LqPhys &ph, const LqFields &f, const double *q, double *partials,
+                      double *out3, cudaStream_t st) {
+    if (ph.L2 != 0.0 || ph.L3 != 0.0) k_energy<true><<<site_grid(g), dim3(BX, BY), 0, st>>>(g, ph, f, q, partials);
+    else k_energy<false><<<site_grid(g), dim3(BX, BY), 0, st>>>(g, ph, f, q, partials);
+    k_final_sum<3><<<1, 256, 0, st>>>(partials, lq_energy_num_blocks(g), out3);
+}
+int lq_fire1_num_blocks(const LqGeom &g) { return lq_energy_num_blocks(g); }
+void lq_launch_fire1_drift(const LqGeom &g, const LqFields &f, double *q, double *v, const double *F,
+                           const LqFireScalars *sc, cudaStream_t st) {
+    k_fire1_drift<<<site_grid(g), dim3(BX, BY), 0, st>>>(g, f, q, v, F, sc);
+}
+void lq_launch_fire1_force(const LqGeom &g, const LqPhys &ph, const LqFields &f, const double *q, double *v,
+                           double *F, const LqFireScalars *sc, double *partials, cudaStream_t st) {
+    if (ph.L2 != 0.0 || ph.L3 != 0.0)
+        k_fire1_force<true><<<site_grid(g), dim3(BX, BY), 0, st>>>(g, ph, f, q, v, F, sc, partials);
+    else
+        k_fire1_force<false><<<site_grid(g), dim3(BX, BY), 0, st>>>(g, ph, f, q, v, F, sc, partials);
+}
+void lq_launch_fire_update(const double *partials, int nblocks, LqFireScalars *sc, LqFireConsts fc, int first,
+                           cudaStream_t st) {
+    k_fire_update<<<1, 256, 0, st>>>(partials, nblocks, sc, fc, first);
+}
+void lq_launch_zero_object_sites(const LqGeom &g, const uint8_t *flags, double *field, cudaStream_t st) {
+    k_zero_object_sites<<<plane_grid(g), dim3(BX, BY), 0, st>>>(g, flags, field);
+}

@@ -1,0 +1,274 @@
+// lq_site.cuh -- per-site Landau-de Gennes arithmetic in GATHER form (device functions).
+//
+// The force on the five stored variables of site x is assembled from the 3x3 gradient
+// G_ab = dF/dQ_ab (entries treated as independent), F = -(Gxx-Gzz, Gxy+Gyx, Gxz+Gzx,
+// Gyy-Gzz, Gyz+Gzy).  Derivation of every piece: DESIGN.md section 6.
+//   bulk      Eq. 5:   G = (A + C tr Q^2) Q + B Q^2
+//   elastic   Eq. 10 averaged over the allowed forward/backward differences
+//             (PAPER.md:177-183).  With a^s_k(y) = "y + s k is simulated",
+//             w_k(y) = 1/(a+_k + a-_k) (0 if none), Dbar_k = w_k * sum_s a^s_k D^s_k:
+//       same-axis:  G_ab(x) -= sum_k (L1 + (L2+L3) d_bk) sum_s a^s_k(x) [w_k(x) + w_k(x+s k)] (Q_ab(x+s k) - Q_ab(x))
+//       mixed:      H^(c)_ab(y) = L2 d_bc sum_{m!=c} Dbar_m Q_am(y) + L3 (1-d_bc) Dbar_b Q_ac(y)
+//                   G_ab(x) += sum_c { w_c(x)(a-_c(x) - a+_c(x)) H^(c)_ab(x)
+//                                      + a-_c(x) w_c(x-c) H^(c)_ab(x-c) - a+_c(x) w_c(x+c) H^(c)_ab(x+c) }
+//   anchoring Eq. 14: G += 2W (Q - Q0), Q0 = 3/2 S0 (n n - I/3)
+//             Eq. 15: G += 2W M, M = Qt - P Qt P, Qt = Q + S0/2 I, P = I - nu nu
+// An accessor type supplies Q (6 numbers xx,xy,xz,yy,yz,zz) and the flag byte at small
+// offsets from the site, so the same code serves global-memory and shared-memory tiles.
+#pragma once
+#include "lq_internal.cuh"
+
+namespace lqs {
+
+__device__ __forceinline__ int m6(int a, int b) {
+    // index of tensor entry (a,b) in (xx,xy,xz,yy,yz,zz)
+    return a == b ? (a == 0 ? 0 : (a == 1 ? 3 : 5)) : (a + b == 1 ? 1 : (a + b == 2 ? 2 : 4));
+}
+__device__ __forceinline__ int a_plus(unsigned fl, int k) { return (fl >> (2 + 2 * k)) & 1u; }
+__device__ __forceinline__ int a_minus(unsigned fl, int k) { return (fl >> (3 + 2 * k)) & 1u; }
+__device__ __forceinline__ double w_axis(unsigned fl, int k) {
+    const int n = a_plus(fl, k) + a_minus(fl, k);
+    return n == 2 ? 0.5 : (n == 1 ? 1.0 : 0.0);
+}
+
+// accessor over padded global arrays, centred on padded index p
+struct GlobalAcc {
+    const double *q;
+    const uint8_t *flags;  // may be null: every site bulk with all neighbours simulated
+    long long NP, sy, sz, p;
+    __device__ __forceinline__ void Q(int dx, int dy, int dz, double o[6]) const {
+        const long long i = p + dx + dy * sy + dz * sz;
+        o[0] = q[i]; o[1] = q[NP + i]; o[2] = q[2 * NP + i]; o[3] = q[3 * NP + i]; o[4] = q[4 * NP + i];
+        o[5] = -o[0] - o[3];
+    }
+    __device__ __forceinline__ unsigned flag(int dx, int dy, int dz) const {
+        return flags ? (unsigned)flags[p + dx + dy * sy + dz * sz] : 0xFCu;
+    }
+};
+
+__device__ __forceinline__ void off3(int k, int s, int &dx, int &dy, int &dz) {
+    dx = k == 0 ? s : 0; dy = k == 1 ? s : 0; dz = k == 2 ? s : 0;
+}
+
+// Dbar_m Q at the site at offset (ox,oy,oz), whose flag byte is fl and tensor is Qy
+template <class Acc>
+__device__ __forceinline__ void dbar(const Acc &acc, int ox, int oy, int oz, unsigned fl, const double Qy[6],
+                                     int m, double out[6]) {
+    const int ap = a_plus(fl, m), am = a_minus(fl, m);
+    const double w = w_axis(fl, m);
+    int dx, dy, dz;
+    double t[6];
+#pragma unroll
+    for (int i = 0; i < 6; ++i) out[i] = 0.0;
+    if (ap) {
+        off3(m, +1, dx, dy, dz);
+        acc.Q(ox + dx, oy + dy, oz + dz, t);
+#pragma unroll
+        for (int i = 0; i < 6; ++i) out[i] += t[i] - Qy[i];
+    }
+    if (am) {
+        off3(m, -1, dx, dy, dz);
+        acc.Q(ox + dx, oy + dy, oz + dz, t);
+#pragma unroll
+        for (int i = 0; i < 6; ++i) out[i] += Qy[i] - t[i];
+    }
+#pragma unroll
+    for (int i = 0; i < 6; ++i) out[i] *= w;
+}
+
+__device__ __forceinline__ void bulk_G(const LqPhys &ph, const double Q[6], double G[3][3]) {
+    const double a = Q[0], b = Q[1], c = Q[2], d = Q[3], e = Q[4], f = Q[5];
+    const double q2xx = a * a + b * b + c * c, q2xy = a * b + b * d + c * e, q2xz = a * c + b * e + c * f;
+    const double q2yy = b * b + d * d + e * e, q2yz = b * c + d * e + e * f, q2zz = c * c + e * e + f * f;
+    const double k = ph.A + ph.C * (q2xx + q2yy + q2zz);
+    G[0][0] = k * a + ph.B * q2xx; G[0][1] = G[1][0] = k * b + ph.B * q2xy; G[0][2] = G[2][0] = k * c + ph.B * q2xz;
+    G[1][1] = k * d + ph.B * q2yy; G[1][2] = G[2][1] = k * e + ph.B * q2yz; G[2][2] = k * f + ph.B * q2zz;
+}
+
+__device__ __forceinline__ double bulk_E(const LqPhys &ph, const double Q[6]) {
+    const double a = Q[0], b = Q[1], c = Q[2], d = Q[3], e = Q[4], f = Q[5];
+    const double q2xx = a * a + b * b + c * c, q2xy = a * b + b * d + c * e, q2xz = a * c + b * e + c * f;
+    const double q2yy = b * b + d * d + e * e, q2yz = b * c + d * e + e * f, q2zz = c * c + e * e + f * f;
+    const double tr2 = q2xx + q2yy + q2zz;
+    const double tr3 = q2xx * a + q2yy * d + q2zz * f + 2.0 * (q2xy * b + q2xz * c + q2yz * e);
+    return 0.5 * ph.A * tr2 + ph.B * (1.0 / 3.0) * tr3 + 0.25 * ph.C * tr2 * tr2;
+}
+
+// anchoring: adds to G (if G != nullptr) and returns the energy
+__device__ __forceinline__ double anchoring(const LqPhys &ph, int kind, double W, const double n[3],
+                                            const double Q[6], double (*G)[3]) {
+    double e = 0.0;
+    if (kind == 1) {
+        const double q0 = 1.5 * ph.S0;
+#pragma unroll
+        for (int a = 0; a < 3; ++a)
+#pragma unroll
+            for (int b = 0; b < 3; ++b) {
+                const double d = Q[m6(a, b)] - q0 * (n[a] * n[b] - (a == b ? 1.0 / 3.0 : 0.0));
+                e += W * d * d;
+                if (G) G[a][b] += 2.0 * W * d;
+            }
+    } else if (kind == 2) {
+        // M = Qt - P Qt P with P = I - nu nu:  M = nu u^T + u nu^T - s nu nu^T, u = Qt nu, s = nu.Qt.nu
+        double u[3];
+        const double h = 0.5 * ph.S0;
+#pragma unroll
+        for (int a = 0; a < 3; ++a)
+            u[a] = Q[m6(a, 0)] * n[0] + Q[m6(a, 1)] * n[1] + Q[m6(a, 2)] * n[2] + h * n[a];
+        const double s = u[0] * n[0] + u[1] * n[1] + u[2] * n[2];
+#pragma unroll
+        for (int a = 0; a < 3; ++a)
+#pragma unroll
+            for (int b = 0; b < 3; ++b) {
+                const double M = n[a] * u[b] + u[a] * n[b] - s * n[a] * n[b];
+                e += W * M * M;
+                if (G) G[a][b] += 2.0 * W * M;
+            }
+    }
+    return e;
+}
+
+__device__ __forceinline__ void G_to_F(const double G[3][3], double F[5]) {
+    F[0] = -(G[0][0] - G[2][2]);
+    F[1] = -(G[0][1] + G[1][0]);
+    F[2] = -(G[0][2] + G[2][0]);
+    F[3] = -(G[1][1] - G[2][2]);
+    F[4] = -(G[1][2] + G[2][1]);
+}
+
+// Force on a simulated site in the general (masked, L1/L2/L3, anchored) case.
+// fl = the site's flag byte; akind/W/n = its anchoring record (akind 0 if none).
+template <bool THREE, class Acc>
+__device__ __forceinline__ void site_force(const LqPhys &ph, const Acc &acc, unsigned fl, int akind, double W,
+                                           const double n[3], double F[5]) {
+    double Qx[6], G[3][3];
+    acc.Q(0, 0, 0, Qx);
+    bulk_G(ph, Qx, G);
+    if ((fl & 3u) == 1u && akind != 0) anchoring(ph, akind, W, n, Qx, G);
+    const double L23 = ph.L2 + ph.L3;
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+        const double wx = w_axis(fl, k);
+#pragma unroll
+        for (int s = +1; s >= -1; s -= 2) {
+            const int allowed = s > 0 ? a_plus(fl, k) : a_minus(fl, k);
+            if (!allowed) continue;
+            int dx, dy, dz;
+            off3(k, s, dx, dy, dz);
+            const unsigned fn = acc.flag(dx, dy, dz);
+            const double coef = wx + w_axis(fn, k);
+            double Qn[6];
+            acc.Q(dx, dy, dz, Qn);
+#pragma unroll
+            for (int a = 0; a < 3; ++a)
+#pragma unroll
+                for (int b = 0; b < 3; ++b) {
+                    const double cab = ph.L1 + ((THREE && b == k) ? L23 : 0.0);
+                    G[a][b] -= cab * coef * (Qn[m6(a, b)] - Qx[m6(a, b)]);
+                }
+        }
+    }
+    if (THREE) {
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            const int m1 = (c + 1) % 3, m2 = (c + 2) % 3;
+#pragma unroll
+            for (int t = 0; t < 3; ++t) {
+                // t = 0: y = x;  t = 1: y = x - c;  t = 2: y = x + c
+                int ox = 0, oy = 0, oz = 0;
+                double coef;
+                unsigned fy;
+                if (t == 0) {
+                    coef = w_axis(fl, c) * (double)(a_minus(fl, c) - a_plus(fl, c));
+                    fy = fl;
+                } else {
+                    const int s = t == 1 ? -1 : +1;
+                    const int allowed = s > 0 ? a_plus(fl, c) : a_minus(fl, c);
+                    if (!allowed) continue;
+                    off3(c, s, ox, oy, oz);
+                    fy = acc.flag(ox, oy, oz);
+                    coef = (s > 0 ? -1.0 : 1.0) * w_axis(fy, c);
+                }
+                if (coef == 0.0) continue;
+                double Qy[6], D1[6], D2[6];
+                acc.Q(ox, oy, oz, Qy);
+                dbar(acc, ox, oy, oz, fy, Qy, m1, D1);
+                dbar(acc, ox, oy, oz, fy, Qy, m2, D2);
+#pragma unroll
+                for (int a = 0; a < 3; ++a) {
+                    G[a][c] += coef * ph.L2 * (D1[m6(a, m1)] + D2[m6(a, m2)]);
+                    G[a][m1] += coef * ph.L3 * D1[m6(a, c)];
+                    G[a][m2] += coef * ph.L3 * D2[m6(a, c)];
+                }
+            }
+        }
+    }
+    G_to_F(G, F);
+}
+
+// Energy of one simulated site: terms = (bulk, distortion, anchoring)
+template <bool THREE, class Acc>
+__device__ __forceinline__ void site_energy(const LqPhys &ph, const Acc &acc, unsigned fl, int akind, double W,
+                                            const double n[3], double terms[3]) {
+    double Qx[6];
+    acc.Q(0, 0, 0, Qx);
+    terms[0] = bulk_E(ph, Qx);
+    terms[2] = ((fl & 3u) == 1u && akind != 0) ? anchoring(ph, akind, W, n, Qx, nullptr) : 0.0;
+    const double L23 = ph.L2 + ph.L3;
+    double ed = 0.0;
+    double Db[3][6];
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+        const double w = w_axis(fl, k);
+#pragma unroll
+        for (int i = 0; i < 6; ++i) Db[k][i] = 0.0;
+#pragma unroll
+        for (int s = +1; s >= -1; s -= 2) {
+            const int allowed = s > 0 ? a_plus(fl, k) : a_minus(fl, k);
+            if (!allowed) continue;
+            int dx, dy, dz;
+            off3(k, s, dx, dy, dz);
+            double Qn[6], D[6];
+            acc.Q(dx, dy, dz, Qn);
+#pragma unroll
+            for (int i = 0; i < 6; ++i) {
+                D[i] = s > 0 ? Qn[i] - Qx[i] : Qx[i] - Qn[i];
+                Db[k][i] += w * D[i];
+            }
+            const double fro = D[0] * D[0] + D[3] * D[3] + D[5] * D[5] + 2.0 * (D[1] * D[1] + D[2] * D[2] + D[4] * D[4]);
+            ed += 0.5 * ph.L1 * w * fro;
+            if (THREE) {
+                const double col = D[m6(0, k)] * D[m6(0, k)] + D[m6(1, k)] * D[m6(1, k)] + D[m6(2, k)] * D[m6(2, k)];
+                ed += 0.5 * L23 * w * col;
+            }
+        }
+    }
+    if (THREE) {
+#pragma unroll
+        for (int j = 0; j < 3; ++j)
+#pragma unroll
+            for (int k = j + 1; k < 3; ++k)
+#pragma unroll
+                for (int i = 0; i < 3; ++i) {
+                    ed += ph.L2 * Db[j][m6(i, j)] * Db[k][m6(i, k)];
+                    ed += ph.L3 * Db[j][m6(i, k)] * Db[k][m6(i, j)];
+                }
+    }
+    terms[1] = ed;
+}
+
+// one-constant, pure-bulk neighbourhood: F from the centre tensor and the 7-point Laplacian
+// lap[c] = sum over the 6 neighbours of (q_c(nbr) - q_c(x))      (Eq. 11)
+__device__ __forceinline__ void bulk_force_oneconst(const LqPhys &ph, const double q5[5], const double lap[5],
+                                                    double F[5]) {
+    double Q[6] = {q5[0], q5[1], q5[2], q5[3], q5[4], -q5[0] - q5[3]};
+    double G[3][3];
+    bulk_G(ph, Q, G);
+    F[0] = -(G[0][0] - G[2][2]) + ph.L1 * (2.0 * lap[0] + lap[3]);
+    F[1] = -2.0 * G[0][1] + 2.0 * ph.L1 * lap[1];
+    F[2] = -2.0 * G[0][2] + 2.0 * ph.L1 * lap[2];
+    F[3] = -(G[1][1] - G[2][2]) + ph.L1 * (2.0 * lap[3] + lap[0]);
+    F[4] = -2.0 * G[1][2] + 2.0 * ph.L1 * lap[4];
+}
+
+}  // namespace lqs

@@ -1,0 +1,16 @@
+// lq_sweep.cuh -- interface of the fused force + FIRE sweep (lq_sweep.cu), the hot path.
+#pragma once
+#include "lq_internal.cuh"
+#include <string>
+
+struct LqSweepPlan;  // tensor maps, per-CTA partials, tile classification; owned by the context
+
+void lq_sweep_destroy(LqSweepPlan *plan);
+void lq_sweep_invalidate(LqSweepPlan *plan);  // geometry / anchoring arrays changed
+
+// Runs up to max_steps FIRE steps, one kernel launch per step.  On entry buffer *cur holds
+// (q, v = 0, F = force(q)) with q's ghost shell valid and dsc[0] the scalars after the step-0
+// update.  On return *cur is the buffer holding the final state, *h the final scalars.
+int lq_sweep_run(LqSweepPlan **plan, const LqGeom &g, const LqPhys &ph, const LqFields &f, double *q[2],
+                 double *v[2], double *F[2], int *cur, LqFireScalars *dsc, const LqFireConsts &fc, long max_steps,
+                 cudaStream_t st, long *launches, long *sweeps, LqFireScalars *h, std::string &err);

@@ -30,7 +30,7 @@ struct lq_ctx {
     unsigned long long *dcounts = nullptr;
     int *dbad = nullptr;
     LqSweepPlan *sweep = nullptr;
-    int fire_path = 1;
+    int fire_path = 0;
     std::string err;
 };
 

@@ -13,6 +13,7 @@
 
 constexpr int LQ_GH = 2;   // ghost width in x, y and z
 constexpr int LQ_XO = 16;  // element offset of x = 0 inside a padded row (128 B for fp64)
+constexpr int LQ_GW = 1;   // ghost width the FIRE kernels keep up to date (stencil radius)
 
 struct LqGeom {
     int Lx, Ly, Lz;
@@ -47,6 +48,27 @@ struct LqFireConsts {
     int Nmin;
     long long max_steps;
 };
+
+// Reductions of one step -> schedule of the next (Algorithm 1; readings
+// DESIGN.md R3, R12, R13).  tot = (P, |F|^2, |v|^2, max|F_a|).  first != 0: the initial force
+// evaluation (ran with dt = 0, no kick): only the convergence test applies.
+__host__ __device__ inline void lq_fire_advance(LqFireScalars &t, const LqFireConsts &fc, const double tot[4], int first) {
+    t.P = tot[0]; t.FF = tot[1]; t.vv = tot[2]; t.Fmax = tot[3];
+    if (first) t.dt = fc.dt0;
+    else t.step += 1;
+    if (t.Fmax < fc.force_tol) {
+        t.converged = 1;
+    } else if (!first) {
+        if (t.FF > 0.0) { t.mix_a = 1.0 - t.alpha; t.mix_b = t.alpha * sqrt(t.vv / t.FF); }
+        else { t.mix_a = 1.0; t.mix_b = 0.0; }
+        if (t.P > 0.0) {
+            t.npos += 1;
+            if (t.npos > fc.Nmin) { t.dt = fmin(t.dt * fc.finc, fc.dtmax); t.alpha *= fc.falpha; }
+        } else {
+            t.npos = 0; t.dt *= fc.fdec; t.alpha = fc.alpha0; t.mix_a = 0.0; t.mix_b = 0.0;
+        }
+    }
+}
 
 struct LqFields {
     // padded device arrays; any of flags/kind/W/axis may be null (no objects / no anchoring)

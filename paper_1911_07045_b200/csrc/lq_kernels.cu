@@ -254,21 +254,7 @@ __global__ void __launch_bounds__(256) k_fire_update(const double *__restrict__ 
     __syncthreads();
     if (threadIdx.x != 0) return;
     LqFireScalars t = *sc;
-    t.P = tot[0]; t.FF = tot[1]; t.vv = tot[2]; t.Fmax = tot[3];
-    if (first) t.dt = fc.dt0;   // the initial force evaluation ran with dt = 0 (no kick)
-    else t.step += 1;
-    if (t.Fmax < fc.force_tol) {
-        t.converged = 1;
-    } else if (!first) {
-        if (t.FF > 0.0) { t.mix_a = 1.0 - t.alpha; t.mix_b = t.alpha * sqrt(t.vv / t.FF); }
-        else { t.mix_a = 1.0; t.mix_b = 0.0; }
-        if (t.P > 0.0) {
-            t.npos += 1;
-            if (t.npos > fc.Nmin) { t.dt = fmin(t.dt * fc.finc, fc.dtmax); t.alpha *= fc.falpha; }
-        } else {
-            t.npos = 0; t.dt *= fc.fdec; t.alpha = fc.alpha0; t.mix_a = 0.0; t.mix_b = 0.0;
-        }
-    }
+    lq_fire_advance(t, fc, tot, first);
     *sc = t;
 }
 

@@ -1,12 +1,478 @@
-// lq_sweep.cu -- placeholder until the fused sweep lands
+// lq_sweep.cu -- the hot path: ONE kernel launch per FIRE step (sm_100a).
+//
+// State carried between steps is (q, vc, F): the Q field, the velocity after the second
+// half-kick (before the rescale), and the force at q.  Step n+1, per site
+// (Algorithm 1):
+//     v_m = mix_a vc + mix_b F                    velocity rescale decided by step n's reductions
+//     v_k = v_m + dt/2 F ;  q' = q + dt v_k       half kick + drift
+//     F'  = force(q')                             bulk + elastic stencil + anchoring (fused)
+//     vc' = v_k + dt/2 F'                         second half kick
+//     partial sums of F'.vc', |F'|^2, |vc'|^2, max|F'_a|
+// q' of a site is a pointwise function of that site's (q, vc, F) and three global scalars, so a CTA
+// recomputes q' on its tile PLUS a one-site halo from TMA-staged boxes of the three input fields and
+// never needs a neighbour CTA's output: no second pass, no grid barrier.  The last CTA to finish
+// reduces the per-CTA partials in a fixed order and advances the FIRE schedule on the device.
+//
+// Tiling: CTA = TX x TY columns marching over a z-chunk.  Per plane, one elected thread issues three
+// 4-D TMA box loads ((TX+4) x (TY+2) x 1 x 5 components) into a 2-stage mbarrier ring; all threads turn
+// the landed plane into q' (own site + a share of the halo ring) in a 3-plane shared-memory ring; the
+// force for plane k then reads its in-plane neighbours from shared memory and its z neighbours from
+// registers.  Outputs go straight from registers to global memory with coalesced 256-byte rows; sites
+// on the lattice faces also refresh the periodic ghost shell of the output buffers.
 #include "lq_sweep.cuh"
+#include "lq_site.cuh"
 #include "../../include/lq.h"
-struct LqSweepPlan { int dummy; };
-void lq_sweep_destroy(LqSweepPlan *p) { delete p; }
+
+#include <cuda.h>
+#include <cstdio>
+#include <cstring>
+
+namespace {
+
+template <int TX_, int TY_>
+struct Cfg {
+    static constexpr int TX = TX_, TY = TY_, NT = TX_ * TY_;
+    static constexpr int BXW = TX_ + 2, BYH = TY_ + 2;      // q' ring: tile + 1 halo
+    static constexpr int PLANE = BXW * BYH;                 // elements of one component plane of the ring
+    static constexpr int RING_STRIDE = (5 * PLANE * 8 + 127) / 128 * 128;
+    // TMA box: the start coordinate of the innermost dimension must be 16-byte aligned (measured: an odd
+    // fp64 start coordinate traps with "illegal instruction"), so the staged box starts at x0-2, not x0-1.
+    static constexpr int SW = TX_ + 4;                      // staged box width: x0-2 .. x0+TX+1
+    static constexpr int SPLANE = SW * BYH;
+    static constexpr int FIELD_BYTES = 5 * SPLANE * 8;      // one TMA box
+    static constexpr int FIELD_STRIDE = (FIELD_BYTES + 127) / 128 * 128;
+    static constexpr int NSTAGE = 2, RING = 3;
+    static constexpr int STAGE_BYTES = 3 * FIELD_STRIDE;
+    static constexpr int OFF_RING = NSTAGE * STAGE_BYTES;
+    static constexpr int OFF_BAR = OFF_RING + RING * RING_STRIDE;
+    static constexpr int OFF_RED = OFF_BAR + 64;
+    static constexpr int SMEM_BYTES = OFF_RED + 4 * (NT / 32) * 8 + 64;
+    static constexpr int NHALO = 2 * BXW + 2 * (BYH - 2);
+};
+
+struct SweepArgs {
+    LqGeom g;
+    LqPhys ph;
+    LqFields f;
+    double *qo, *vo, *Fo;
+    LqFireScalars *sc;
+    LqFireConsts fc;
+    double *partials;
+    unsigned int *counter;
+    int zc;
+};
+
+// ---------------------------------------------------------------- PTX wrappers (TMA + mbarrier)
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint64_t *bar, int count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_LOOP:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra WAIT_DONE;\n"
+        "bra WAIT_LOOP;\n"
+        "WAIT_DONE:\n"
+        "}\n" ::"r"(smem_u32(bar)),
+        "r"(parity)
+        : "memory");
+}
+__device__ __forceinline__ void tma_load_4d(void *dst, const CUtensorMap *map, uint64_t *bar, int c0, int c1, int c2,
+                                            int c3) {
+    asm volatile(
+        "cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5, %6}], [%2];"
+        ::"r"(smem_u32(dst)), "l"(map), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2), "r"(c3)
+        : "memory");
+}
+
+__device__ __forceinline__ double warp_sum(double v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+    return v;
+}
+__device__ __forceinline__ double warp_max(double v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v = fmax(v, __shfl_down_sync(0xffffffffu, v, o));
+    return v;
+}
+
+// accessor over the shared-memory ring of q' planes (k-1, k, k+1); flags come from global memory
+template <class C>
+struct RingAcc {
+    const double *pl[3];
+    int idx;
+    const uint8_t *flags;
+    long long sy, sz, p;
+    __device__ __forceinline__ void Q(int dx, int dy, int dz, double o[6]) const {
+        const double *b = pl[dz + 1] + idx + dy * C::BXW + dx;
+        o[0] = b[0]; o[1] = b[C::PLANE]; o[2] = b[2 * C::PLANE]; o[3] = b[3 * C::PLANE]; o[4] = b[4 * C::PLANE];
+        o[5] = -o[0] - o[3];
+    }
+    __device__ __forceinline__ unsigned flag(int dx, int dy, int dz) const {
+        return flags ? (unsigned)flags[p + dx + dy * sy + dz * sz] : 0xFCu;
+    }
+};
+
+// q' and v_k of one site from its staged (q, vc, F): the SAME instruction sequence for a CTA's own
+// sites and for the halo copies its neighbours compute, so every CTA sees bit-identical q'.
+__device__ __forceinline__ void drift(double q, double vc, double F, double ma, double cF, double dt, double &vk,
+                                      double &qn) {
+    vk = __fma_rn(ma, vc, cF * F);
+    qn = __fma_rn(dt, vk, q);
+}
+
+template <class C, bool THREE, bool MASKED>
+__global__ void __launch_bounds__(C::NT, 1)
+k_sweep(const __grid_constant__ CUtensorMap tq, const __grid_constant__ CUtensorMap tv,
+        const __grid_constant__ CUtensorMap tF, const SweepArgs a) {
+    extern __shared__ __align__(1024) unsigned char smem[];
+    constexpr bool TWO_SYNC = THREE || MASKED;   // the general force reads ring plane k-1 too
+    const LqFireScalars sc = *a.sc;
+    if (sc.converged) return;
+
+    uint64_t *full = reinterpret_cast<uint64_t *>(smem + C::OFF_BAR);
+    double *red = reinterpret_cast<double *>(smem + C::OFF_RED);
+    const int tid = threadIdx.x;
+    const int tx = tid % C::TX, ty = tid / C::TX;
+    const int x0 = blockIdx.x * C::TX, y0 = blockIdx.y * C::TY;
+    const int zb = blockIdx.z * a.zc, ze = min(a.g.Lz, zb + a.zc);
+    const int x = x0 + tx, y = y0 + ty;
+    const bool active = x < a.g.Lx && y < a.g.Ly;
+    const int nplanes = ze - zb + 2;             // planes zb-1 .. ze
+    const long long NP = a.g.NP;
+
+    if (tid == 0) {
+        mbar_init(&full[0], 1);
+        mbar_init(&full[1], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+
+    auto issue = [&](int j) {
+        const int s = j & 1;
+        unsigned char *st = smem + s * C::STAGE_BYTES;
+        const int cx = x0 + LQ_XO - 2, cy = y0 + LQ_GH - 1, cz = zb - 1 + j + LQ_GH;
+        mbar_expect_tx(&full[s], 3u * C::FIELD_BYTES);
+        tma_load_4d(st, &tq, &full[s], cx, cy, cz, 0);
+        tma_load_4d(st + C::FIELD_STRIDE, &tv, &full[s], cx, cy, cz, 0);
+        tma_load_4d(st + 2 * C::FIELD_STRIDE, &tF, &full[s], cx, cy, cz, 0);
+    };
+    if (tid == 0) {
+        issue(0);
+        if (nplanes > 1) issue(1);
+    }
+
+    const double dt = sc.dt, ma = sc.mix_a, cF = sc.mix_b + 0.5 * sc.dt, hdt = 0.5 * sc.dt;
+    double qm[5], qc[5], qp[5], vk0[5], vk1[5];
+#pragma unroll
+    for (int c = 0; c < 5; ++c) qm[c] = qc[c] = qp[c] = vk0[c] = vk1[c] = 0.0;
+    double r[4] = {0.0, 0.0, 0.0, 0.0};
+    const int idx = (ty + 1) * C::BXW + tx + 1;    // own site in a ring plane
+    const int sidx = (ty + 1) * C::SW + tx + 2;    // own site in a staged box
+
+    // halo share of this thread: perimeter cell h of the (TX+2) x (TY+2) box
+    int hidx = -1, hsidx = -1;
+    if (tid < C::NHALO) {
+        int h = tid, hx, hy;
+        if (h < C::BXW) { hx = h; hy = 0; }
+        else if (h < 2 * C::BXW) { hx = h - C::BXW; hy = C::BYH - 1; }
+        else { h -= 2 * C::BXW; hy = 1 + (h >> 1); hx = (h & 1) ? C::BXW - 1 : 0; }
+        hidx = hy * C::BXW + hx;
+        hsidx = hy * C::SW + hx + 1;
+    }
+
+    for (int j = 0; j < nplanes; ++j) {
+        const int s = j & 1;
+        mbar_wait(&full[s], (j >> 1) & 1);
+        const double *sq = reinterpret_cast<const double *>(smem + s * C::STAGE_BYTES);
+        const double *sv = sq + C::FIELD_STRIDE / 8, *sF = sq + 2 * (C::FIELD_STRIDE / 8);
+        double *rn = reinterpret_cast<double *>(smem + C::OFF_RING + (j % 3) * C::RING_STRIDE);
+
+        // ---- [A] plane z = zb-1+j: q' on tile + halo into the ring; own column into registers
+#pragma unroll
+        for (int c = 0; c < 5; ++c) {
+            qm[c] = qc[c]; qc[c] = qp[c]; vk0[c] = vk1[c];
+            drift(sq[c * C::SPLANE + sidx], sv[c * C::SPLANE + sidx], sF[c * C::SPLANE + sidx], ma, cF, dt, vk1[c], qp[c]);
+            rn[c * C::PLANE + idx] = qp[c];
+        }
+        if (hidx >= 0) {
+#pragma unroll
+            for (int c = 0; c < 5; ++c) {
+                double vk, qn;
+                drift(sq[c * C::SPLANE + hsidx], sv[c * C::SPLANE + hsidx], sF[c * C::SPLANE + hsidx], ma, cF, dt, vk, qn);
+                rn[c * C::PLANE + hidx] = qn;
+            }
+        }
+        __syncthreads();
+        if (tid == 0 && j + 2 < nplanes) issue(j + 2);   // stage s has been consumed by every thread
+
+        // ---- [B] force, second half kick, reductions and stores for plane k = zb + j - 2
+        if (j >= 2 && active) {
+            const int k = zb + j - 2;
+            const double *rk = reinterpret_cast<const double *>(smem + C::OFF_RING + ((j - 1) % 3) * C::RING_STRIDE);
+            const long long p = a.g.pidx(x, y, k);
+            double Fn[5] = {0.0, 0.0, 0.0, 0.0, 0.0}, vn[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
+            unsigned fl = 0xFCu;
+            bool plain = true;                    // bulk site whose 6 neighbours see only simulated sites
+            if (MASKED) {
+                fl = a.f.flags[p];
+                plain = (fl >> 2) == 0x3Fu && (a.f.flags[p + 1] >> 2) == 0x3Fu && (a.f.flags[p - 1] >> 2) == 0x3Fu &&
+                        (a.f.flags[p + a.g.sy] >> 2) == 0x3Fu && (a.f.flags[p - a.g.sy] >> 2) == 0x3Fu &&
+                        (a.f.flags[p + a.g.sz] >> 2) == 0x3Fu && (a.f.flags[p - a.g.sz] >> 2) == 0x3Fu &&
+                        (fl & 3u) == 0u;
+            }
+            const bool sim = (fl & 3u) != 2u;
+            if (sim) {
+                if (!THREE && plain) {
+                    double lap[5];
+#pragma unroll
+                    for (int c = 0; c < 5; ++c) {
+                        const double *b = rk + c * C::PLANE + idx;
+                        lap[c] = ((b[-1] + b[1]) + (b[-C::BXW] + b[C::BXW]) + (qm[c] + qp[c])) - 6.0 * qc[c];
+                    }
+                    lqs::bulk_force_oneconst(a.ph, qc, lap, Fn);
+                } else {
+                    RingAcc<C> acc;
+                    acc.pl[0] = reinterpret_cast<const double *>(smem + C::OFF_RING + ((j - 2) % 3) * C::RING_STRIDE);
+                    acc.pl[1] = rk;
+                    acc.pl[2] = rn;
+                    acc.idx = idx; acc.flags = MASKED ? a.f.flags : nullptr;
+                    acc.sy = a.g.sy; acc.sz = a.g.sz; acc.p = p;
+                    int kind = 0; double W = 0.0, n[3] = {0.0, 0.0, 0.0};
+                    if (MASKED && a.f.kind != nullptr && (fl & 3u) == 1u) {
+                        kind = a.f.kind[p];
+                        if (kind != 0) { W = a.f.W[p]; n[0] = a.f.axis[p]; n[1] = a.f.axis[NP + p]; n[2] = a.f.axis[2 * NP + p]; }
+                    }
+                    lqs::site_force<THREE>(a.ph, acc, fl, kind, W, n, Fn);
+                }
+#pragma unroll
+                for (int c = 0; c < 5; ++c) {
+                    vn[c] = __fma_rn(hdt, Fn[c], vk0[c]);
+                    r[0] = __fma_rn(Fn[c], vn[c], r[0]);
+                    r[1] = __fma_rn(Fn[c], Fn[c], r[1]);
+                    r[2] = __fma_rn(vn[c], vn[c], r[2]);
+                    r[3] = fmax(r[3], fabs(Fn[c]));
+                }
+            }
+#pragma unroll
+            for (int c = 0; c < 5; ++c) {
+                a.qo[c * NP + p] = qc[c];
+                a.vo[c * NP + p] = vn[c];
+                a.Fo[c * NP + p] = Fn[c];
+            }
+            // periodic ghost shell of the outputs (width LQ_GW)
+            const int shx = x < LQ_GW ? a.g.Lx : (x >= a.g.Lx - LQ_GW ? -a.g.Lx : 0);
+            const int shy = y < LQ_GW ? a.g.Ly : (y >= a.g.Ly - LQ_GW ? -a.g.Ly : 0);
+            const int shz = k < LQ_GW ? a.g.Lz : (k >= a.g.Lz - LQ_GW ? -a.g.Lz : 0);
+            if (shx | shy | shz) {
+                for (int m = 1; m < 8; ++m) {
+                    if (((m & 1) && !shx) || ((m & 2) && !shy) || ((m & 4) && !shz)) continue;
+                    const long long pg = p + ((m & 1) ? shx : 0) + ((m & 2) ? shy * a.g.sy : 0) + ((m & 4) ? shz * a.g.sz : 0);
+#pragma unroll
+                    for (int c = 0; c < 5; ++c) {
+                        a.qo[c * NP + pg] = qc[c];
+                        a.vo[c * NP + pg] = vn[c];
+                        a.Fo[c * NP + pg] = Fn[c];
+                    }
+                }
+            }
+        }
+        if (TWO_SYNC) __syncthreads();
+    }
+
+    // ---- per-CTA partials, then the last CTA reduces all of them in index order and advances FIRE
+    const int lane = tid & 31, wid = tid >> 5;
+    constexpr int NW = C::NT / 32;
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        const double w = i < 3 ? warp_sum(r[i]) : warp_max(r[i]);
+        if (lane == 0) red[i * NW + wid] = w;
+    }
+    __syncthreads();
+    __shared__ unsigned s_last;
+    const unsigned ncta = gridDim.x * gridDim.y * gridDim.z;
+    const unsigned cta = blockIdx.x + gridDim.x * (blockIdx.y + gridDim.y * blockIdx.z);
+    if (tid == 0) {
+        double t[4];
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            t[i] = red[i * NW];
+            for (int w = 1; w < NW; ++w) t[i] = i < 3 ? t[i] + red[i * NW + w] : fmax(t[i], red[i * NW + w]);
+            a.partials[4 * cta + i] = t[i];
+        }
+        __threadfence();
+        s_last = atomicAdd(a.counter, 1u) == ncta - 1 ? 1u : 0u;
+    }
+    __syncthreads();
+    if (!s_last) return;
+    __threadfence();
+    double t[4] = {0.0, 0.0, 0.0, 0.0};
+    for (unsigned b = tid; b < ncta; b += C::NT) {
+        t[0] += __ldcg(a.partials + 4 * b); t[1] += __ldcg(a.partials + 4 * b + 1); t[2] += __ldcg(a.partials + 4 * b + 2);
+        t[3] = fmax(t[3], __ldcg(a.partials + 4 * b + 3));
+    }
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        const double w = i < 3 ? warp_sum(t[i]) : warp_max(t[i]);
+        if (lane == 0) red[i * NW + wid] = w;
+    }
+    __syncthreads();
+    if (tid == 0) {
+        double tot[4];
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            tot[i] = red[i * NW];
+            for (int w = 1; w < NW; ++w) tot[i] = i < 3 ? tot[i] + red[i * NW + w] : fmax(tot[i], red[i * NW + w]);
+        }
+        LqFireScalars nx = sc;
+        lq_fire_advance(nx, a.fc, tot, 0);
+        *a.sc = nx;
+        *a.counter = 0u;
+    }
+}
+
+// ---------------------------------------------------------------- host side
+typedef CUresult (*PFN_encodeTiled)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                    const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
+                                    CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+PFN_encodeTiled get_encode() {
+    static PFN_encodeTiled fn = nullptr;
+    if (fn) return fn;
+    void *p = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) != cudaSuccess ||
+        q != cudaDriverEntryPointSuccess)
+        return nullptr;
+    fn = (PFN_encodeTiled)p;
+    return fn;
+}
+
+bool make_map(CUtensorMap *m, const LqGeom &g, double *base, int bxw, int byh) {
+    PFN_encodeTiled enc = get_encode();
+    if (!enc) return false;
+    cuuint64_t dims[4] = {(cuuint64_t)g.Px, (cuuint64_t)g.Py, (cuuint64_t)g.Pz, 5};
+    cuuint64_t strides[3] = {(cuuint64_t)g.Px * 8, (cuuint64_t)g.sz * 8, (cuuint64_t)g.NP * 8};
+    cuuint32_t box[4] = {(cuuint32_t)bxw, (cuuint32_t)byh, 1, 5};
+    cuuint32_t es[4] = {1, 1, 1, 1};
+    return enc(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, base, dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
+               CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+               CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+}  // namespace
+
+struct LqSweepPlan {
+    CUtensorMap mq[2], mv[2], mF[2];
+    double *bq[2] = {nullptr, nullptr}, *bv[2] = {nullptr, nullptr}, *bF[2] = {nullptr, nullptr};
+    bool three = false;
+    double *partials = nullptr;
+    unsigned int *counter = nullptr;
+    dim3 grid;
+    int zc = 0;
+    bool attr_set[4] = {false, false, false, false};
+};
+
+void lq_sweep_destroy(LqSweepPlan *p) {
+    if (!p) return;
+    cudaFree(p->partials);
+    cudaFree(p->counter);
+    delete p;
+}
 void lq_sweep_invalidate(LqSweepPlan *) {}
-int lq_sweep_run(LqSweepPlan **, const LqGeom &, const LqPhys &, const LqFields &, double *[2], double *[2],
-                 double *[2], int *, LqFireScalars *, const LqFireConsts &, long, cudaStream_t, long *, long *,
-                 LqFireScalars *, std::string &err) {
-    err = "fused sweep not built";
-    return LQ_ERR_STATE;
+
+template <class C, bool THREE, bool MASKED>
+static cudaError_t launch(LqSweepPlan *pl, int in, const SweepArgs &a, int variant, cudaStream_t st) {
+    if (!pl->attr_set[variant]) {
+        cudaError_t e = cudaFuncSetAttribute(k_sweep<C, THREE, MASKED>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                             C::SMEM_BYTES);
+        if (e != cudaSuccess) return e;
+        pl->attr_set[variant] = true;
+    }
+    k_sweep<C, THREE, MASKED><<<pl->grid, C::NT, C::SMEM_BYTES, st>>>(pl->mq[in], pl->mv[in], pl->mF[in], a);
+    return cudaGetLastError();
+}
+
+int lq_sweep_run(LqSweepPlan **planp, const LqGeom &g, const LqPhys &ph, const LqFields &f, double *q[2],
+                 double *v[2], double *F[2], int *cur, LqFireScalars *dsc, const LqFireConsts &fc, long max_steps,
+                 cudaStream_t st, long *launches, long *sweeps, LqFireScalars *h, std::string &err) {
+    using C1 = Cfg<32, 16>;   // one-constant: 512 threads, <= 128 registers
+    using C3 = Cfg<32, 8>;    // three-constant: 256 threads, <= 255 registers
+    const bool three = ph.L2 != 0.0 || ph.L3 != 0.0;
+    const bool masked = f.flags != nullptr;
+    LqSweepPlan *pl = *planp;
+    if (!pl) {
+        pl = new LqSweepPlan();
+        *planp = pl;
+    }
+    const int TX = 32, TY = three ? C3::TY : C1::TY;
+    bool rebuild = pl->three != three || pl->partials == nullptr;
+    for (int i = 0; i < 2; ++i) rebuild |= pl->bq[i] != q[i] || pl->bv[i] != v[i] || pl->bF[i] != F[i];
+    if (rebuild) {
+        for (int i = 0; i < 2; ++i) {
+            if (!make_map(&pl->mq[i], g, q[i], TX + 4, TY + 2) || !make_map(&pl->mv[i], g, v[i], TX + 4, TY + 2) ||
+                !make_map(&pl->mF[i], g, F[i], TX + 4, TY + 2)) {
+                err = "lq_sweep: cuTensorMapEncodeTiled failed";
+                return LQ_ERR_CUDA;
+            }
+            pl->bq[i] = q[i]; pl->bv[i] = v[i]; pl->bF[i] = F[i];
+        }
+        pl->three = three;
+        const int ntx = (g.Lx + TX - 1) / TX, nty = (g.Ly + TY - 1) / TY;
+        // z-chunk: aim for >= 4 CTAs per SM worth of work items, chunk >= 8 planes, <= 64
+        int zc = 64;
+        while (zc > 8 && (long long)ntx * nty * ((g.Lz + zc - 1) / zc) < 4 * 148) zc >>= 1;
+        if (zc > g.Lz) zc = g.Lz;
+        pl->zc = zc;
+        pl->grid = dim3(ntx, nty, (g.Lz + zc - 1) / zc);
+        cudaFree(pl->partials); cudaFree(pl->counter);
+        pl->partials = nullptr; pl->counter = nullptr;
+        const size_t ncta = (size_t)pl->grid.x * pl->grid.y * pl->grid.z;
+        if (cudaMalloc(&pl->partials, ncta * 4 * sizeof(double)) != cudaSuccess ||
+            cudaMalloc(&pl->counter, sizeof(unsigned int)) != cudaSuccess) {
+            err = "lq_sweep: cudaMalloc failed";
+            return LQ_ERR_NOMEM;
+        }
+    }
+    cudaError_t e = cudaMemsetAsync(pl->counter, 0, sizeof(unsigned int), st);
+    if (e != cudaSuccess) { err = cudaGetErrorString(e); return LQ_ERR_CUDA; }
+    // F of the entry state was written by the generic kernel without its ghost shell
+    lq_launch_fill_ghosts_f64(g, F[*cur], 5, st);
+    *launches += 1;
+
+    const int cur0 = *cur;
+    SweepArgs a;
+    a.g = g; a.ph = ph; a.f = f; a.sc = dsc; a.fc = fc; a.partials = pl->partials; a.counter = pl->counter; a.zc = pl->zc;
+    const long chunk = fc.force_tol > 0.0 ? 100 : (1L << 30);
+    long done = 0;
+    while (done < max_steps) {
+        const long n = (max_steps - done) < chunk ? (max_steps - done) : chunk;
+        for (long i = 0; i < n; ++i) {
+            const int in = (int)((cur0 + done + i) & 1), out = in ^ 1;
+            a.qo = q[out]; a.vo = v[out]; a.Fo = F[out];
+            if (three) e = masked ? launch<C3, true, true>(pl, in, a, 3, st) : launch<C3, true, false>(pl, in, a, 2, st);
+            else e = masked ? launch<C1, false, true>(pl, in, a, 1, st) : launch<C1, false, false>(pl, in, a, 0, st);
+            if (e != cudaSuccess) { err = std::string("lq_sweep launch: ") + cudaGetErrorString(e); return LQ_ERR_CUDA; }
+        }
+        done += n;
+        *launches += n; *sweeps += n;
+        if (fc.force_tol > 0.0) {
+            e = cudaMemcpyAsync(h, dsc, sizeof(*h), cudaMemcpyDeviceToHost, st);
+            if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+            if (e != cudaSuccess) { err = std::string("lq_sweep: ") + cudaGetErrorString(e); return LQ_ERR_CUDA; }
+            if (h->converged) break;
+        }
+    }
+    e = cudaMemcpyAsync(h, dsc, sizeof(*h), cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    if (e != cudaSuccess) { err = std::string("lq_sweep: ") + cudaGetErrorString(e); return LQ_ERR_CUDA; }
+    *cur = (int)((cur0 + h->step) & 1);
+    return LQ_OK;
 }

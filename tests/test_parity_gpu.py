@@ -210,7 +210,7 @@ def test_edge_cases(lq, oracle_mod):
     mask[3, 4, 4] = mask[5, 4, 4] = 1
     c = wl.random_masked_problem(7, 6, 6, 6)
     c["mask"] = mask.reshape(-1)
-    c["kind"] = np.where(wl.neighbour_is_object(mask) & (mask == 0), c["kind"].reshape(6, 6, 6) | 1, 0).astype(np.uint8).reshape(-1)
+    c["kind"] = np.where(wl.neighbour_is_object(mask) & (mask == 0), np.maximum(c["kind"].reshape(6, 6, 6), 1), 0).astype(np.uint8).reshape(-1)
     ctx = lq.create_from_config(c)
     o = make_oracle(oracle_mod, c)
     assert np.array_equal(lq.lq_get_flags(ctx), o.classify())

@@ -1,0 +1,326 @@
+#!/usr/bin/env python
+"""bench.py -- FIRE lattice site-updates/s of the fused LdG sweep on B200 (fp64).
+
+One "step" = one FIRE step (one launch of the fused force+FIRE sweep kernel) over the whole
+lattice.  Default workload: BASELINE.json config 4 (512^3 periodic, one-constant, random-director
+quench), the largest single-GPU configuration and the one the >= 256^3 roofline target is quoted on.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload 4|3|5|5p|2|1] [--impl reference]
+
+Prints ONE JSON line (rank 0).  Keys follow the driver's contract; see DESIGN.md section 8.
+  value      N_sim * K / device time of lq_fire_minimize(K steps) with Q resident in HBM (CUDA events
+             on the library's stream, max over ranks)
+  e2e        same metric through the C ABI with HOST buffers: lq_set_Q(pinned host) +
+             lq_fire_minimize(K) + lq_get_Q(pinned host), all inside the timed region
+  roofline   algorithmic bytes (160 B per site-update, +1 flag byte with objects) per launch
+             / average launch duration, against MEASURED_PEAKS.json's HBM copy bandwidth
+  cpu_baseline  the oracle (oracle/, OpenMP, as it stands) timed on this box's host cores on a bounded
+             crop of the same workload
+Multi-GPU: the path is single-GPU by design (north_star); --gpus N runs N independent replicas
+("replicas only"), value = N * units / max-over-ranks time, scaling "weak".
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "FIRE lattice site-updates/sec (fp64, 1 B200); achieved HBM GB/s vs peak"
+UNIT = "site-updates/s"
+FALLBACK_HBM_GBS = 6650.0   # B200_PROFILING.md fallback
+
+
+def measured_hbm_peak():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(p) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured"
+    except Exception:
+        return FALLBACK_HBM_GBS, "fallback"
+
+
+class ClockSampler:
+    """samples SM clock / throttle reasons during the timed region (pynvml, else nvidia-smi)"""
+
+    def __init__(self, index=0, period=0.05):
+        self.index, self.period = index, period
+        self.samples, self.reasons, self.max_mhz = [], set(), None
+        self._stop = threading.Event()
+        self._thr = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+        except Exception:
+            self.nv = None
+
+    def _loop(self):
+        nv = self.nv
+        names = {}
+        for n in dir(nv):
+            if n.startswith("nvmlClocksEventReason") or n.startswith("nvmlClocksThrottleReason"):
+                v = getattr(nv, n)
+                if isinstance(v, int) and v and n not in ("nvmlClocksEventReasonAll", "nvmlClocksThrottleReasonAll"):
+                    names.setdefault(v, n.replace("nvmlClocksEventReason", "").replace("nvmlClocksThrottleReason", ""))
+        while not self._stop.is_set():
+            try:
+                self.samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                try:
+                    r = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)
+                except Exception:
+                    r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                for bit, nm in names.items():
+                    if r & bit and bit & (bit - 1) == 0:
+                        self.reasons.add(nm)
+            except Exception:
+                pass
+            time.sleep(self.period)
+
+    def start(self):
+        if self.nv is not None:
+            self._thr = threading.Thread(target=self._loop, daemon=True)
+            self._thr.start()
+
+    def stop(self):
+        self._stop.set()
+        if self._thr:
+            self._thr.join()
+        s = sorted(self.samples)
+        rs = sorted(x for x in self.reasons if x not in ("None", "GpuIdle", "ApplicationsClocksSetting"))
+        return {"sm_mhz": (s[len(s) // 2] if s else None), "sm_max_mhz": self.max_mhz, "reasons": rs,
+                "samples": len(s)}
+
+
+def build_workload(name):
+    from paper_1911_07045_b200 import workloads as wl
+    return wl.make_config(name)
+
+
+def oracle_problem(c):
+    import oracle
+    return oracle.Oracle(c["Lx"], c["Ly"], c["Lz"], c["A"], c["B"], c["C"], c["L1"], c["L2"], c["L3"],
+                         mask=c["mask"], kind=c["kind"], W=c["W"], axis=c["axis"])
+
+
+def crop_config(c, L):
+    """bounded sample of the workload for the CPU oracle: the [0,L)^3 corner crop of every array (periodic
+    wrap of the crop; same value distributions / structure, smaller lattice)"""
+    Lx, Ly, Lz = min(L, c["Lx"]), min(L, c["Ly"]), min(L, c["Lz"])
+
+    def crop(a, lead):
+        if a is None:
+            return None
+        a = a.reshape(*lead, c["Lz"], c["Ly"], c["Lx"])[..., :Lz, :Ly, :Lx]
+        return np.ascontiguousarray(a).reshape(*lead, -1)
+
+    d = dict(c)
+    d.update(Lx=Lx, Ly=Ly, Lz=Lz, N=Lx * Ly * Lz, q=crop(c["q"], (5,)), mask=crop(c["mask"], ()),
+             kind=crop(c["kind"], ()), W=crop(c["W"], ()), axis=crop(c["axis"], (3,)))
+    return d
+
+
+def time_oracle(c, target_s=15.0, crop=128):
+    """oracle FIRE steps on a crop; returns (site-updates/s, cores, sample description)"""
+    import oracle
+    oracle.build_oracle()
+    s = crop_config(c, crop)
+    o = oracle_problem(s)
+    nsim = s["N"] if s["mask"] is None else int(np.sum(s["mask"] == 0))
+    t0 = time.perf_counter()
+    o.fire(s["q"], 1, 0.0, s["fire"], variant=1)
+    t1 = time.perf_counter() - t0                      # 1 step (+ the initial force evaluation)
+    steps = int(max(2, min(200, target_s / max(t1 / 2.0, 1e-4))))
+    t0 = time.perf_counter()
+    o.fire(s["q"], steps, 0.0, s["fire"], variant=1)
+    dt = time.perf_counter() - t0
+    val = nsim * steps / dt
+    desc = "%dx%dx%d corner crop of %s, %d FIRE steps, oracle variant=factorised+OpenMP, %.1f s" % (
+        s["Lx"], s["Ly"], s["Lz"], c["name"], steps, dt)
+    return val, oracle.num_threads(), desc, dt, steps
+
+
+def run_reference(args):
+    """--impl reference: the oracle as it stands, on host cores, same metric/config keys"""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    c = build_workload(args.workload)
+    per_step = []
+    import oracle
+    oracle.build_oracle()
+    s = crop_config(c, args.ref_crop)
+    o = oracle_problem(s)
+    nsim = s["N"] if s["mask"] is None else int(np.sum(s["mask"] == 0))
+    q = s["q"]
+    for _ in range(args.warmup if args.warmup is not None else 1):
+        q, _ = o.fire(q, 1, 0.0, s["fire"], variant=1)
+    K = args.steps if args.steps is not None else 5
+    t0 = time.perf_counter()
+    q, _ = o.fire(q, K, 0.0, s["fire"], variant=1)
+    dt = time.perf_counter() - t0
+    val = nsim * K / dt
+    sample = "%dx%dx%d corner crop of %s, %d FIRE steps per timed call" % (s["Lx"], s["Ly"], s["Lz"], c["name"], K)
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": K,
+            "warmup": args.warmup if args.warmup is not None else 1, "ms_per_step": 1e3 * dt / K,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": c["name"], "sample": sample},
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
+                             "sample": sample},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def aggregate(local_ms, local_units, world, dist=None, device=None):
+    """max-over-ranks time and total units (replicas): used by the N>1 path and the gloo CPU test"""
+    if world == 1 or dist is None:
+        return local_ms, local_units
+    import torch
+    t = torch.tensor([local_ms], dtype=torch.float64, device=device)
+    u = torch.tensor([float(local_units)], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    dist.all_reduce(u, op=dist.ReduceOp.SUM)
+    return float(t.item()), float(u.item())
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=None)
+    ap.add_argument("--warmup", type=int, default=None)
+    ap.add_argument("--workload", default="4")
+    ap.add_argument("--impl", default="lq", choices=["lq", "reference"])
+    ap.add_argument("--ref-crop", type=int, default=128)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--fire-path", type=int, default=0)
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import torch
+    from paper_1911_07045_b200 import binding as lq, build
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (no CPU fallback)")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl")
+    build.build()
+    K = args.steps if args.steps is not None else 200
+    W = args.warmup if args.warmup is not None else 5
+    if W < 3:
+        W = 3
+
+    c = build_workload(args.workload)
+    N = c["N"]
+    ctx = lq.lq_create(c["Lx"], c["Ly"], c["Lz"], c["A"], c["B"], c["C"], c["L1"], c["L2"], c["L3"])
+    stream = torch.cuda.current_stream()
+    lq.lq_set_stream(ctx, stream.cuda_stream)
+    lq.lq_set_option(ctx, "fire_path", args.fire_path)
+    if c["mask"] is not None:
+        lq.lq_set_sites(ctx, c["mask"], c["kind"], c["W"], c["axis"])
+    nsim = int(lq.lq_get_info(ctx, "n_simulated"))
+    # pinned host staging for the e2e leg
+    hq = torch.empty((5, N), dtype=torch.float64, pin_memory=True)
+    hq.numpy()[...] = c["q"]
+    hout = torch.empty((5, N), dtype=torch.float64, pin_memory=True)
+    lq.lq_set_Q(ctx, hq)
+
+    # warm-up: W steps (also builds the sweep plan / tensor maps)
+    lq.lq_fire_minimize(ctx, W, 0.0, c["fire"])
+    torch.cuda.synchronize()
+    if dist is not None:
+        dist.barrier()
+    sampler = ClockSampler(local)
+    sampler.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    e0.record(stream)
+    rep = lq.lq_fire_minimize(ctx, K, 0.0, c["fire"])
+    e1.record(stream)
+    torch.cuda.synchronize()
+    clocks = sampler.stop()
+    ms = e0.elapsed_time(e1)
+    assert rep["steps"] == K
+    if dist is not None:
+        dist.barrier()
+    ms_max, units = aggregate(ms, nsim * K, world, dist, torch.device("cuda", local))
+    value = units / (ms_max * 1e-3)
+
+    # e2e: host buffers in, K steps, host buffers out -- all inside the timed region
+    e2e = None
+    if not args.no_e2e:
+        torch.cuda.synchronize()
+        if dist is not None:
+            dist.barrier()
+        t0 = time.perf_counter()
+        lq.lq_set_Q(ctx, hq)
+        rep2 = lq.lq_fire_minimize(ctx, K, 0.0, c["fire"])
+        lq.lq_get_Q(ctx, hout)
+        torch.cuda.synchronize()
+        t_e2e = (time.perf_counter() - t0) * 1e3
+        t_max, units2 = aggregate(t_e2e, nsim * K, world, dist, torch.device("cuda", local))
+        e2e = {"value": units2 / (t_max * 1e-3), "unit": UNIT, "h2d_bytes_per_step": 40.0 * N / K,
+               "d2h_bytes_per_step": 40.0 * N / K, "ms_total": t_max,
+               "call": "lq_set_Q(pinned host) + lq_fire_minimize(%d) + lq_get_Q(pinned host)" % K}
+
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+
+    peak, peak_kind = measured_hbm_peak()
+    flag_byte = 1.0 if lq.lq_get_info(ctx, "n_object") > 0 else 0.0
+    alg_bytes_site = 160.0 + flag_byte                       # read+write q and v (+ flag byte)
+    launch_ms = ms / max(rep["sweep_launches"], 1)           # average launch duration over the timed region
+    achieved = alg_bytes_site * N / (launch_ms * 1e-3) / 1e9
+    design_bytes_site = lq.lq_get_info(ctx, "sweep_bytes_per_site")
+    traffic = None
+    tpath = os.path.join(ROOT, "profiles", "traffic_cfg%s.json" % args.workload)
+    if os.path.exists(tpath):
+        try:
+            traffic = json.load(open(tpath)).get("dram_bytes_per_launch")
+        except Exception:
+            traffic = None
+    roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                "traffic": traffic, "peak_kind": peak_kind, "kernel": "k_sweep",
+                "algorithmic_bytes_per_site": alg_bytes_site, "design_bytes_per_site": design_bytes_site,
+                "achieved_design_GBs": design_bytes_site * N / (launch_ms * 1e-3) / 1e9,
+                "launch_ms": launch_ms}
+
+    cpu = None
+    if not args.no_cpu_baseline:
+        v, cores, desc, _, _ = time_oracle(c, target_s=15.0, crop=args.ref_crop)
+        cpu = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc}
+
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+            "ms_per_step": ms_max / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic",
+            "config": {"workload": c["name"], "lattice": [c["Lx"], c["Ly"], c["Lz"]], "n_simulated": nsim,
+                       "elastic": "L1" if c["L2"] == 0 and c["L3"] == 0 else "L1+L2+L3",
+                       "l2": "inputs_larger_than_L2" if 120.0 * N > 126e6 * 4 else "L2_resident_no_flush",
+                       "multi_gpu": "replicas only", "fire_path": args.fire_path},
+            "clocks": clocks, "e2e": e2e, "gpu_launches": rep["launches"], "roofline": roofline,
+            "cpu_baseline": cpu}
+    print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -140,7 +140,9 @@ int lq_fire_minimize(lq_ctx *ctx, long max_steps, double force_tol,
 int lq_get_S0(lq_ctx *ctx, double *S0);
 
 /* Tuning / introspection, not part of the method.  Keys:
- *   "fire_path" (set): 0 = fused one-sweep-per-step kernel (default), 1 = unfused four-kernel path
+ *   "fire_path" (set): 0 = fused one-launch-per-step sweep (default; one-constant: force recomputed,
+ *                      state (q, v); L2/L3 != 0: force stored, state (q, v, F)), 1 = unfused four-kernel
+ *                      path, 2 = fused sweep with the force stored (any constants)
  *   "sweep_bytes_per_site" (get): algorithmic HBM bytes one sweep moves per site
  *   "n_simulated" (get), "n_boundary" (get), "n_object" (get)
  * Unknown key: LQ_ERR_ARG. */

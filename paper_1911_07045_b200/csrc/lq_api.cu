@@ -202,6 +202,9 @@ int lq_set_sites(lq_ctx *c, const uint8_t *mask, const uint8_t *anch_kind, const
         LQ_CUDA(c, copy_box(g, c->kind, anch_kind, 1, 1, true, st));
         LQ_CUDA(c, copy_box(g, c->W, W, sizeof(double), 1, true, st));
         LQ_CUDA(c, copy_box(g, c->axis, axis, sizeof(double), 3, true, st));
+        lq_launch_fill_ghosts_u8(g, c->kind, st);     // the recompute sweep evaluates anchoring on halo sites
+        lq_launch_fill_ghosts_f64(g, c->W, 1, st);
+        lq_launch_fill_ghosts_f64(g, c->axis, 3, st);
         int *dbad2 = c->dbad;  // reuse after reading the first result
         int bad_mask = 0;
         LQ_CUDA(c, cudaMemcpyAsync(&bad_mask, c->dbad, sizeof(int), cudaMemcpyDeviceToHost, st));
@@ -315,7 +318,7 @@ int lq_get_S0(lq_ctx *c, double *S0) {
 int lq_set_option(lq_ctx *c, const char *key, double value) {
     if (!c || !key) return LQ_ERR_ARG;
     if (!strcmp(key, "fire_path")) {
-        if (value != 0.0 && value != 1.0) return fail(c, LQ_ERR_ARG, "fire_path must be 0 or 1");
+        if (value != 0.0 && value != 1.0 && value != 2.0) return fail(c, LQ_ERR_ARG, "fire_path must be 0, 1 or 2");
         c->fire_path = (int)value;
         return LQ_OK;
     }
@@ -329,8 +332,10 @@ int lq_get_info(lq_ctx *c, const char *key, double *value) {
     if (!strcmp(key, "n_boundary")) { *value = c->flags_active ? (double)c->n_class[1] : 0.0; return LQ_OK; }
     if (!strcmp(key, "n_object")) { *value = c->flags_active ? (double)c->n_class[2] : 0.0; return LQ_OK; }
     if (!strcmp(key, "sweep_bytes_per_site")) {
-        // fused sweep: read q, v, F and write q, v, F (5 fp64 each) + the flag byte where objects exist
-        *value = c->fire_path == 0 ? 240.0 + (c->flags_active ? 1.0 : 0.0) : 0.0;
+        // fused sweep: read + write q, v (and F when it is stored), 5 fp64 each, + the flag byte where objects exist
+        const bool three = c->ph.L2 != 0.0 || c->ph.L3 != 0.0;
+        const double fields = (three || c->fire_path == 2) ? 6.0 : 4.0;
+        *value = c->fire_path == 1 ? 0.0 : fields * 40.0 + (c->flags_active ? 1.0 : 0.0);
         return LQ_OK;
     }
     return fail(c, LQ_ERR_ARG, std::string("lq_get_info: unknown key ") + key);
@@ -350,11 +355,13 @@ int lq_fire_minimize(lq_ctx *c, long max_steps, double force_tol, const lq_fire_
     int rc;
     if ((rc = ensure_field(c, &c->v[c->cur])) != LQ_OK) return rc;
     if ((rc = ensure_field(c, &c->F[c->cur])) != LQ_OK) return rc;
-    const bool fused = c->fire_path == 0;
+    const bool fused = c->fire_path != 1;
+    const bool three = c->ph.L2 != 0.0 || c->ph.L3 != 0.0;
+    const bool stored_F = three || c->fire_path == 2;   // recompute-F sweep: one-constant only
     if (fused) {
         if ((rc = ensure_field(c, &c->q[c->cur ^ 1])) != LQ_OK) return rc;
         if ((rc = ensure_field(c, &c->v[c->cur ^ 1])) != LQ_OK) return rc;
-        if ((rc = ensure_field(c, &c->F[c->cur ^ 1])) != LQ_OK) return rc;
+        if (stored_F && (rc = ensure_field(c, &c->F[c->cur ^ 1])) != LQ_OK) return rc;
     }
     const int nb1 = lq_fire1_num_blocks(g);
     if ((rc = ensure_partials(c, (size_t)4 * nb1)) != LQ_OK) return rc;
@@ -380,7 +387,7 @@ int lq_fire_minimize(lq_ctx *c, long max_steps, double force_tol, const lq_fire_
 
     long done = 0;
     if (fused) {
-        rc = lq_sweep_run(&c->sweep, g, c->ph, f, c->q, c->v, c->F, &c->cur, c->dsc, fc, max_steps, st, &launches,
+        rc = lq_sweep_run(&c->sweep, stored_F, g, c->ph, f, c->q, c->v, c->F, &c->cur, c->dsc, fc, max_steps, st, &launches,
                           &sweeps, &h, c->err);
         if (rc != LQ_OK) { cudaEventDestroy(ev0); cudaEventDestroy(ev1); return rc; }
     } else {

@@ -20,14 +20,17 @@
 // registers.  Outputs go straight from registers to global memory with coalesced 256-byte rows; sites
 // on the lattice faces also refresh the periodic ghost shell of the output buffers.
 #include "lq_sweep.cuh"
+#include "lq_sweep_dev.cuh"
 #include "lq_site.cuh"
 #include "../../include/lq.h"
 
 #include <cuda.h>
 #include <cstdio>
 #include <cstring>
+#include <cstdlib>
 
 namespace {
+using namespace lqsw;
 
 template <int TX_, int TY_>
 struct Cfg {
@@ -50,59 +53,6 @@ struct Cfg {
     static constexpr int NHALO = 2 * BXW + 2 * (BYH - 2);
 };
 
-struct SweepArgs {
-    LqGeom g;
-    LqPhys ph;
-    LqFields f;
-    double *qo, *vo, *Fo;
-    LqFireScalars *sc;
-    LqFireConsts fc;
-    double *partials;
-    unsigned int *counter;
-    int zc;
-};
-
-// ---------------------------------------------------------------- PTX wrappers (TMA + mbarrier)
-__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
-
-__device__ __forceinline__ void mbar_init(uint64_t *bar, int count) {
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
-}
-__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes) {
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity) {
-    asm volatile(
-        "{\n"
-        ".reg .pred p;\n"
-        "WAIT_LOOP:\n"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
-        "@p bra WAIT_DONE;\n"
-        "bra WAIT_LOOP;\n"
-        "WAIT_DONE:\n"
-        "}\n" ::"r"(smem_u32(bar)),
-        "r"(parity)
-        : "memory");
-}
-__device__ __forceinline__ void tma_load_4d(void *dst, const CUtensorMap *map, uint64_t *bar, int c0, int c1, int c2,
-                                            int c3) {
-    asm volatile(
-        "cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5, %6}], [%2];"
-        ::"r"(smem_u32(dst)), "l"(map), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2), "r"(c3)
-        : "memory");
-}
-
-__device__ __forceinline__ double warp_sum(double v) {
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
-    return v;
-}
-__device__ __forceinline__ double warp_max(double v) {
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) v = fmax(v, __shfl_down_sync(0xffffffffu, v, o));
-    return v;
-}
-
 // accessor over the shared-memory ring of q' planes (k-1, k, k+1); flags come from global memory
 template <class C>
 struct RingAcc {
@@ -119,14 +69,6 @@ struct RingAcc {
         return flags ? (unsigned)flags[p + dx + dy * sy + dz * sz] : 0xFCu;
     }
 };
-
-// q' and v_k of one site from its staged (q, vc, F): the SAME instruction sequence for a CTA's own
-// sites and for the halo copies its neighbours compute, so every CTA sees bit-identical q'.
-__device__ __forceinline__ void drift(double q, double vc, double F, double ma, double cF, double dt, double &vk,
-                                      double &qn) {
-    vk = __fma_rn(ma, vc, cF * F);
-    qn = __fma_rn(dt, vk, q);
-}
 
 template <class C, bool THREE, bool MASKED>
 __global__ void __launch_bounds__(C::NT, 1)
@@ -261,11 +203,20 @@ k_sweep(const __grid_constant__ CUtensorMap tq, const __grid_constant__ CUtensor
                     r[3] = fmax(r[3], fabs(Fn[c]));
                 }
             }
+            if (a.store_cs) {
 #pragma unroll
-            for (int c = 0; c < 5; ++c) {
-                a.qo[c * NP + p] = qc[c];
-                a.vo[c * NP + p] = vn[c];
-                a.Fo[c * NP + p] = Fn[c];
+                for (int c = 0; c < 5; ++c) {
+                    __stcs(a.qo + c * NP + p, qc[c]);
+                    __stcs(a.vo + c * NP + p, vn[c]);
+                    __stcs(a.Fo + c * NP + p, Fn[c]);
+                }
+            } else {
+#pragma unroll
+                for (int c = 0; c < 5; ++c) {
+                    a.qo[c * NP + p] = qc[c];
+                    a.vo[c * NP + p] = vn[c];
+                    a.Fo[c * NP + p] = Fn[c];
+                }
             }
             // periodic ghost shell of the outputs (width LQ_GW)
             const int shx = x < LQ_GW ? a.g.Lx : (x >= a.g.Lx - LQ_GW ? -a.g.Lx : 0);
@@ -287,55 +238,7 @@ k_sweep(const __grid_constant__ CUtensorMap tq, const __grid_constant__ CUtensor
         if (TWO_SYNC) __syncthreads();
     }
 
-    // ---- per-CTA partials, then the last CTA reduces all of them in index order and advances FIRE
-    const int lane = tid & 31, wid = tid >> 5;
-    constexpr int NW = C::NT / 32;
-#pragma unroll
-    for (int i = 0; i < 4; ++i) {
-        const double w = i < 3 ? warp_sum(r[i]) : warp_max(r[i]);
-        if (lane == 0) red[i * NW + wid] = w;
-    }
-    __syncthreads();
-    __shared__ unsigned s_last;
-    const unsigned ncta = gridDim.x * gridDim.y * gridDim.z;
-    const unsigned cta = blockIdx.x + gridDim.x * (blockIdx.y + gridDim.y * blockIdx.z);
-    if (tid == 0) {
-        double t[4];
-#pragma unroll
-        for (int i = 0; i < 4; ++i) {
-            t[i] = red[i * NW];
-            for (int w = 1; w < NW; ++w) t[i] = i < 3 ? t[i] + red[i * NW + w] : fmax(t[i], red[i * NW + w]);
-            a.partials[4 * cta + i] = t[i];
-        }
-        __threadfence();
-        s_last = atomicAdd(a.counter, 1u) == ncta - 1 ? 1u : 0u;
-    }
-    __syncthreads();
-    if (!s_last) return;
-    __threadfence();
-    double t[4] = {0.0, 0.0, 0.0, 0.0};
-    for (unsigned b = tid; b < ncta; b += C::NT) {
-        t[0] += __ldcg(a.partials + 4 * b); t[1] += __ldcg(a.partials + 4 * b + 1); t[2] += __ldcg(a.partials + 4 * b + 2);
-        t[3] = fmax(t[3], __ldcg(a.partials + 4 * b + 3));
-    }
-#pragma unroll
-    for (int i = 0; i < 4; ++i) {
-        const double w = i < 3 ? warp_sum(t[i]) : warp_max(t[i]);
-        if (lane == 0) red[i * NW + wid] = w;
-    }
-    __syncthreads();
-    if (tid == 0) {
-        double tot[4];
-#pragma unroll
-        for (int i = 0; i < 4; ++i) {
-            tot[i] = red[i * NW];
-            for (int w = 1; w < NW; ++w) tot[i] = i < 3 ? tot[i] + red[i * NW + w] : fmax(tot[i], red[i * NW + w]);
-        }
-        LqFireScalars nx = sc;
-        lq_fire_advance(nx, a.fc, tot, 0);
-        *a.sc = nx;
-        *a.counter = 0u;
-    }
+    lqsw::finish_step<C::NT>(a, sc, r, red);
 }
 
 // ---------------------------------------------------------------- host side
@@ -362,9 +265,13 @@ bool make_map(CUtensorMap *m, const LqGeom &g, double *base, int bxw, int byh) {
     cuuint64_t strides[3] = {(cuuint64_t)g.Px * 8, (cuuint64_t)g.sz * 8, (cuuint64_t)g.NP * 8};
     cuuint32_t box[4] = {(cuuint32_t)bxw, (cuuint32_t)byh, 1, 5};
     cuuint32_t es[4] = {1, 1, 1, 1};
+    const char *pe = getenv("LQ_TMA_PROMO");
+    const int promo = pe ? atoi(pe) : 0;
+    const CUtensorMapL2promotion pr = promo == 3 ? CU_TENSOR_MAP_L2_PROMOTION_L2_256B
+                                    : promo == 2 ? CU_TENSOR_MAP_L2_PROMOTION_L2_128B
+                                    : promo == 1 ? CU_TENSOR_MAP_L2_PROMOTION_L2_64B : CU_TENSOR_MAP_L2_PROMOTION_NONE;
     return enc(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, base, dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
-               CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
-               CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+               CU_TENSOR_MAP_SWIZZLE_NONE, pr, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
 }  // namespace
@@ -372,7 +279,7 @@ bool make_map(CUtensorMap *m, const LqGeom &g, double *base, int bxw, int byh) {
 struct LqSweepPlan {
     CUtensorMap mq[2], mv[2], mF[2];
     double *bq[2] = {nullptr, nullptr}, *bv[2] = {nullptr, nullptr}, *bF[2] = {nullptr, nullptr};
-    bool three = false;
+    bool three = false, stored = true;
     double *partials = nullptr;
     unsigned int *counter = nullptr;
     dim3 grid;
@@ -400,7 +307,7 @@ static cudaError_t launch(LqSweepPlan *pl, int in, const SweepArgs &a, int varia
     return cudaGetLastError();
 }
 
-int lq_sweep_run(LqSweepPlan **planp, const LqGeom &g, const LqPhys &ph, const LqFields &f, double *q[2],
+int lq_sweep_run(LqSweepPlan **planp, bool stored_F, const LqGeom &g, const LqPhys &ph, const LqFields &f, double *q[2],
                  double *v[2], double *F[2], int *cur, LqFireScalars *dsc, const LqFireConsts &fc, long max_steps,
                  cudaStream_t st, long *launches, long *sweeps, LqFireScalars *h, std::string &err) {
     using C1 = Cfg<32, 16>;   // one-constant: 512 threads, <= 128 registers
@@ -412,22 +319,28 @@ int lq_sweep_run(LqSweepPlan **planp, const LqGeom &g, const LqPhys &ph, const L
         pl = new LqSweepPlan();
         *planp = pl;
     }
-    const int TX = 32, TY = three ? C3::TY : C1::TY;
-    bool rebuild = pl->three != three || pl->partials == nullptr;
+    if (three && !stored_F) { err = "lq_sweep: the recompute path is one-constant only"; return LQ_ERR_ARG; }
+    const int TX = 32, TY = !stored_F ? lq_sweep_rc_tile(1) : (three ? C3::TY : C1::TY);
+    bool rebuild = pl->three != three || pl->stored != stored_F || pl->partials == nullptr;
     for (int i = 0; i < 2; ++i) rebuild |= pl->bq[i] != q[i] || pl->bv[i] != v[i] || pl->bF[i] != F[i];
     if (rebuild) {
         for (int i = 0; i < 2; ++i) {
-            if (!make_map(&pl->mq[i], g, q[i], TX + 4, TY + 2) || !make_map(&pl->mv[i], g, v[i], TX + 4, TY + 2) ||
-                !make_map(&pl->mF[i], g, F[i], TX + 4, TY + 2)) {
+            const bool ok = stored_F
+                ? make_map(&pl->mq[i], g, q[i], TX + 4, TY + 2) && make_map(&pl->mv[i], g, v[i], TX + 4, TY + 2) &&
+                  make_map(&pl->mF[i], g, F[i], TX + 4, TY + 2)
+                : make_map(&pl->mq[i], g, q[i], lq_sweep_rc_box(0, 0), lq_sweep_rc_box(0, 1)) &&
+                  make_map(&pl->mv[i], g, v[i], lq_sweep_rc_box(1, 0), lq_sweep_rc_box(1, 1));
+            if (!ok) {
                 err = "lq_sweep: cuTensorMapEncodeTiled failed";
                 return LQ_ERR_CUDA;
             }
             pl->bq[i] = q[i]; pl->bv[i] = v[i]; pl->bF[i] = F[i];
         }
         pl->three = three;
+        pl->stored = stored_F;
         const int ntx = (g.Lx + TX - 1) / TX, nty = (g.Ly + TY - 1) / TY;
         // z-chunk: aim for >= 4 CTAs per SM worth of work items, chunk >= 8 planes, <= 64
-        int zc = 64;
+        int zc = getenv("LQ_ZC") ? atoi(getenv("LQ_ZC")) : 64;
         while (zc > 8 && (long long)ntx * nty * ((g.Lz + zc - 1) / zc) < 4 * 148) zc >>= 1;
         if (zc > g.Lz) zc = g.Lz;
         pl->zc = zc;
@@ -443,13 +356,15 @@ int lq_sweep_run(LqSweepPlan **planp, const LqGeom &g, const LqPhys &ph, const L
     }
     cudaError_t e = cudaMemsetAsync(pl->counter, 0, sizeof(unsigned int), st);
     if (e != cudaSuccess) { err = cudaGetErrorString(e); return LQ_ERR_CUDA; }
-    // F of the entry state was written by the generic kernel without its ghost shell
-    lq_launch_fill_ghosts_f64(g, F[*cur], 5, st);
-    *launches += 1;
+    if (stored_F) {   // F of the entry state was written by the generic kernel without its ghost shell
+        lq_launch_fill_ghosts_f64(g, F[*cur], 5, st);
+        *launches += 1;
+    }
 
     const int cur0 = *cur;
     SweepArgs a;
     a.g = g; a.ph = ph; a.f = f; a.sc = dsc; a.fc = fc; a.partials = pl->partials; a.counter = pl->counter; a.zc = pl->zc;
+    a.store_cs = getenv("LQ_STORE_CS") ? atoi(getenv("LQ_STORE_CS")) : 0;
     const long chunk = fc.force_tol > 0.0 ? 100 : (1L << 30);
     long done = 0;
     while (done < max_steps) {
@@ -457,7 +372,8 @@ int lq_sweep_run(LqSweepPlan **planp, const LqGeom &g, const LqPhys &ph, const L
         for (long i = 0; i < n; ++i) {
             const int in = (int)((cur0 + done + i) & 1), out = in ^ 1;
             a.qo = q[out]; a.vo = v[out]; a.Fo = F[out];
-            if (three) e = masked ? launch<C3, true, true>(pl, in, a, 3, st) : launch<C3, true, false>(pl, in, a, 2, st);
+            if (!stored_F) e = lq_launch_sweep_rc(masked, pl->grid, pl->mq[in], pl->mv[in], a, st);
+            else if (three) e = masked ? launch<C3, true, true>(pl, in, a, 3, st) : launch<C3, true, false>(pl, in, a, 2, st);
             else e = masked ? launch<C1, false, true>(pl, in, a, 1, st) : launch<C1, false, false>(pl, in, a, 0, st);
             if (e != cudaSuccess) { err = std::string("lq_sweep launch: ") + cudaGetErrorString(e); return LQ_ERR_CUDA; }
         }

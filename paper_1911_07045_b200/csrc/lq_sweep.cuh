@@ -11,6 +11,16 @@ void lq_sweep_invalidate(LqSweepPlan *plan);  // geometry / anchoring arrays cha
 // Runs up to max_steps FIRE steps, one kernel launch per step.  On entry buffer *cur holds
 // (q, v = 0, F = force(q)) with q's ghost shell valid and dsc[0] the scalars after the step-0
 // update.  On return *cur is the buffer holding the final state, *h the final scalars.
-int lq_sweep_run(LqSweepPlan **plan, const LqGeom &g, const LqPhys &ph, const LqFields &f, double *q[2],
+// stored_F: true = state (q, vc, F), 240 B/site (any elastic constants); false = state (q, vc) with the force
+// recomputed, 160 B/site (one-constant only).
+int lq_sweep_run(LqSweepPlan **plan, bool stored_F, const LqGeom &g, const LqPhys &ph, const LqFields &f, double *q[2],
                  double *v[2], double *F[2], int *cur, LqFireScalars *dsc, const LqFireConsts &fc, long max_steps,
                  cudaStream_t st, long *launches, long *sweeps, LqFireScalars *h, std::string &err);
+
+// recompute-F kernel (lq_sweep_rc.cu)
+#include <cuda.h>
+namespace lqsw { struct SweepArgs; }
+int lq_sweep_rc_box(int which, int dim);
+int lq_sweep_rc_tile(int dim);
+cudaError_t lq_launch_sweep_rc(bool masked, dim3 grid, const CUtensorMap &mq, const CUtensorMap &mv,
+                               const lqsw::SweepArgs &a, cudaStream_t st);

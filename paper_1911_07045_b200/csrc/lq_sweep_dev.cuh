@@ -1,0 +1,131 @@
+// lq_sweep_dev.cuh -- device helpers shared by the fused sweep kernels (TMA / mbarrier PTX wrappers,
+// the drift formula, and the end-of-step reduction + on-device FIRE schedule).
+#pragma once
+#include "lq_internal.cuh"
+#include <cuda.h>
+
+namespace lqsw {
+
+struct SweepArgs {
+    LqGeom g;
+    LqPhys ph;
+    LqFields f;
+    double *qo, *vo, *Fo;
+    LqFireScalars *sc;
+    LqFireConsts fc;
+    double *partials;
+    unsigned int *counter;
+    int zc;
+    int store_cs;
+};
+
+// ---------------------------------------------------------------- PTX wrappers (TMA + mbarrier)
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint64_t *bar, int count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_LOOP:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra WAIT_DONE;\n"
+        "bra WAIT_LOOP;\n"
+        "WAIT_DONE:\n"
+        "}\n" ::"r"(smem_u32(bar)),
+        "r"(parity)
+        : "memory");
+}
+__device__ __forceinline__ void tma_load_4d(void *dst, const CUtensorMap *map, uint64_t *bar, int c0, int c1, int c2,
+                                            int c3) {
+    asm volatile(
+        "cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5, %6}], [%2];"
+        ::"r"(smem_u32(dst)), "l"(map), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2), "r"(c3)
+        : "memory");
+}
+
+__device__ __forceinline__ double warp_sum(double v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+    return v;
+}
+__device__ __forceinline__ double warp_max(double v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v = fmax(v, __shfl_down_sync(0xffffffffu, v, o));
+    return v;
+}
+
+
+// q' and v_k of one site from (q, vc, F): v_k = mix_a vc + (mix_b + dt/2) F ; q' = q + dt v_k.
+// The SAME instruction sequence serves a CTA's own sites and the halo copies its neighbours compute,
+// so every CTA sees bit-identical q'.
+__device__ __forceinline__ void drift(double q, double vc, double F, double ma, double cF, double dt, double &vk,
+                                      double &qn) {
+    vk = __fma_rn(ma, vc, cF * F);
+    qn = __fma_rn(dt, vk, q);
+}
+
+// ghost-shell shift of coordinate i in a periodic dimension of length L, ghost width gw (0 if interior)
+__device__ __forceinline__ int ghost_shift(int i, int L, int gw) { return i < gw ? L : (i >= L - gw ? -L : 0); }
+
+// End of a sweep: block-reduce r = (P, FF, vv, Fmax) partials, publish them, and let the LAST CTA to finish
+// reduce all CTAs' partials in index order (bitwise reproducible) and advance the FIRE schedule
+// (Algorithm 1) in place.  red: >= 4*NT/32 doubles of shared memory.
+template <int NT>
+__device__ __forceinline__ void finish_step(const SweepArgs &a, const LqFireScalars &sc, const double r[4], double *red) {
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    constexpr int NW = NT / 32;
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        const double w = i < 3 ? warp_sum(r[i]) : warp_max(r[i]);
+        if (lane == 0) red[i * NW + wid] = w;
+    }
+    __syncthreads();
+    __shared__ unsigned s_last;
+    const unsigned ncta = gridDim.x * gridDim.y * gridDim.z;
+    const unsigned cta = blockIdx.x + gridDim.x * (blockIdx.y + gridDim.y * blockIdx.z);
+    if (tid == 0) {
+        double t[4];
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            t[i] = red[i * NW];
+            for (int w = 1; w < NW; ++w) t[i] = i < 3 ? t[i] + red[i * NW + w] : fmax(t[i], red[i * NW + w]);
+            a.partials[4 * cta + i] = t[i];
+        }
+        __threadfence();
+        s_last = atomicAdd(a.counter, 1u) == ncta - 1 ? 1u : 0u;
+    }
+    __syncthreads();
+    if (!s_last) return;
+    __threadfence();
+    double t[4] = {0.0, 0.0, 0.0, 0.0};
+    for (unsigned b = tid; b < ncta; b += NT) {
+        t[0] += __ldcg(a.partials + 4 * b); t[1] += __ldcg(a.partials + 4 * b + 1); t[2] += __ldcg(a.partials + 4 * b + 2);
+        t[3] = fmax(t[3], __ldcg(a.partials + 4 * b + 3));
+    }
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        const double w = i < 3 ? warp_sum(t[i]) : warp_max(t[i]);
+        if (lane == 0) red[i * NW + wid] = w;
+    }
+    __syncthreads();
+    if (tid == 0) {
+        double tot[4];
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            tot[i] = red[i * NW];
+            for (int w = 1; w < NW; ++w) tot[i] = i < 3 ? tot[i] + red[i * NW + w] : fmax(tot[i], red[i * NW + w]);
+        }
+        LqFireScalars nx = sc;
+        lq_fire_advance(nx, a.fc, tot, 0);
+        *a.sc = nx;
+        *a.counter = 0u;
+    }
+}
+
+}  // namespace lqsw

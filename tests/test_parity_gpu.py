@@ -86,7 +86,7 @@ def test_energy_matches_oracle(case, lq):
     assert np.all(np.abs(t - tref) <= TOL_E * np.maximum(np.abs(tref), abs(eref) * 1e-3))
 
 
-@pytest.mark.parametrize("path", [0, 1])
+@pytest.mark.parametrize("path", [0, 1, 2])
 def test_q_after_100_fire_steps(case, lq, path):
     name, c, ctx, o = case
     lq.lq_set_option(ctx, "fire_path", path)
@@ -111,13 +111,14 @@ def test_q_after_100_fire_steps(case, lq, path):
 def test_fused_and_unfused_paths_agree(case, lq):
     name, c, ctx, o = case
     out = []
-    for path in (0, 1):
+    for path in (0, 1, 2):
         lq.lq_set_option(ctx, "fire_path", path)
         lq.lq_set_Q(ctx, c["q"])
         lq.lq_fire_minimize(ctx, 37, 0.0, c["fire"])
         out.append(lq.lq_get_Q(ctx))
     lq.lq_set_option(ctx, "fire_path", 0)
     assert np.abs(out[0] - out[1]).max() <= 1e-11
+    assert np.abs(out[2] - out[1]).max() <= 1e-11
 
 
 # ------------------------------------------------------------------ convergence
@@ -145,7 +146,7 @@ def test_converges_and_stops_early(lq, oracle_mod):
     c = wl.bulk_quench(8, 12345)
     ctx = lq.create_from_config(c)
     o = make_oracle(oracle_mod, c)
-    for path in (0, 1):
+    for path in (0, 1, 2):
         lq.lq_set_option(ctx, "fire_path", path)
         lq.lq_set_Q(ctx, c["q"])
         rep = lq.lq_fire_minimize(ctx, 4000, 1e-9, c["fire"], report_energy=True)

@@ -205,7 +205,7 @@ k_sweep_rc(const __grid_constant__ CUtensorMap tq, const __grid_constant__ CUten
 #pragma unroll
             for (int c = 0; c < 5; ++c) rn[c * RC::PLANE + idx] = qp[c];
         }
-        if (hx >= 0) {
+        if (hx >= 0 && !(a.store_cs & 1)) {
             double vk[5], qn[5];
             first(hx, hy, vk, qn);
             const int idx = hy * RC::BXW + hx;
@@ -271,7 +271,7 @@ k_sweep_rc(const __grid_constant__ CUtensorMap tq, const __grid_constant__ CUten
                 }
             }
         }
-        __syncthreads();   // q' slot (j-1)&1 is rewritten by the next iteration's phase 1
+        if (!(a.store_cs & 2)) __syncthreads();   // q' slot (j-1)&1 is rewritten by the next iteration's phase 1
     }
     finish_step<RC::NT>(a, sc, r, red);
 }

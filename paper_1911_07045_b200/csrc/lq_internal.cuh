@@ -99,3 +99,6 @@ void lq_launch_fire1_force(const LqGeom &g, const LqPhys &ph, const LqFields &f,
 void lq_launch_fire_update(const double *partials, int nblocks, LqFireScalars *sc_in_out, LqFireConsts fc,
                            int first, cudaStream_t st);
 void lq_launch_zero_object_sites(const LqGeom &g, const uint8_t *flags, double *field, cudaStream_t st);
+void lq_launch_plain_map(const LqGeom &g, const uint8_t *flags, uint8_t *plain, cudaStream_t st);
+void lq_launch_tile_summary(const LqGeom &g, const uint8_t *plain, uint8_t *tsum, int TX, int TY, int ntx, int nty,
+                            cudaStream_t st);

@@ -268,6 +268,33 @@ __global__ void k_zero_object_sites(LqGeom g, const uint8_t *__restrict__ flags,
         for (int c = 0; c < 5; ++c) field[c * g.NP + p] = 0.0;
 }
 
+// plain[p] = 1 iff the site is bulk with all 6 neighbours simulated AND each of its 6 neighbours also has all
+// 6 of its neighbours simulated (constant stencil weights).  Computed on the interior plus
+// a one-site ghost margin (flags carry a 2-wide ghost shell).
+__global__ void k_plain_map(LqGeom g, const uint8_t *__restrict__ flags, uint8_t *__restrict__ plain) {
+    const int x = (int)(blockIdx.x * blockDim.x + threadIdx.x) - 1;
+    const int y = (int)(blockIdx.y * blockDim.y + threadIdx.y) - 1;
+    const int z = (int)blockIdx.z - 1;
+    if (x > g.Lx || y > g.Ly) return;
+    const long long p = g.pidx(x, y, z);
+    const bool ok = flags[p] == 0xFCu && (flags[p + 1] >> 2) == 0x3Fu && (flags[p - 1] >> 2) == 0x3Fu &&
+                    (flags[p + g.sy] >> 2) == 0x3Fu && (flags[p - g.sy] >> 2) == 0x3Fu &&
+                    (flags[p + g.sz] >> 2) == 0x3Fu && (flags[p - g.sz] >> 2) == 0x3Fu;
+    plain[p] = ok ? 1 : 0;
+}
+
+// tsum[(z+1)][by][bx] = 1 iff every site of tile (bx, by) plus its one-site halo is plain at plane z (z = -1 .. Lz)
+__global__ void k_tile_summary(LqGeom g, const uint8_t *__restrict__ plain, uint8_t *__restrict__ tsum, int TX, int TY) {
+    const int bx = blockIdx.x, by = blockIdx.y, z = (int)blockIdx.z - 1;
+    int ok = 1;
+    for (int i = threadIdx.x; i < (TX + 2) * (TY + 2); i += blockDim.x) {
+        const int x = bx * TX - 1 + i % (TX + 2), y = by * TY - 1 + i / (TX + 2);
+        if (x <= g.Lx && y <= g.Ly && !plain[g.pidx(x, y, z)]) ok = 0;
+    }
+    ok = __syncthreads_and(ok);
+    if (threadIdx.x == 0) tsum[((size_t)(z + 1) * gridDim.y + by) * gridDim.x + bx] = (uint8_t)ok;
+}
+
 inline dim3 site_grid(const LqGeom &g) {
     return dim3((g.Lx + BX - 1) / BX, (g.Ly + BY - 1) / BY, (g.Lz + ZPER - 1) / ZPER);
 }
@@ -325,4 +352,13 @@ void lq_launch_fire_update(const double *partials, int nblocks, LqFireScalars *s
 }
 void lq_launch_zero_object_sites(const LqGeom &g, const uint8_t *flags, double *field, cudaStream_t st) {
     k_zero_object_sites<<<plane_grid(g), dim3(BX, BY), 0, st>>>(g, flags, field);
+}
+
+void lq_launch_plain_map(const LqGeom &g, const uint8_t *flags, uint8_t *plain, cudaStream_t st) {
+    dim3 b(64, 4), gr((g.Lx + 2 + 63) / 64, (g.Ly + 2 + 3) / 4, g.Lz + 2);
+    k_plain_map<<<gr, b, 0, st>>>(g, flags, plain);
+}
+void lq_launch_tile_summary(const LqGeom &g, const uint8_t *plain, uint8_t *tsum, int TX, int TY, int ntx, int nty,
+                            cudaStream_t st) {
+    k_tile_summary<<<dim3(ntx, nty, g.Lz + 2), 128, 0, st>>>(g, plain, tsum, TX, TY);
 }

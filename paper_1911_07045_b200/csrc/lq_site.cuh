@@ -271,4 +271,69 @@ __device__ __forceinline__ void bulk_force_oneconst(const LqPhys &ph, const doub
     F[4] = -2.0 * G[1][2] + 2.0 * ph.L1 * lap[4];
 }
 
+// three-constant, pure-bulk neighbourhood (19-point).  get(c, dx, dy, dz) returns stored component c at an
+// offset with |dx|+|dy|+|dz| <= 2 and at most two non-zero entries.  With T_ab the elastic part of -G_ab,
+//   T_ab = L1 lap(Q_ab) + (L2+L3) [ d2_b(Q_ab) + sum_{m != b} X_bm(Q_am) ],
+//   X_bm f = 1/4 [f(+b+m) - f(+b-m) - f(-b+m) + f(-b-m)]   (bulk specialisation)
+// and Qzz = -Qxx - Qyy eliminated by linearity:
+//   F0 = L1(2 lap xx + lap yy) + L23[d2x xx + d2z xx + d2z yy + Xxy xy - Xyz yz]
+//   F3 = L1(2 lap yy + lap xx) + L23[d2y yy + d2z xx + d2z yy + Xxy xy - Xxz xz]
+//   F1 = 2 L1 lap xy + L23[d2x xy + d2y xy + Xxy xx + Xxy yy + Xyz xz + Xxz yz]
+//   F2 = 2 L1 lap xz + L23[d2x xz + d2z xz + Xyz xy + Xxy yz - Xxz yy]
+//   F4 = 2 L1 lap yz + L23[d2y yz + d2z yz + Xxz xy + Xxy xz - Xyz xx]
+template <class Get>
+__device__ __forceinline__ void bulk_force_threeconst(const LqPhys &ph, const Get &g, const double qc[5], double F[5]) {
+    const double L1 = ph.L1, L23 = ph.L2 + ph.L3;
+    auto d2 = [&](int c, int ax) -> double {
+        return (g(c, ax == 0, ax == 1, ax == 2) + g(c, -(ax == 0), -(ax == 1), -(ax == 2))) - 2.0 * qc[c];
+    };
+    auto X = [&](int c, int b, int m) -> double {   // axes b < m
+        const int bx = b == 0, by = b == 1, bz = b == 2, mx = m == 0, my = m == 1, mz = m == 2;
+        return 0.25 * ((g(c, bx + mx, by + my, bz + mz) - g(c, bx - mx, by - my, bz - mz)) -
+                       (g(c, -bx + mx, -by + my, -bz + mz) - g(c, -bx - mx, -by - my, -bz - mz)));
+    };
+    double Q[6] = {qc[0], qc[1], qc[2], qc[3], qc[4], -qc[0] - qc[3]};
+    double G[3][3];
+    bulk_G(ph, Q, G);
+    F[0] = -(G[0][0] - G[2][2]); F[1] = -2.0 * G[0][1]; F[2] = -2.0 * G[0][2];
+    F[3] = -(G[1][1] - G[2][2]); F[4] = -2.0 * G[1][2];
+    {   // xx: lap, d2x, d2z, Xxy, Xyz
+        const double dx = d2(0, 0), dy = d2(0, 1), dz = d2(0, 2), lap = dx + dy + dz;
+        F[0] += 2.0 * L1 * lap + L23 * (dx + dz);
+        F[3] += L1 * lap + L23 * dz;
+        F[1] += L23 * X(0, 0, 1);
+        F[4] -= L23 * X(0, 1, 2);
+    }
+    {   // yy: lap, d2y, d2z, Xxy, Xxz
+        const double dx = d2(3, 0), dy = d2(3, 1), dz = d2(3, 2), lap = dx + dy + dz;
+        F[3] += 2.0 * L1 * lap + L23 * (dy + dz);
+        F[0] += L1 * lap + L23 * dz;
+        F[1] += L23 * X(3, 0, 1);
+        F[2] -= L23 * X(3, 0, 2);
+    }
+    {   // xy: lap, d2x, d2y, Xxy, Xxz, Xyz
+        const double dx = d2(1, 0), dy = d2(1, 1), dz = d2(1, 2), lap = dx + dy + dz;
+        F[1] += 2.0 * L1 * lap + L23 * (dx + dy);
+        const double xxy = X(1, 0, 1);
+        F[0] += L23 * xxy;
+        F[3] += L23 * xxy;
+        F[4] += L23 * X(1, 0, 2);
+        F[2] += L23 * X(1, 1, 2);
+    }
+    {   // xz: lap, d2x, d2z, Xxy, Xxz, Xyz
+        const double dx = d2(2, 0), dy = d2(2, 1), dz = d2(2, 2), lap = dx + dy + dz;
+        F[2] += 2.0 * L1 * lap + L23 * (dx + dz);
+        F[4] += L23 * X(2, 0, 1);
+        F[3] -= L23 * X(2, 0, 2);
+        F[1] += L23 * X(2, 1, 2);
+    }
+    {   // yz: lap, d2y, d2z, Xxy, Xxz, Xyz
+        const double dx = d2(4, 0), dy = d2(4, 1), dz = d2(4, 2), lap = dx + dy + dz;
+        F[4] += 2.0 * L1 * lap + L23 * (dy + dz);
+        F[2] += L23 * X(4, 0, 1);
+        F[1] += L23 * X(4, 0, 2);
+        F[0] -= L23 * X(4, 1, 2);
+    }
+}
+
 }  // namespace lqs

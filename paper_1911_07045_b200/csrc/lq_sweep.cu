@@ -49,7 +49,8 @@ struct Cfg {
     static constexpr int OFF_RING = NSTAGE * STAGE_BYTES;
     static constexpr int OFF_BAR = OFF_RING + RING * RING_STRIDE;
     static constexpr int OFF_RED = OFF_BAR + 64;
-    static constexpr int SMEM_BYTES = OFF_RED + 4 * (NT / 32) * 8 + 64;
+    static constexpr int OFF_TS = OFF_RED + 4 * (NT / 32) * 8;     // tile summaries of this CTA's planes
+    static constexpr int SMEM_BYTES = OFF_TS + 128;
     static constexpr int NHALO = 2 * BXW + 2 * (BYH - 2);
 };
 
@@ -95,6 +96,9 @@ k_sweep(const __grid_constant__ CUtensorMap tq, const __grid_constant__ CUtensor
         mbar_init(&full[1], 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
+    uint8_t *ts = smem + C::OFF_TS;               // ts[i] = summary of plane zb+i
+    if (MASKED && tid < ze - zb)
+        ts[tid] = a.tsum[((size_t)(zb + tid + 1) * gridDim.y + blockIdx.y) * gridDim.x + blockIdx.x];
     __syncthreads();
 
     auto issue = [&](int j) {
@@ -158,28 +162,36 @@ k_sweep(const __grid_constant__ CUtensorMap tq, const __grid_constant__ CUtensor
         // ---- [B] force, second half kick, reductions and stores for plane k = zb + j - 2
         if (j >= 2 && active) {
             const int k = zb + j - 2;
+            const bool tile_plain = !MASKED || ts[k - zb] != 0;
             const double *rk = reinterpret_cast<const double *>(smem + C::OFF_RING + ((j - 1) % 3) * C::RING_STRIDE);
             const long long p = a.g.pidx(x, y, k);
             double Fn[5] = {0.0, 0.0, 0.0, 0.0, 0.0}, vn[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
             unsigned fl = 0xFCu;
-            bool plain = true;                    // bulk site whose 6 neighbours see only simulated sites
-            if (MASKED) {
-                fl = a.f.flags[p];
-                plain = (fl >> 2) == 0x3Fu && (a.f.flags[p + 1] >> 2) == 0x3Fu && (a.f.flags[p - 1] >> 2) == 0x3Fu &&
-                        (a.f.flags[p + a.g.sy] >> 2) == 0x3Fu && (a.f.flags[p - a.g.sy] >> 2) == 0x3Fu &&
-                        (a.f.flags[p + a.g.sz] >> 2) == 0x3Fu && (a.f.flags[p - a.g.sz] >> 2) == 0x3Fu &&
-                        (fl & 3u) == 0u;
+            bool plain = true;                    // constant stencil weights
+            if (MASKED && !tile_plain) {
+                plain = a.plain[p] != 0;
+                if (!plain) fl = a.f.flags[p];
             }
             const bool sim = (fl & 3u) != 2u;
             if (sim) {
-                if (!THREE && plain) {
-                    double lap[5];
+                if (plain) {
+                    if (!THREE) {
+                        double lap[5];
 #pragma unroll
-                    for (int c = 0; c < 5; ++c) {
-                        const double *b = rk + c * C::PLANE + idx;
-                        lap[c] = ((b[-1] + b[1]) + (b[-C::BXW] + b[C::BXW]) + (qm[c] + qp[c])) - 6.0 * qc[c];
+                        for (int c = 0; c < 5; ++c) {
+                            const double *b = rk + c * C::PLANE + idx;
+                            lap[c] = ((b[-1] + b[1]) + (b[-C::BXW] + b[C::BXW]) + (qm[c] + qp[c])) - 6.0 * qc[c];
+                        }
+                        lqs::bulk_force_oneconst(a.ph, qc, lap, Fn);
+                    } else {
+                        const double *rkm = reinterpret_cast<const double *>(smem + C::OFF_RING + ((j - 2) % 3) * C::RING_STRIDE);
+                        auto get = [&](int c, int dx, int dy, int dz) -> double {
+                            if (dz == 0) return rk[c * C::PLANE + idx + dy * C::BXW + dx];
+                            if (dx == 0 && dy == 0) return dz < 0 ? qm[c] : qp[c];
+                            return (dz < 0 ? rkm : rn)[c * C::PLANE + idx + dy * C::BXW + dx];
+                        };
+                        lqs::bulk_force_threeconst(a.ph, get, qc, Fn);
                     }
-                    lqs::bulk_force_oneconst(a.ph, qc, lap, Fn);
                 } else {
                     RingAcc<C> acc;
                     acc.pl[0] = reinterpret_cast<const double *>(smem + C::OFF_RING + ((j - 2) % 3) * C::RING_STRIDE);
@@ -282,6 +294,9 @@ struct LqSweepPlan {
     bool three = false, stored = true;
     double *partials = nullptr;
     unsigned int *counter = nullptr;
+    uint8_t *plain = nullptr, *tsum = nullptr;   // masked lattices: per-site and per-(plane, tile) 'plain' maps
+    const uint8_t *flags_seen = nullptr;
+    bool sites_dirty = true;
     dim3 grid;
     int zc = 0;
     bool attr_set[4] = {false, false, false, false};
@@ -291,9 +306,13 @@ void lq_sweep_destroy(LqSweepPlan *p) {
     if (!p) return;
     cudaFree(p->partials);
     cudaFree(p->counter);
+    cudaFree(p->plain);
+    cudaFree(p->tsum);
     delete p;
 }
-void lq_sweep_invalidate(LqSweepPlan *) {}
+void lq_sweep_invalidate(LqSweepPlan *p) {
+    if (p) p->sites_dirty = true;
+}
 
 template <class C, bool THREE, bool MASKED>
 static cudaError_t launch(LqSweepPlan *pl, int in, const SweepArgs &a, int variant, cudaStream_t st) {
@@ -311,7 +330,7 @@ int lq_sweep_run(LqSweepPlan **planp, bool stored_F, const LqGeom &g, const LqPh
                  double *v[2], double *F[2], int *cur, LqFireScalars *dsc, const LqFireConsts &fc, long max_steps,
                  cudaStream_t st, long *launches, long *sweeps, LqFireScalars *h, std::string &err) {
     using C1 = Cfg<32, 16>;   // one-constant: 512 threads, <= 128 registers
-    using C3 = Cfg<32, 8>;    // three-constant: 256 threads, <= 255 registers
+    using C3 = Cfg<32, 16>;   // three-constant: same tile (ptxas fits the 19-point fast path in 128 registers)
     const bool three = ph.L2 != 0.0 || ph.L3 != 0.0;
     const bool masked = f.flags != nullptr;
     LqSweepPlan *pl = *planp;
@@ -340,8 +359,19 @@ int lq_sweep_run(LqSweepPlan **planp, bool stored_F, const LqGeom &g, const LqPh
         pl->stored = stored_F;
         const int ntx = (g.Lx + TX - 1) / TX, nty = (g.Ly + TY - 1) / TY;
         // z-chunk: aim for >= 4 CTAs per SM worth of work items, chunk >= 8 planes, <= 64
-        int zc = getenv("LQ_ZC") ? atoi(getenv("LQ_ZC")) : 64;
-        while (zc > 8 && (long long)ntx * nty * ((g.Lz + zc - 1) / zc) < 4 * 148) zc >>= 1;
+        // z-chunking: equal chunks; pick the chunk count that minimises the modelled makespan
+        //   waves(ntiles * nzc / 148 SMs, 1 CTA/SM) * (planes per chunk + halo planes + pipeline fill)
+        const int halo_planes = stored_F ? 2 : 4;
+        long long best = -1;
+        int zc = g.Lz;
+        for (int nzc = 1; nzc <= (g.Lz + 7) / 8; ++nzc) {
+            const int c = (g.Lz + nzc - 1) / nzc;
+            if (c > 64 && nzc < (g.Lz + 63) / 64) continue;
+            const long long ncta = (long long)ntx * nty * ((g.Lz + c - 1) / c);
+            const long long cost = ((ncta + 147) / 148) * (c + halo_planes + 3);
+            if (best < 0 || cost < best) { best = cost; zc = c; }
+        }
+        if (getenv("LQ_ZC")) zc = atoi(getenv("LQ_ZC"));
         if (zc > g.Lz) zc = g.Lz;
         pl->zc = zc;
         pl->grid = dim3(ntx, nty, (g.Lz + zc - 1) / zc);
@@ -354,6 +384,18 @@ int lq_sweep_run(LqSweepPlan **planp, bool stored_F, const LqGeom &g, const LqPh
             return LQ_ERR_NOMEM;
         }
     }
+    if (masked && (pl->sites_dirty || rebuild || pl->flags_seen != f.flags)) {
+        const size_t nts = (size_t)pl->grid.x * pl->grid.y * (g.Lz + 2);
+        if (!pl->plain && cudaMalloc(&pl->plain, (size_t)g.NP) != cudaSuccess) { err = "lq_sweep: cudaMalloc failed"; return LQ_ERR_NOMEM; }
+        cudaFree(pl->tsum); pl->tsum = nullptr;
+        if (cudaMalloc(&pl->tsum, nts) != cudaSuccess) { err = "lq_sweep: cudaMalloc failed"; return LQ_ERR_NOMEM; }
+        cudaMemsetAsync(pl->plain, 0, (size_t)g.NP, st);
+        lq_launch_plain_map(g, f.flags, pl->plain, st);
+        lq_launch_tile_summary(g, pl->plain, pl->tsum, TX, TY, pl->grid.x, pl->grid.y, st);
+        *launches += 2;
+        pl->sites_dirty = false;
+        pl->flags_seen = f.flags;
+    }
     cudaError_t e = cudaMemsetAsync(pl->counter, 0, sizeof(unsigned int), st);
     if (e != cudaSuccess) { err = cudaGetErrorString(e); return LQ_ERR_CUDA; }
     if (stored_F) {   // F of the entry state was written by the generic kernel without its ghost shell
@@ -365,6 +407,7 @@ int lq_sweep_run(LqSweepPlan **planp, bool stored_F, const LqGeom &g, const LqPh
     SweepArgs a;
     a.g = g; a.ph = ph; a.f = f; a.sc = dsc; a.fc = fc; a.partials = pl->partials; a.counter = pl->counter; a.zc = pl->zc;
     a.store_cs = getenv("LQ_STORE_CS") ? atoi(getenv("LQ_STORE_CS")) : 0;
+    a.plain = pl->plain; a.tsum = pl->tsum;
     const long chunk = fc.force_tol > 0.0 ? 100 : (1L << 30);
     long done = 0;
     while (done < max_steps) {

@@ -17,6 +17,8 @@ struct SweepArgs {
     unsigned int *counter;
     int zc;
     int store_cs;
+    const uint8_t *plain;   // per-site 'constant stencil weights' byte (masked lattices)
+    const uint8_t *tsum;    // per (plane, tile): tile + halo all plain
 };
 
 // ---------------------------------------------------------------- PTX wrappers (TMA + mbarrier)

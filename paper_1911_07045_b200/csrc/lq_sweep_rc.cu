@@ -31,7 +31,8 @@ struct RC {
     static constexpr int OFF_N = OFF_V + NV * V_STRIDE;
     static constexpr int OFF_BAR = OFF_N + NN * N_STRIDE;
     static constexpr int OFF_RED = OFF_BAR + 64;
-    static constexpr int SMEM_BYTES = OFF_RED + 4 * (NT / 32) * 8 + 64;
+    static constexpr int OFF_TS = OFF_RED + 4 * (NT / 32) * 8;     // tile summaries of this CTA's planes (<= 80)
+    static constexpr int SMEM_BYTES = OFF_TS + 128;
     static constexpr int NHALO = 2 * BXW + 2 * (BYH - 2);
 };
 static_assert(RC::SMEM_BYTES <= 232448, "shared memory budget");
@@ -75,13 +76,6 @@ struct NewAcc {
     }
 };
 
-__device__ __forceinline__ bool plain_site(const uint8_t *fl, long long p, long long sy, long long sz, unsigned &own) {
-    own = fl[p];
-    return (own >> 2) == 0x3Fu && (own & 3u) == 0u && (fl[p + 1] >> 2) == 0x3Fu && (fl[p - 1] >> 2) == 0x3Fu &&
-           (fl[p + sy] >> 2) == 0x3Fu && (fl[p - sy] >> 2) == 0x3Fu && (fl[p + sz] >> 2) == 0x3Fu &&
-           (fl[p - sz] >> 2) == 0x3Fu;
-}
-
 __device__ __forceinline__ void load_anchor(const LqFields &f, long long NP, long long p, unsigned fl, int &kind,
                                             double &W, double n[3]) {
     kind = 0; W = 0.0; n[0] = n[1] = n[2] = 0.0;
@@ -114,6 +108,9 @@ k_sweep_rc(const __grid_constant__ CUtensorMap tq, const __grid_constant__ CUten
         for (int i = 0; i < RC::NQ; ++i) mbar_init(&full[i], 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
+    uint8_t *ts = smem + RC::OFF_TS;              // ts[i] = summary of plane zb-1+i
+    if (MASKED && tid < ze - zb + 2)
+        ts[tid] = a.tsum[((size_t)(zb + tid) * gridDim.y + blockIdx.y) * gridDim.x + blockIdx.x];
     __syncthreads();
 
     // issue(j): raw q plane zb-2+j -> q slot j%4; with it (j >= 2) vc plane zb-3+j -> v slot (j-1)%2
@@ -135,6 +132,7 @@ k_sweep_rc(const __grid_constant__ CUtensorMap tq, const __grid_constant__ CUten
 #pragma unroll
     for (int c = 0; c < 5; ++c) qm[c] = qc[c] = qp[c] = vk0[c] = vk1[c] = 0.0;
     double r[4] = {0.0, 0.0, 0.0, 0.0};
+    bool tp2 = true, tp_prev = true;
 
     // halo share: perimeter cell (hx, hy) of the 34 x 18 q' box; own cell is (tx+1, ty+1)
     int hx = -1, hy = -1;
@@ -155,6 +153,10 @@ k_sweep_rc(const __grid_constant__ CUtensorMap tq, const __grid_constant__ CUten
         const double *sv = reinterpret_cast<const double *>(smem + RC::OFF_V + ((j - 1) & 1) * RC::V_STRIDE);
         double *rn = reinterpret_cast<double *>(smem + RC::OFF_N + (j & 1) * RC::N_STRIDE);         // q'(zc)
 
+        // tile + halo all "plain" at plane zc?  (uniform per CTA; skips every per-site flag access)
+        tp2 = tp_prev;                             // summary of plane zc-1 (phase 2's plane)
+        const bool tp1 = !MASKED || ts[zc - zb + 1] != 0;
+        tp_prev = tp1;
         // ---- phase 1: F(q) and q' at (cx_, cy_) in q'-box coordinates; returns v_k for the own cell
         auto first = [&](int cx_, int cy_, double vk[5], double qn[5]) {
             const int ridx = (cy_ + 1) * RC::RW + cx_ + 1;
@@ -171,10 +173,10 @@ k_sweep_rc(const __grid_constant__ CUtensorMap tq, const __grid_constant__ CUten
             bool plain = true, sim = true;
             unsigned fl = 0xFCu;
             long long p = 0;
-            if (MASKED) {
+            if (MASKED && !tp1) {
                 p = a.g.pidx(gx, gy, zc);
-                plain = plain_site(a.f.flags, p, a.g.sy, a.g.sz, fl);
-                sim = (fl & 3u) != 2u;
+                plain = a.plain[p] != 0;
+                if (!plain) { fl = a.f.flags[p]; sim = (fl & 3u) != 2u; }
             }
             if (plain) {
                 double lap[5];
@@ -225,7 +227,10 @@ k_sweep_rc(const __grid_constant__ CUtensorMap tq, const __grid_constant__ CUten
             double Fn[5] = {0.0, 0.0, 0.0, 0.0, 0.0}, vn[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
             unsigned fl = 0xFCu;
             bool plain = true;
-            if (MASKED) plain = plain_site(a.f.flags, p, a.g.sy, a.g.sz, fl);
+            if (MASKED && !tp2) {
+                plain = a.plain[p] != 0;
+                if (!plain) fl = a.f.flags[p];
+            }
             const bool sim = (fl & 3u) != 2u;
             if (sim) {
                 if (plain) {

@@ -361,7 +361,7 @@ int lq_fire_minimize(lq_ctx *c, long max_steps, double force_tol, const lq_fire_
     if (fused) {
         if ((rc = ensure_field(c, &c->q[c->cur ^ 1])) != LQ_OK) return rc;
         if ((rc = ensure_field(c, &c->v[c->cur ^ 1])) != LQ_OK) return rc;
-        if (stored_F && (rc = ensure_field(c, &c->F[c->cur ^ 1])) != LQ_OK) return rc;
+        if ((stored_F || c->flags_active) && (rc = ensure_field(c, &c->F[c->cur ^ 1])) != LQ_OK) return rc;
     }
     const int nb1 = lq_fire1_num_blocks(g);
     if ((rc = ensure_partials(c, (size_t)4 * nb1)) != LQ_OK) return rc;

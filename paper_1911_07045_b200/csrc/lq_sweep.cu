@@ -54,23 +54,6 @@ struct Cfg {
     static constexpr int NHALO = 2 * BXW + 2 * (BYH - 2);
 };
 
-// accessor over the shared-memory ring of q' planes (k-1, k, k+1); flags come from global memory
-template <class C>
-struct RingAcc {
-    const double *pl[3];
-    int idx;
-    const uint8_t *flags;
-    long long sy, sz, p;
-    __device__ __forceinline__ void Q(int dx, int dy, int dz, double o[6]) const {
-        const double *b = pl[dz + 1] + idx + dy * C::BXW + dx;
-        o[0] = b[0]; o[1] = b[C::PLANE]; o[2] = b[2 * C::PLANE]; o[3] = b[3 * C::PLANE]; o[4] = b[4 * C::PLANE];
-        o[5] = -o[0] - o[3];
-    }
-    __device__ __forceinline__ unsigned flag(int dx, int dy, int dz) const {
-        return flags ? (unsigned)flags[p + dx + dy * sy + dz * sz] : 0xFCu;
-    }
-};
-
 template <class C, bool THREE, bool MASKED>
 __global__ void __launch_bounds__(C::NT, 1)
 k_sweep(const __grid_constant__ CUtensorMap tq, const __grid_constant__ CUtensorMap tv,
@@ -192,42 +175,35 @@ k_sweep(const __grid_constant__ CUtensorMap tq, const __grid_constant__ CUtensor
                         };
                         lqs::bulk_force_threeconst(a.ph, get, qc, Fn);
                     }
-                } else {
-                    RingAcc<C> acc;
-                    acc.pl[0] = reinterpret_cast<const double *>(smem + C::OFF_RING + ((j - 2) % 3) * C::RING_STRIDE);
-                    acc.pl[1] = rk;
-                    acc.pl[2] = rn;
-                    acc.idx = idx; acc.flags = MASKED ? a.f.flags : nullptr;
-                    acc.sy = a.g.sy; acc.sz = a.g.sz; acc.p = p;
-                    int kind = 0; double W = 0.0, n[3] = {0.0, 0.0, 0.0};
-                    if (MASKED && a.f.kind != nullptr && (fl & 3u) == 1u) {
-                        kind = a.f.kind[p];
-                        if (kind != 0) { W = a.f.W[p]; n[0] = a.f.axis[p]; n[1] = a.f.axis[NP + p]; n[2] = a.f.axis[2 * NP + p]; }
-                    }
-                    lqs::site_force<THREE>(a.ph, acc, fl, kind, W, n, Fn);
-                }
 #pragma unroll
-                for (int c = 0; c < 5; ++c) {
-                    vn[c] = __fma_rn(hdt, Fn[c], vk0[c]);
-                    r[0] = __fma_rn(Fn[c], vn[c], r[0]);
-                    r[1] = __fma_rn(Fn[c], Fn[c], r[1]);
-                    r[2] = __fma_rn(vn[c], vn[c], r[2]);
-                    r[3] = fmax(r[3], fabs(Fn[c]));
+                    for (int c = 0; c < 5; ++c) {
+                        vn[c] = __fma_rn(hdt, Fn[c], vk0[c]);
+                        r[0] = __fma_rn(Fn[c], vn[c], r[0]);
+                        r[1] = __fma_rn(Fn[c], Fn[c], r[1]);
+                        r[2] = __fma_rn(vn[c], vn[c], r[2]);
+                        r[3] = fmax(r[3], fabs(Fn[c]));
+                    }
+                } else {
+                    // non-plain site: leave v_k in the velocity slot; the fix-up kernel computes F', adds
+                    // dt/2 F' and writes the force slot (and both ghost images)
+#pragma unroll
+                    for (int c = 0; c < 5; ++c) vn[c] = vk0[c];
                 }
             }
+            const bool store_F = !(sim && !plain);
             if (a.store_cs) {
 #pragma unroll
                 for (int c = 0; c < 5; ++c) {
                     __stcs(a.qo + c * NP + p, qc[c]);
                     __stcs(a.vo + c * NP + p, vn[c]);
-                    __stcs(a.Fo + c * NP + p, Fn[c]);
+                    if (store_F) __stcs(a.Fo + c * NP + p, Fn[c]);
                 }
             } else {
 #pragma unroll
                 for (int c = 0; c < 5; ++c) {
                     a.qo[c * NP + p] = qc[c];
                     a.vo[c * NP + p] = vn[c];
-                    a.Fo[c * NP + p] = Fn[c];
+                    if (store_F) a.Fo[c * NP + p] = Fn[c];
                 }
             }
             // periodic ghost shell of the outputs (width LQ_GW)
@@ -242,7 +218,7 @@ k_sweep(const __grid_constant__ CUtensorMap tq, const __grid_constant__ CUtensor
                     for (int c = 0; c < 5; ++c) {
                         a.qo[c * NP + pg] = qc[c];
                         a.vo[c * NP + pg] = vn[c];
-                        a.Fo[c * NP + pg] = Fn[c];
+                        if (store_F) a.Fo[c * NP + pg] = Fn[c];
                     }
                 }
             }
@@ -295,6 +271,10 @@ struct LqSweepPlan {
     double *partials = nullptr;
     unsigned int *counter = nullptr;
     uint8_t *plain = nullptr, *tsum = nullptr;   // masked lattices: per-site and per-(plane, tile) 'plain' maps
+    int *np_list = nullptr;                      // index-ordered non-plain simulated sites (fix-up kernel)
+    int n_np = 0;
+    double *partials2 = nullptr;
+    unsigned int *counter2 = nullptr;
     const uint8_t *flags_seen = nullptr;
     bool sites_dirty = true;
     dim3 grid;
@@ -308,6 +288,9 @@ void lq_sweep_destroy(LqSweepPlan *p) {
     cudaFree(p->counter);
     cudaFree(p->plain);
     cudaFree(p->tsum);
+    cudaFree(p->np_list);
+    cudaFree(p->partials2);
+    cudaFree(p->counter2);
     delete p;
 }
 void lq_sweep_invalidate(LqSweepPlan *p) {
@@ -393,12 +376,17 @@ int lq_sweep_run(LqSweepPlan **planp, bool stored_F, const LqGeom &g, const LqPh
         lq_launch_plain_map(g, f.flags, pl->plain, st);
         lq_launch_tile_summary(g, pl->plain, pl->tsum, TX, TY, pl->grid.x, pl->grid.y, st);
         *launches += 2;
+        if (lq_fixup_build_list(g, f.flags, pl->plain, &pl->np_list, &pl->n_np, st) != 0) { err = "lq_sweep: building the non-plain site list failed"; return LQ_ERR_NOMEM; }
+        cudaFree(pl->partials2); pl->partials2 = nullptr;
+        if (cudaMalloc(&pl->partials2, (size_t)4 * lq_fixup_num_blocks(pl->n_np) * sizeof(double)) != cudaSuccess ||
+            (!pl->counter2 && cudaMalloc(&pl->counter2, sizeof(unsigned int)) != cudaSuccess)) { err = "lq_sweep: cudaMalloc failed"; return LQ_ERR_NOMEM; }
+        cudaMemsetAsync(pl->counter2, 0, sizeof(unsigned int), st);
         pl->sites_dirty = false;
         pl->flags_seen = f.flags;
     }
     cudaError_t e = cudaMemsetAsync(pl->counter, 0, sizeof(unsigned int), st);
     if (e != cudaSuccess) { err = cudaGetErrorString(e); return LQ_ERR_CUDA; }
-    if (stored_F) {   // F of the entry state was written by the generic kernel without its ghost shell
+    if (stored_F || masked) {   // F of the entry state was written by the generic kernel without its ghost shell
         lq_launch_fill_ghosts_f64(g, F[*cur], 5, st);
         *launches += 1;
     }
@@ -408,20 +396,25 @@ int lq_sweep_run(LqSweepPlan **planp, bool stored_F, const LqGeom &g, const LqPh
     a.g = g; a.ph = ph; a.f = f; a.sc = dsc; a.fc = fc; a.partials = pl->partials; a.counter = pl->counter; a.zc = pl->zc;
     a.store_cs = getenv("LQ_STORE_CS") ? atoi(getenv("LQ_STORE_CS")) : 0;
     a.plain = pl->plain; a.tsum = pl->tsum;
+    a.defer_advance = masked ? 1 : 0;
+    const int ncta = (int)(pl->grid.x * pl->grid.y * pl->grid.z);
     const long chunk = fc.force_tol > 0.0 ? 100 : (1L << 30);
     long done = 0;
     while (done < max_steps) {
         const long n = (max_steps - done) < chunk ? (max_steps - done) : chunk;
         for (long i = 0; i < n; ++i) {
             const int in = (int)((cur0 + done + i) & 1), out = in ^ 1;
-            a.qo = q[out]; a.vo = v[out]; a.Fo = F[out];
+            a.qo = q[out]; a.vo = v[out]; a.Fo = F[out]; a.Fi = F[in];
             if (!stored_F) e = lq_launch_sweep_rc(masked, pl->grid, pl->mq[in], pl->mv[in], a, st);
             else if (three) e = masked ? launch<C3, true, true>(pl, in, a, 3, st) : launch<C3, true, false>(pl, in, a, 2, st);
             else e = masked ? launch<C1, false, true>(pl, in, a, 1, st) : launch<C1, false, false>(pl, in, a, 0, st);
+            if (e == cudaSuccess && masked)
+                e = lq_launch_fixup(three, g, ph, f, q[out], v[out], F[out], pl->np_list, pl->n_np, dsc, fc, pl->partials,
+                                    ncta, pl->partials2, pl->counter2, st);
             if (e != cudaSuccess) { err = std::string("lq_sweep launch: ") + cudaGetErrorString(e); return LQ_ERR_CUDA; }
         }
         done += n;
-        *launches += n; *sweeps += n;
+        *launches += masked ? 2 * n : n; *sweeps += n;
         if (fc.force_tol > 0.0) {
             e = cudaMemcpyAsync(h, dsc, sizeof(*h), cudaMemcpyDeviceToHost, st);
             if (e == cudaSuccess) e = cudaStreamSynchronize(st);

@@ -24,3 +24,11 @@ int lq_sweep_rc_box(int which, int dim);
 int lq_sweep_rc_tile(int dim);
 cudaError_t lq_launch_sweep_rc(bool masked, dim3 grid, const CUtensorMap &mq, const CUtensorMap &mv,
                                const lqsw::SweepArgs &a, cudaStream_t st);
+
+// fix-up kernel for the non-plain sites of masked lattices (lq_fixup.cu)
+int lq_fixup_build_list(const LqGeom &g, const uint8_t *flags, const uint8_t *plain, int **list, int *n, cudaStream_t st);
+int lq_fixup_num_blocks(int n);
+cudaError_t lq_launch_fixup(bool three, const LqGeom &g, const LqPhys &ph, const LqFields &f, const double *q,
+                            double *v, double *F, const int *list, int n, LqFireScalars *sc, const LqFireConsts &fc,
+                            const double *sweep_partials, int n_sweep, double *partials, unsigned int *counter,
+                            cudaStream_t st);

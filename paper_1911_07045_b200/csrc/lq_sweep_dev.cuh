@@ -19,6 +19,8 @@ struct SweepArgs {
     int store_cs;
     const uint8_t *plain;   // per-site 'constant stencil weights' byte (masked lattices)
     const uint8_t *tsum;    // per (plane, tile): tile + halo all plain
+    const double *Fi;       // masked recompute sweep: stored force of the NON-plain sites (input buffer)
+    int defer_advance;      // masked lattices: the fix-up kernel (lq_fixup.cu) finishes the step
 };
 
 // ---------------------------------------------------------------- PTX wrappers (TMA + mbarrier)
@@ -99,8 +101,11 @@ __device__ __forceinline__ void finish_step(const SweepArgs &a, const LqFireScal
             for (int w = 1; w < NW; ++w) t[i] = i < 3 ? t[i] + red[i * NW + w] : fmax(t[i], red[i * NW + w]);
             a.partials[4 * cta + i] = t[i];
         }
-        __threadfence();
-        s_last = atomicAdd(a.counter, 1u) == ncta - 1 ? 1u : 0u;
+        if (a.defer_advance) s_last = 0u;
+        else {
+            __threadfence();
+            s_last = atomicAdd(a.counter, 1u) == ncta - 1 ? 1u : 0u;
+        }
     }
     __syncthreads();
     if (!s_last) return;

@@ -37,54 +37,6 @@ struct RC {
 };
 static_assert(RC::SMEM_BYTES <= 232448, "shared memory budget");
 
-// accessor over the raw q ring: planes z-1, z, z+1 of the ORIGINAL field, centred on a raw-box index
-struct RawAcc {
-    const double *pl[3];
-    int idx;
-    const uint8_t *flags;
-    long long sy, sz, p;
-    __device__ __forceinline__ void Q(int dx, int dy, int dz, double o[6]) const {
-        const double *b = pl[dz + 1] + idx + dy * RC::RW + dx;
-        o[0] = b[0]; o[1] = b[RC::RPLANE]; o[2] = b[2 * RC::RPLANE]; o[3] = b[3 * RC::RPLANE]; o[4] = b[4 * RC::RPLANE];
-        o[5] = -o[0] - o[3];
-    }
-    __device__ __forceinline__ unsigned flag(int dx, int dy, int dz) const {
-        return (unsigned)flags[p + dx + dy * sy + dz * sz];
-    }
-};
-
-// accessor over q': plane k in the shared-memory ring, z neighbours of the own column in registers
-struct NewAcc {
-    const double *pk;
-    const double *qm, *qc, *qp;
-    int idx;
-    const uint8_t *flags;
-    long long sy, sz, p;
-    __device__ __forceinline__ void Q(int dx, int dy, int dz, double o[6]) const {
-        if (dz == 0 && dx == 0 && dy == 0) { o[0] = qc[0]; o[1] = qc[1]; o[2] = qc[2]; o[3] = qc[3]; o[4] = qc[4]; }
-        else if (dz == 0) {
-            const double *b = pk + idx + dy * RC::BXW + dx;
-            o[0] = b[0]; o[1] = b[RC::PLANE]; o[2] = b[2 * RC::PLANE]; o[3] = b[3 * RC::PLANE]; o[4] = b[4 * RC::PLANE];
-        } else {
-            const double *r = dz < 0 ? qm : qp;   // one-constant: z neighbours only of the own column
-            o[0] = r[0]; o[1] = r[1]; o[2] = r[2]; o[3] = r[3]; o[4] = r[4];
-        }
-        o[5] = -o[0] - o[3];
-    }
-    __device__ __forceinline__ unsigned flag(int dx, int dy, int dz) const {
-        return (unsigned)flags[p + dx + dy * sy + dz * sz];
-    }
-};
-
-__device__ __forceinline__ void load_anchor(const LqFields &f, long long NP, long long p, unsigned fl, int &kind,
-                                            double &W, double n[3]) {
-    kind = 0; W = 0.0; n[0] = n[1] = n[2] = 0.0;
-    if (f.kind != nullptr && (fl & 3u) == 1u) {
-        kind = f.kind[p];
-        if (kind != 0) { W = f.W[p]; n[0] = f.axis[p]; n[1] = f.axis[NP + p]; n[2] = f.axis[2 * NP + p]; }
-    }
-}
-
 template <bool MASKED>
 __global__ void __launch_bounds__(RC::NT, 1)
 k_sweep_rc(const __grid_constant__ CUtensorMap tq, const __grid_constant__ CUtensorMap tv, const SweepArgs a) {
@@ -188,10 +140,9 @@ k_sweep_rc(const __grid_constant__ CUtensorMap tq, const __grid_constant__ CUten
                 }
                 lqs::bulk_force_oneconst(a.ph, q5, lap, F);
             } else if (sim) {
-                RawAcc acc{{ra, rb, rc}, ridx, a.f.flags, a.g.sy, a.g.sz, p};
-                int kind; double W, n[3];
-                load_anchor(a.f, NP, p, fl, kind, W, n);
-                lqs::site_force<false>(a.ph, acc, fl, kind, W, n, F);
+                // non-plain site: its force was computed by the fix-up kernel of the previous step
+#pragma unroll
+                for (int c = 0; c < 5; ++c) F[c] = a.Fi[c * NP + p];
             }
 #pragma unroll
             for (int c = 0; c < 5; ++c) {
@@ -241,19 +192,18 @@ k_sweep_rc(const __grid_constant__ CUtensorMap tq, const __grid_constant__ CUten
                         lap[c] = ((b[-1] + b[1]) + (b[-RC::BXW] + b[RC::BXW]) + (qm[c] + qp[c])) - 6.0 * qc[c];
                     }
                     lqs::bulk_force_oneconst(a.ph, qc, lap, Fn);
-                } else {
-                    NewAcc acc{rk, qm, qc, qp, idx, a.f.flags, a.g.sy, a.g.sz, p};
-                    int kind; double W, n[3];
-                    load_anchor(a.f, NP, p, fl, kind, W, n);
-                    lqs::site_force<false>(a.ph, acc, fl, kind, W, n, Fn);
-                }
 #pragma unroll
-                for (int c = 0; c < 5; ++c) {
-                    vn[c] = __fma_rn(hdt, Fn[c], vk0[c]);
-                    r[0] = __fma_rn(Fn[c], vn[c], r[0]);
-                    r[1] = __fma_rn(Fn[c], Fn[c], r[1]);
-                    r[2] = __fma_rn(vn[c], vn[c], r[2]);
-                    r[3] = fmax(r[3], fabs(Fn[c]));
+                    for (int c = 0; c < 5; ++c) {
+                        vn[c] = __fma_rn(hdt, Fn[c], vk0[c]);
+                        r[0] = __fma_rn(Fn[c], vn[c], r[0]);
+                        r[1] = __fma_rn(Fn[c], Fn[c], r[1]);
+                        r[2] = __fma_rn(vn[c], vn[c], r[2]);
+                        r[3] = fmax(r[3], fabs(Fn[c]));
+                    }
+                } else {
+                    // non-plain site: leave v_k in the velocity slot; the fix-up kernel adds dt/2 F'
+#pragma unroll
+                    for (int c = 0; c < 5; ++c) vn[c] = vk0[c];
                 }
             }
 #pragma unroll

@@ -1,0 +1,129 @@
+"""GPU parity at BASELINE.json's FULL sizes (configs 2, 3, 4, 5, 5'), in the launch configuration bench.py times.
+
+What the oracle can do at these sizes in seconds it does in full (classification, energy, force field with the
+OpenMP variant); FIRE trajectories are compared for a few steps in full (10 steps; 100 steps for config 2, and
+for configs 3 / 5 / 5' when LQ_FULL_PARITY=1 -- the 100-step runs on their declared replicas are in
+test_parity_gpu.py); config 4 (512^3, 134M sites) uses sampled sites for forces and the first FIRE step, plus
+properties that hold at any size: lattice-translation equivariance of the fused trajectory and agreement of the
+fused sweep with the unfused generic path.
+"""
+import os
+
+import numpy as np
+import pytest
+
+from paper_1911_07045_b200 import workloads as wl
+
+pytestmark = pytest.mark.gpu
+TOL_F, TOL_E, TOL_Q = 1e-10, 1e-9, 1e-8
+FULL = os.environ.get("LQ_FULL_PARITY", "0") == "1"
+
+
+@pytest.fixture(scope="module")
+def lq():
+    import torch
+    assert torch.cuda.is_available()
+    from paper_1911_07045_b200 import binding, build
+    build.build()
+    binding.load()
+    return binding
+
+
+def make_oracle(oracle_mod, c):
+    return oracle_mod.Oracle(c["Lx"], c["Ly"], c["Lz"], c["A"], c["B"], c["C"], c["L1"], c["L2"], c["L3"],
+                             mask=c["mask"], kind=c["kind"], W=c["W"], axis=c["axis"])
+
+
+@pytest.mark.parametrize("name,steps", [("2", 100), ("3", 100 if FULL else 10), ("5", 100 if FULL else 10),
+                                        ("5p", 100 if FULL else 10)])
+def test_full_size_masked_configs(lq, oracle_mod, name, steps):
+    c = wl.make_config(name)
+    ctx = lq.create_from_config(c)
+    o = make_oracle(oracle_mod, c)
+    # classification: bit-exact
+    ref = o.classify()
+    assert np.array_equal(lq.lq_get_flags(ctx), ref)
+    assert lq.lq_get_info(ctx, "n_object") == int(np.sum((ref & 3) == 2))
+    # force field and energy on the seeded initial state, every site
+    Fref = o.forces(c["q"], 1)
+    F = lq.lq_forces(ctx)
+    assert np.abs(F - Fref).max() <= TOL_F * np.abs(Fref).max()
+    del F
+    eref, tref = o.energy(c["q"], 1, terms=True)
+    assert abs(lq.lq_energy(ctx) - eref) <= TOL_E * abs(eref)
+    # FIRE: exactly `steps` fused steps vs the oracle, every site
+    rep = lq.lq_fire_minimize(ctx, steps, 0.0, c["fire"], report_energy=True)
+    qref, rref = o.fire(c["q"], steps, 0.0, c["fire"], variant=1)
+    q = lq.lq_get_Q(ctx)
+    assert rep["steps"] == steps
+    assert np.abs(q - qref).max() <= TOL_Q
+    assert abs(rep["energy"] - rref["energy"]) <= TOL_E * abs(rref["energy"])
+    assert abs(rep["dt"] - rref["dt"]) <= 1e-15 and abs(rep["alpha"] - rref["alpha"]) <= 1e-15
+    assert rep["energy"] < eref                                   # DESIGN.md R18
+    obj = c["mask"] == 1
+    assert np.array_equal(q[:, obj], c["q"][:, obj])
+    lq.lq_destroy(ctx)
+
+
+def test_config3_classification_counts(lq):
+    """integer geometry rules of DESIGN.md section 4, counted on the GPU (lattice-point counts)"""
+    c = wl.make_config("3")
+    ctx = lq.create_from_config(c)
+    L = 256
+    idx = np.arange(-128, 128)
+    n_sph = int(np.sum(idx[:, None, None] ** 2 + idx[None, :, None] ** 2 + idx[None, None, :] ** 2 <= 625))
+    n_wall = L ** 3 - (L - 2) ** 3
+    assert lq.lq_get_info(ctx, "n_object") == n_wall + n_sph
+    f = lq.lq_get_flags(ctx)
+    assert int(np.sum(((f & 3) == 1) & (c["W"] == 0.5))) == (L - 2) ** 3 - (L - 4) ** 3
+    assert lq.lq_get_info(ctx, "n_simulated") == L ** 3 - n_wall - n_sph
+    lq.lq_destroy(ctx)
+
+
+def test_config4_full_size(lq, oracle_mod):
+    """512^3 periodic quench: sampled forces, full energy, first FIRE step on sampled sites (closed form of the
+    kick-drift from the oracle's force), translation equivariance and fused-vs-unfused agreement."""
+    c = wl.make_config("4")
+    L = 512
+    N = c["N"]
+    ctx = lq.create_from_config(c)
+    o = make_oracle(oracle_mod, c)
+    rng = np.random.default_rng(4)
+    sites = rng.integers(0, L, size=(3000, 3))
+    sites[:64] = np.array([[x, y, z] for x in (0, 1, 510, 511) for y in (0, 17, 495, 511) for z in (0, 63, 64, 511)])
+    F = lq.lq_forces(ctx)
+    Fs = np.array([o.force_at(c["q"], x, y, z, 1) for x, y, z in sites])
+    sidx = sites[:, 0] + L * (sites[:, 1] + L * sites[:, 2])
+    scale = np.abs(F).max()
+    assert np.abs(F[:, sidx].T - Fs).max() <= TOL_F * scale
+    eref = o.energy(c["q"], 1)
+    assert abs(lq.lq_energy(ctx) - eref) <= TOL_E * abs(eref)
+    # one fused step: q1 = q0 + dt0 * (dt0/2) F0 at every sampled site (v0 = 0; Alg. 1)
+    dt0 = c["fire"]["dt0"]
+    rep = lq.lq_fire_minimize(ctx, 1, 0.0, c["fire"])
+    q1 = lq.lq_get_Q(ctx)
+    assert rep["steps"] == 1 and rep["sweep_launches"] == 1
+    assert np.abs(q1[:, sidx].T - (c["q"][:, sidx].T + dt0 * 0.5 * dt0 * Fs)).max() <= 1e-13
+    assert abs(rep["Fmax"] - np.abs(lq.lq_forces(ctx)).max()) <= 1e-9 * scale
+    del F
+    # K fused steps vs K unfused steps (independent generic kernels), every site
+    K = 6
+    lq.lq_set_Q(ctx, c["q"])
+    lq.lq_fire_minimize(ctx, K, 0.0, c["fire"])
+    qa = lq.lq_get_Q(ctx)
+    lq.lq_set_option(ctx, "fire_path", 1)
+    lq.lq_set_Q(ctx, c["q"])
+    lq.lq_fire_minimize(ctx, K, 0.0, c["fire"])
+    qb = lq.lq_get_Q(ctx)
+    lq.lq_set_option(ctx, "fire_path", 0)
+    assert np.abs(qa - qb).max() <= 1e-11
+    del qb
+    # translation equivariance of the fused trajectory (periodic lattice): roll by (37, 5, 130) sites
+    sh = (130, 5, 37)                                              # (z, y, x)
+    qr = np.ascontiguousarray(np.roll(c["q"].reshape(5, L, L, L), sh, axis=(1, 2, 3)).reshape(5, N))
+    lq.lq_set_Q(ctx, qr)
+    del qr
+    lq.lq_fire_minimize(ctx, K, 0.0, c["fire"])
+    qc = lq.lq_get_Q(ctx)
+    assert np.abs(qc.reshape(5, L, L, L) - np.roll(qa.reshape(5, L, L, L), sh, axis=(1, 2, 3))).max() <= 1e-11
+    lq.lq_destroy(ctx)

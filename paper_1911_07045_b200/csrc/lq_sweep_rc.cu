@@ -165,9 +165,9 @@ k_sweep_rc(const __grid_constant__ CUtensorMap tq, const __grid_constant__ CUten
 #pragma unroll
             for (int c = 0; c < 5; ++c) rn[c * RC::PLANE + idx] = qn[c];
         }
-        __syncthreads();
-        // raw slot (j-2)%4 and v slot (j-1)%2 are consumed: refill them with planes j+2
-        if (tid == 0 && j + 2 < nplanes) issue(j + 2);
+        // No barrier between the phases: phase 2 reads the q' slot written in the PREVIOUS iteration (ordered by
+        // that iteration's closing barrier) and this thread's own registers, so both phases form one
+        // instruction stream the scheduler can interleave.
 
         // ---- phase 2: F' = force(q'), second half kick, reductions, stores for plane k = zc - 1
         if (j >= 4 && active) {
@@ -226,7 +226,10 @@ k_sweep_rc(const __grid_constant__ CUtensorMap tq, const __grid_constant__ CUten
                 }
             }
         }
-        if (!(a.store_cs & 2)) __syncthreads();   // q' slot (j-1)&1 is rewritten by the next iteration's phase 1
+        // one barrier per plane: q' slot (j-1)&1 is rewritten by the next iteration's phase 1, and raw slot
+        // (j-2)%4 / v slot (j-1)%2 are consumed by every thread: refill them with planes j+2
+        __syncthreads();
+        if (tid == 0 && j + 2 < nplanes) issue(j + 2);
     }
     finish_step<RC::NT>(a, sc, r, red);
 }

@@ -280,7 +280,7 @@ __global__ void k_plain_map(LqGeom g, const uint8_t *__restrict__ flags, uint8_t
     const bool ok = flags[p] == 0xFCu && (flags[p + 1] >> 2) == 0x3Fu && (flags[p - 1] >> 2) == 0x3Fu &&
                     (flags[p + g.sy] >> 2) == 0x3Fu && (flags[p - g.sy] >> 2) == 0x3Fu &&
                     (flags[p + g.sz] >> 2) == 0x3Fu && (flags[p - g.sz] >> 2) == 0x3Fu;
-    plain[p] = ok ? 1 : 0;
+    plain[p] = ok ? 1 : ((flags[p] & 3u) == 2u ? 2 : 0);   // 1 plain, 0 non-plain simulated, 2 object
 }
 
 // tsum[(z+1)][by][bx] = 1 iff every site of tile (bx, by) plus its one-site halo is plain at plane z (z = -1 .. Lz)
@@ -289,7 +289,7 @@ __global__ void k_tile_summary(LqGeom g, const uint8_t *__restrict__ plain, uint
     int ok = 1;
     for (int i = threadIdx.x; i < (TX + 2) * (TY + 2); i += blockDim.x) {
         const int x = bx * TX - 1 + i % (TX + 2), y = by * TY - 1 + i / (TX + 2);
-        if (x <= g.Lx && y <= g.Ly && !plain[g.pidx(x, y, z)]) ok = 0;
+        if (x <= g.Lx && y <= g.Ly && plain[g.pidx(x, y, z)] != 1) ok = 0;
     }
     ok = __syncthreads_and(ok);
     if (threadIdx.x == 0) tsum[((size_t)(z + 1) * gridDim.y + by) * gridDim.x + bx] = (uint8_t)ok;

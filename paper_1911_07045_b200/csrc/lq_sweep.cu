@@ -117,8 +117,14 @@ k_sweep(const __grid_constant__ CUtensorMap tq, const __grid_constant__ CUtensor
         hsidx = hy * C::SW + hx + 1;
     }
 
+    // per-site 'plain' byte of the plane phase B handles, fetched one iteration ahead (1 plain, 0 non-plain
+    // simulated, 2 object): no dependent global load sits on the critical path of tiles that touch objects
+    unsigned pb_next = 1u;
     for (int j = 0; j < nplanes; ++j) {
         const int s = j & 1;
+        const unsigned pb = pb_next;
+        pb_next = 1u;
+        if (MASKED && active && j >= 1 && j + 1 < nplanes && ts[j - 1] == 0) pb_next = a.plain[a.g.pidx(x, y, zb + j - 1)];
         mbar_wait(&full[s], (j >> 1) & 1);
         const double *sq = reinterpret_cast<const double *>(smem + s * C::STAGE_BYTES);
         const double *sv = sq + C::FIELD_STRIDE / 8, *sF = sq + 2 * (C::FIELD_STRIDE / 8);
@@ -149,13 +155,9 @@ k_sweep(const __grid_constant__ CUtensorMap tq, const __grid_constant__ CUtensor
             const double *rk = reinterpret_cast<const double *>(smem + C::OFF_RING + ((j - 1) % 3) * C::RING_STRIDE);
             const long long p = a.g.pidx(x, y, k);
             double Fn[5] = {0.0, 0.0, 0.0, 0.0, 0.0}, vn[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
-            unsigned fl = 0xFCu;
-            bool plain = true;                    // constant stencil weights
-            if (MASKED && !tile_plain) {
-                plain = a.plain[p] != 0;
-                if (!plain) fl = a.f.flags[p];
-            }
-            const bool sim = (fl & 3u) != 2u;
+            // plain: constant stencil weights
+            const bool plain = !MASKED || tile_plain || pb == 1u;
+            const bool sim = !MASKED || tile_plain || pb != 2u;
             if (sim) {
                 if (plain) {
                     if (!THREE) {

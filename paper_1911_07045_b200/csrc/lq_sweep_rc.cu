@@ -84,7 +84,6 @@ k_sweep_rc(const __grid_constant__ CUtensorMap tq, const __grid_constant__ CUten
 #pragma unroll
     for (int c = 0; c < 5; ++c) qm[c] = qc[c] = qp[c] = vk0[c] = vk1[c] = 0.0;
     double r[4] = {0.0, 0.0, 0.0, 0.0};
-    bool tp2 = true, tp_prev = true;
 
     // halo share: perimeter cell (hx, hy) of the 34 x 18 q' box; own cell is (tx+1, ty+1)
     int hx = -1, hy = -1;
@@ -95,7 +94,20 @@ k_sweep_rc(const __grid_constant__ CUtensorMap tq, const __grid_constant__ CUten
         else { h -= 2 * RC::BXW; hy = 1 + (h >> 1); hx = (h & 1) ? RC::BXW - 1 : 0; }
     }
 
+    // per-site 'plain' bytes (1 plain, 0 non-plain simulated, 2 object) of the own cell and the halo cell,
+    // fetched one iteration ahead so that no dependent global load gates a plane of a tile that touches
+    // objects; phase 2 reuses the own-cell byte of the previous iteration (same plane)
+    const bool own_in = x <= a.g.Lx && y <= a.g.Ly;
+    const bool halo_in = hx >= 0 && x0 - 1 + hx <= a.g.Lx && y0 - 1 + hy <= a.g.Ly;
+    unsigned pbo_next = 1u, pbh_next = 1u, pbo = 1u;
     for (int j = 0; j < nplanes; ++j) {
+        const unsigned pbo_prev = pbo, pbh = pbh_next;
+        pbo = pbo_next;
+        pbo_next = pbh_next = 1u;
+        if (MASKED && j >= 1 && j + 1 < nplanes && ts[j - 1] == 0) {
+            if (own_in) pbo_next = a.plain[a.g.pidx(x, y, zb + j - 2)];
+            if (halo_in) pbh_next = a.plain[a.g.pidx(x0 - 1 + hx, y0 - 1 + hy, zb + j - 2)];
+        }
         mbar_wait(&full[j & 3], (j >> 2) & 1);
         if (j < 2) continue;                       // the first stencil needs three raw planes
         const int zc = zb + j - 3;                 // plane whose q' is produced now (zb-1 .. ze)
@@ -105,12 +117,8 @@ k_sweep_rc(const __grid_constant__ CUtensorMap tq, const __grid_constant__ CUten
         const double *sv = reinterpret_cast<const double *>(smem + RC::OFF_V + ((j - 1) & 1) * RC::V_STRIDE);
         double *rn = reinterpret_cast<double *>(smem + RC::OFF_N + (j & 1) * RC::N_STRIDE);         // q'(zc)
 
-        // tile + halo all "plain" at plane zc?  (uniform per CTA; skips every per-site flag access)
-        tp2 = tp_prev;                             // summary of plane zc-1 (phase 2's plane)
-        const bool tp1 = !MASKED || ts[zc - zb + 1] != 0;
-        tp_prev = tp1;
         // ---- phase 1: F(q) and q' at (cx_, cy_) in q'-box coordinates; returns v_k for the own cell
-        auto first = [&](int cx_, int cy_, double vk[5], double qn[5]) {
+        auto first = [&](int cx_, int cy_, unsigned pb, double vk[5], double qn[5]) {
             const int ridx = (cy_ + 1) * RC::RW + cx_ + 1;
             const int vidx = cy_ * RC::VW + cx_ + 1;
             const int gx = x0 - 1 + cx_, gy = y0 - 1 + cy_;
@@ -122,14 +130,8 @@ k_sweep_rc(const __grid_constant__ CUtensorMap tq, const __grid_constant__ CUten
                 for (int c = 0; c < 5; ++c) { vk[c] = 0.0; qn[c] = q5[c]; }
                 return;
             }
-            bool plain = true, sim = true;
-            unsigned fl = 0xFCu;
-            long long p = 0;
-            if (MASKED && !tp1) {
-                p = a.g.pidx(gx, gy, zc);
-                plain = a.plain[p] != 0;
-                if (!plain) { fl = a.f.flags[p]; sim = (fl & 3u) != 2u; }
-            }
+            const bool plain = !MASKED || pb == 1u, sim = !MASKED || pb != 2u;
+            const long long p = (MASKED && !plain) ? a.g.pidx(gx, gy, zc) : 0;
             if (plain) {
                 double lap[5];
 #pragma unroll
@@ -152,7 +154,7 @@ k_sweep_rc(const __grid_constant__ CUtensorMap tq, const __grid_constant__ CUten
         };
 #pragma unroll
         for (int c = 0; c < 5; ++c) { qm[c] = qc[c]; qc[c] = qp[c]; vk0[c] = vk1[c]; }
-        first(tx + 1, ty + 1, vk1, qp);
+        first(tx + 1, ty + 1, pbo, vk1, qp);
         {
             const int idx = (ty + 1) * RC::BXW + tx + 1;
 #pragma unroll
@@ -160,7 +162,7 @@ k_sweep_rc(const __grid_constant__ CUtensorMap tq, const __grid_constant__ CUten
         }
         if (hx >= 0 && !(a.store_cs & 1)) {
             double vk[5], qn[5];
-            first(hx, hy, vk, qn);
+            first(hx, hy, pbh, vk, qn);
             const int idx = hy * RC::BXW + hx;
 #pragma unroll
             for (int c = 0; c < 5; ++c) rn[c * RC::PLANE + idx] = qn[c];
@@ -176,13 +178,7 @@ k_sweep_rc(const __grid_constant__ CUtensorMap tq, const __grid_constant__ CUten
             const int idx = (ty + 1) * RC::BXW + tx + 1;
             const long long p = a.g.pidx(x, y, k);
             double Fn[5] = {0.0, 0.0, 0.0, 0.0, 0.0}, vn[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
-            unsigned fl = 0xFCu;
-            bool plain = true;
-            if (MASKED && !tp2) {
-                plain = a.plain[p] != 0;
-                if (!plain) fl = a.f.flags[p];
-            }
-            const bool sim = (fl & 3u) != 2u;
+            const bool plain = !MASKED || pbo_prev == 1u, sim = !MASKED || pbo_prev != 2u;
             if (sim) {
                 if (plain) {
                     double lap[5];

@@ -670,3 +670,61 @@ int lqo_fire(const lqo_problem *p, double *q, double *v_out, long max_steps, dou
     free(v); free(F);
     return 0;
 }
+
+/* ------------------------------------------- gradient descent and Nesterov
+ * the paper's comparator minimiser (gradient descent, PAPER.md:189,
+ * 205-211, "steepest descent relaxation ... overdamped molecular dynamics at zero
+ * temperature") and its second GUI minimiser (Nesterov's accelerated gradient,
+ * PAPER.md:189, 289, 445).  The paper gives neither formula nor parameters; the
+ * readings (R23, R24) are the textbook fixed-step forms:
+ *   method 0 (GD):        y_k = q_k
+ *   method 1 (Nesterov):  y_k = q_k + mu (q_k - q_{k-1}),   q_{-1} = q_0   [80]
+ *   q_{k+1} = y_k + eta F(y_k),   F = -dF/dq
+ * on simulated sites only; object sites never move.  Stop (R12) when
+ * max |F_a(y_k)| < force_tol; the step that measured it is still applied (its
+ * update is a by-product of the same pass), so steps = number of updates applied.
+ * trace, if not NULL, gets 3 doubles per step: |F|^2, max|F_a| of F(y_k), and the
+ * energy of q_{k+1} if trace_energy (else 0).                                    */
+int lqo_descent(const lqo_problem *p, double *q, int method, long max_steps, double force_tol,
+                double eta, double mu, lqo_fire_report *rep, int variant, double *trace, int trace_energy)
+{
+    const long N = (long)p->Lx * p->Ly * p->Lz;
+    long nsim = 0;
+    for (long s = 0; s < N; ++s) nsim += is_sim(p, s);
+    double *F = (double *)malloc(5 * N * sizeof(double));
+    double *y = (double *)malloc(5 * N * sizeof(double));
+    double *qprev = (double *)malloc(5 * N * sizeof(double));
+    double *zero = (double *)calloc(5 * N, sizeof(double));
+    if (!F || !y || !qprev || !zero) { free(F); free(y); free(qprev); free(zero); return -4; }
+    memcpy(qprev, q, 5 * N * sizeof(double));
+    double P = 0.0, FF = 0.0, vv = 0.0, Fmax = 0.0;
+    long step = 0;
+    int converged = 0;
+    while (!converged && step < max_steps) {
+        ++step;
+        for (long i = 0; i < 5 * N; ++i) {
+            y[i] = q[i];
+            if (method == 1 && is_sim(p, i % N)) y[i] = q[i] + mu * (q[i] - qprev[i]);
+        }
+        lqo_forces(p, y, F, variant);
+        reduce4(p, F, zero, N, &P, &FF, &vv, &Fmax);
+        if (Fmax < force_tol) converged = 1;
+        memcpy(qprev, q, 5 * N * sizeof(double));
+        for (long i = 0; i < 5 * N; ++i) {
+            if (!is_sim(p, i % N)) continue;
+            q[i] = y[i] + eta * F[i];
+        }
+        if (trace) {
+            double *t = trace + 3 * (step - 1);
+            t[0] = FF; t[1] = Fmax; t[2] = trace_energy ? lqo_energy(p, q, variant, NULL) : 0.0;
+        }
+    }
+    if (rep) {
+        rep->steps = step; rep->converged = converged;
+        rep->Fmax = Fmax; rep->Frms = nsim ? sqrt(FF / (double)nsim) : 0.0;
+        rep->P = 0.0; rep->dt = eta; rep->alpha = mu;
+        rep->energy = lqo_energy(p, q, variant, NULL);
+    }
+    free(F); free(y); free(qprev); free(zero);
+    return 0;
+}

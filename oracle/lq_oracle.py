@@ -77,6 +77,9 @@ def _load():
     L.lqo_fire.restype = C.c_int
     L.lqo_fire.argtypes = [PP, C.c_void_p, C.c_void_p, C.c_long, C.c_double,
                            C.POINTER(_FireParams), C.POINTER(_FireReport), C.c_int, C.c_void_p, C.c_int]
+    L.lqo_descent.restype = C.c_int
+    L.lqo_descent.argtypes = [PP, C.c_void_p, C.c_int, C.c_long, C.c_double, C.c_double, C.c_double,
+                              C.POINTER(_FireReport), C.c_int, C.c_void_p, C.c_int]
     _lib = L
     return L
 
@@ -173,3 +176,16 @@ class Oracle:
         if trace:
             out.append(tr[: report["steps"]])
         return tuple(out)
+
+    def descent(self, q, method, max_steps, force_tol, eta, mu=0.0, variant=1, trace=False, trace_energy=False):
+        """Fixed-step gradient descent (method 0) or Nesterov's accelerated gradient (method 1) from q (not
+        modified).  Returns (q_final, report dict[, trace])."""
+        q = self._q(q).copy()
+        rep = _FireReport()
+        tr = np.zeros((max(int(max_steps), 1), 3), dtype=np.float64) if trace else None
+        rc = self.lib.lqo_descent(C.byref(self.p), _ptr(q), int(method), int(max_steps), float(force_tol),
+                                  float(eta), float(mu), C.byref(rep), variant, _ptr(tr), int(bool(trace_energy)))
+        if rc != 0:
+            raise MemoryError("lqo_descent rc=%d" % rc)
+        report = {k: getattr(rep, k) for k, _ in _FireReport._fields_}
+        return (q, report, tr[: report["steps"]]) if trace else (q, report)

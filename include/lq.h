@@ -136,6 +136,27 @@ typedef struct {
 int lq_fire_minimize(lq_ctx *ctx, long max_steps, double force_tol,
                      const lq_fire_params *params, lq_fire_report *out);
 
+/* Other first-order minimisers on the same force.  The paper compares FIRE with gradient
+ * descent and offers Nesterov's accelerated gradient as its second minimiser
+ * without printing either update; the fixed-step textbook forms are used
+ * (R23, R24):
+ *     LQ_MIN_GD:        y_k = q_k
+ *     LQ_MIN_NESTEROV:  y_k = q_k + mu (q_k - q_{k-1}),  q_{-1} = q_0
+ *     q_{k+1} = y_k + eta F(y_k) on simulated sites; object sites never move.
+ * One kernel launch per step.  The stop test max|F_a(y_k)| < force_tol uses the force the step evaluates and
+ * the step's update is still applied, so steps = updates applied (force_tol = 0: exactly max_steps).
+ * The report reuses lq_fire_report: Fmax, Frms of F(y_k) of the last step; P = 0; dt = eta; alpha = mu.
+ * Errors: LQ_ERR_STATE before lq_set_Q; LQ_ERR_ARG on eta <= 0, mu outside [0, 1), unknown method,
+ * max_steps < 0, NULL pointers. */
+enum { LQ_MIN_GD = 0, LQ_MIN_NESTEROV = 1 };
+typedef struct {
+    double eta;          /* step size */
+    double mu;           /* momentum of LQ_MIN_NESTEROV (ignored by LQ_MIN_GD) */
+    int report_energy;
+} lq_descent_params;
+int lq_descent_minimize(lq_ctx *ctx, int method, long max_steps, double force_tol,
+                        const lq_descent_params *params, lq_fire_report *out);
+
 /* S0 of Eq. 7 for the context's A, B, C (host double). */
 int lq_get_S0(lq_ctx *ctx, double *S0);
 

@@ -23,7 +23,7 @@ _lib = None
 
 # every symbol include/lq.h declares (checked by tests/test_abi.py against the header)
 SYMBOLS = ["lq_create", "lq_destroy", "lq_set_stream", "lq_set_sites", "lq_get_flags", "lq_set_Q", "lq_get_Q",
-           "lq_get_velocity", "lq_energy", "lq_energy_terms", "lq_forces", "lq_fire_minimize", "lq_get_S0",
+           "lq_get_velocity", "lq_energy", "lq_energy_terms", "lq_forces", "lq_fire_minimize", "lq_descent_minimize", "lq_get_S0",
            "lq_set_option", "lq_get_info", "lq_last_error", "lq_version"]
 
 
@@ -43,6 +43,13 @@ class lq_fire_report(C.Structure):
     _fields_ = [("steps", C.c_long), ("converged", C.c_int), ("Fmax", C.c_double), ("Frms", C.c_double),
                 ("P", C.c_double), ("dt", C.c_double), ("alpha", C.c_double), ("energy", C.c_double),
                 ("launches", C.c_long), ("sweep_launches", C.c_long), ("gpu_ms", C.c_double)]
+
+
+class lq_descent_params(C.Structure):
+    _fields_ = [("eta", C.c_double), ("mu", C.c_double), ("report_energy", C.c_int)]
+
+
+LQ_MIN_GD, LQ_MIN_NESTEROV = 0, 1
 
 
 def lib_path() -> str:
@@ -72,6 +79,7 @@ def load():
     L.lq_energy_terms.argtypes = [vp, dp]
     L.lq_forces.argtypes = [vp, vp, ip]
     L.lq_fire_minimize.argtypes = [vp, C.c_long, C.c_double, C.POINTER(lq_fire_params), C.POINTER(lq_fire_report)]
+    L.lq_descent_minimize.argtypes = [vp, ip, C.c_long, C.c_double, C.POINTER(lq_descent_params), C.POINTER(lq_fire_report)]
     L.lq_get_S0.argtypes = [vp, dp]
     L.lq_set_option.argtypes = [vp, C.c_char_p, C.c_double]
     L.lq_get_info.argtypes = [vp, C.c_char_p, dp]
@@ -227,6 +235,15 @@ def lq_fire_minimize(ctx, max_steps, force_tol, params: dict, report_energy=Fals
                         int(bool(report_energy)))
     rep = lq_fire_report()
     _check(ctx.handle, load().lq_fire_minimize(ctx.handle, int(max_steps), float(force_tol), C.byref(fp), C.byref(rep)))
+    return {k: getattr(rep, k) for k, _ in lq_fire_report._fields_}
+
+
+def lq_descent_minimize(ctx, method, max_steps, force_tol, eta, mu=0.0, report_energy=False) -> dict:
+    """method: LQ_MIN_GD or LQ_MIN_NESTEROV; fixed step eta, momentum mu.  Returns the report as a dict."""
+    dpar = lq_descent_params(float(eta), float(mu), int(bool(report_energy)))
+    rep = lq_fire_report()
+    _check(ctx.handle, load().lq_descent_minimize(ctx.handle, int(method), int(max_steps), float(force_tol),
+                                                  C.byref(dpar), C.byref(rep)))
     return {k: getattr(rep, k) for k, _ in lq_fire_report._fields_}
 
 

@@ -30,6 +30,7 @@ struct lq_ctx {
     unsigned long long *dcounts = nullptr;
     int *dbad = nullptr;
     LqSweepPlan *sweep = nullptr;
+    LqDescentPlan *descent = nullptr;
     int fire_path = 0;
     std::string err;
 };
@@ -157,6 +158,7 @@ void lq_destroy(lq_ctx *c) {
     cudaFree(c->maskp); cudaFree(c->flags); cudaFree(c->kind); cudaFree(c->W); cudaFree(c->axis);
     cudaFree(c->partials); cudaFree(c->dscal3); cudaFree(c->dsc); cudaFree(c->dcounts); cudaFree(c->dbad);
     lq_sweep_destroy(c->sweep);
+    lq_descent_destroy(c->descent);
     delete c;
 }
 
@@ -423,6 +425,58 @@ int lq_fire_minimize(lq_ctx *c, long max_steps, double force_tol, const lq_fire_
     out->P = h.P; out->dt = h.dt; out->alpha = h.alpha;
     out->launches = launches; out->sweep_launches = sweeps; out->gpu_ms = ms;
     if (fp->report_energy) {
+        rc = lq_energy(c, &out->energy);
+        if (rc != LQ_OK) return rc;
+    }
+    return LQ_OK;
+}
+
+
+int lq_descent_minimize(lq_ctx *c, int method, long max_steps, double force_tol, const lq_descent_params *dp,
+                        lq_fire_report *out) {
+    if (!c) return LQ_ERR_ARG;
+    if (!dp || !out) return fail(c, LQ_ERR_ARG, "lq_descent_minimize: NULL pointer");
+    memset(out, 0, sizeof(*out));
+    if (!c->has_Q) return fail(c, LQ_ERR_STATE, "lq_descent_minimize: call lq_set_Q first");
+    if ((method != LQ_MIN_GD && method != LQ_MIN_NESTEROV) || !(dp->eta > 0.0) || max_steps < 0 || !(force_tol >= 0.0) ||
+        (method == LQ_MIN_NESTEROV && !(dp->mu >= 0.0 && dp->mu < 1.0)))
+        return fail(c, LQ_ERR_ARG, "lq_descent_minimize: bad parameters");
+    const LqGeom &g = c->g;
+    cudaStream_t st = c->stream;
+    int rc;
+    const int nbuf = method == LQ_MIN_NESTEROV ? 3 : 2;
+    if ((rc = ensure_field(c, &c->q[c->cur ^ 1])) != LQ_OK) return rc;
+    if (nbuf == 3 && (rc = ensure_field(c, &c->v[0])) != LQ_OK) return rc;
+    double *buf[3] = {c->q[c->cur], c->q[c->cur ^ 1], c->v[0]};
+    LqFireScalars h;
+    memset(&h, 0, sizeof(h));
+    h.dt = dp->eta; h.alpha = dp->mu;
+    LQ_CUDA(c, cudaMemcpyAsync(&c->dsc[0], &h, sizeof(h), cudaMemcpyHostToDevice, st));
+    cudaEvent_t ev0, ev1;
+    LQ_CUDA(c, cudaEventCreate(&ev0));
+    LQ_CUDA(c, cudaEventCreate(&ev1));
+    LQ_CUDA(c, cudaEventRecord(ev0, st));
+    long launches = 0;
+    int fin = 0;
+    rc = lq_descent_run(&c->descent, method, g, c->ph, fields_of(c), buf, nbuf, &fin, c->dsc, dp->eta, dp->mu, force_tol,
+                        max_steps, st, &launches, &h, c->err);
+    if (rc == LQ_OK) {
+        cudaEventRecord(ev1, st);
+        cudaStreamSynchronize(st);
+    }
+    float ms = 0.f;
+    if (rc == LQ_OK) cudaEventElapsedTime(&ms, ev0, ev1);
+    cudaEventDestroy(ev0); cudaEventDestroy(ev1);
+    if (rc != LQ_OK) return rc;
+    // make the buffer that holds the last iterate the live one
+    if (fin == 1) c->cur ^= 1;
+    else if (fin == 2) { double *t = c->q[c->cur]; c->q[c->cur] = c->v[0]; c->v[0] = t; }
+    const double nsim = (double)(c->flags_active ? c->n_class[0] + c->n_class[1] : (unsigned long long)g.N);
+    out->steps = (long)h.step; out->converged = h.converged;
+    out->Fmax = h.Fmax; out->Frms = nsim > 0 ? sqrt(h.FF / nsim) : 0.0;
+    out->P = 0.0; out->dt = dp->eta; out->alpha = dp->mu;
+    out->launches = launches; out->sweep_launches = launches; out->gpu_ms = ms;
+    if (dp->report_energy) {
         rc = lq_energy(c, &out->energy);
         if (rc != LQ_OK) return rc;
     }

@@ -17,6 +17,14 @@ int lq_sweep_run(LqSweepPlan **plan, bool stored_F, const LqGeom &g, const LqPhy
                  double *v[2], double *F[2], int *cur, LqFireScalars *dsc, const LqFireConsts &fc, long max_steps,
                  cudaStream_t st, long *launches, long *sweeps, LqFireScalars *h, std::string &err);
 
+// gradient descent / Nesterov (lq_descent.cu): one launch per step; buf[0] holds q_0, nbuf rotating buffers
+struct LqDescentPlan;
+void lq_descent_destroy(LqDescentPlan *plan);
+int lq_descent_run(LqDescentPlan **plan, int method, const LqGeom &g, const LqPhys &ph, const LqFields &f,
+                   double *const *buf, int nbuf, int *final, LqFireScalars *dsc, double eta, double mu,
+                   double force_tol, long max_steps, cudaStream_t st, long *launches, LqFireScalars *h,
+                   std::string &err);
+
 // recompute-F kernel (lq_sweep_rc.cu)
 #include <cuda.h>
 namespace lqsw { struct SweepArgs; }

@@ -204,6 +204,10 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--fire-path", type=int, default=0)
+    ap.add_argument("--method", default="fire", choices=["fire", "gd", "nesterov"],
+                    help="minimiser whose step is timed (default: FIRE, the headline metric; gd / nesterov: SURVEY 8(f1))")
+    ap.add_argument("--eta", type=float, default=0.004)
+    ap.add_argument("--mu", type=float, default=0.8)
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
@@ -241,8 +245,17 @@ def main():
     hout = torch.empty((5, N), dtype=torch.float64, pin_memory=True)
     lq.lq_set_Q(ctx, hq)
 
+    if args.method == "fire":
+        def minimize(steps):
+            return lq.lq_fire_minimize(ctx, steps, 0.0, c["fire"])
+    else:
+        meth = lq.LQ_MIN_GD if args.method == "gd" else lq.LQ_MIN_NESTEROV
+
+        def minimize(steps):
+            return lq.lq_descent_minimize(ctx, meth, steps, 0.0, args.eta, args.mu)
+
     # warm-up: W steps (also builds the sweep plan / tensor maps)
-    lq.lq_fire_minimize(ctx, W, 0.0, c["fire"])
+    minimize(W)
     torch.cuda.synchronize()
     if dist is not None:
         dist.barrier()
@@ -251,7 +264,7 @@ def main():
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     torch.cuda.synchronize()
     e0.record(stream)
-    rep = lq.lq_fire_minimize(ctx, K, 0.0, c["fire"])
+    rep = minimize(K)
     e1.record(stream)
     torch.cuda.synchronize()
     clocks = sampler.stop()
@@ -270,14 +283,15 @@ def main():
             dist.barrier()
         t0 = time.perf_counter()
         lq.lq_set_Q(ctx, hq)
-        rep2 = lq.lq_fire_minimize(ctx, K, 0.0, c["fire"])
+        rep2 = minimize(K)
         lq.lq_get_Q(ctx, hout)
         torch.cuda.synchronize()
         t_e2e = (time.perf_counter() - t0) * 1e3
         t_max, units2 = aggregate(t_e2e, nsim * K, world, dist, torch.device("cuda", local))
         e2e = {"value": units2 / (t_max * 1e-3), "unit": UNIT, "h2d_bytes_per_step": 40.0 * N / K,
                "d2h_bytes_per_step": 40.0 * N / K, "ms_total": t_max,
-               "call": "lq_set_Q(pinned host) + lq_fire_minimize(%d) + lq_get_Q(pinned host)" % K}
+               "call": "lq_set_Q(pinned host) + %s(%d) + lq_get_Q(pinned host)" % (
+                   "lq_fire_minimize" if args.method == "fire" else "lq_descent_minimize", K)}
 
     if rank != 0:
         if dist is not None:
@@ -286,19 +300,25 @@ def main():
 
     peak, peak_kind = measured_hbm_peak()
     flag_byte = 1.0 if lq.lq_get_info(ctx, "n_object") > 0 else 0.0
-    alg_bytes_site = 160.0 + flag_byte                       # read+write q and v (+ flag byte)
+    # FIRE reads + writes q and v (+ flag byte).  GD: read q, write q; Nesterov: read q_k, q_{k-1}, write q_{k+1}
+    alg_bytes_site = {"fire": 160.0, "gd": 80.0, "nesterov": 120.0}[args.method] + flag_byte
     launch_ms = ms / max(rep["sweep_launches"], 1)           # average launch duration over the timed region
     achieved = alg_bytes_site * N / (launch_ms * 1e-3) / 1e9
-    design_bytes_site = lq.lq_get_info(ctx, "sweep_bytes_per_site")
+    design_bytes_site = lq.lq_get_info(ctx, "sweep_bytes_per_site") if args.method == "fire" else alg_bytes_site
+    three = c["L2"] != 0 or c["L3"] != 0
+    if args.method != "fire":
+        kernel_name = "k_descent" if (three or args.fire_path == 1) else "k_descent_sweep"
+    else:
+        kernel_name = {1: "k_fire1_force"}.get(args.fire_path, "k_sweep" if (three or args.fire_path == 2) else "k_sweep_rc")
     traffic = None
-    tpath = os.path.join(ROOT, "profiles", "traffic_cfg%s.json" % args.workload)
+    tpath = os.path.join(ROOT, "profiles", "traffic_cfg%s%s.json" % (args.workload, "" if args.method == "fire" else "_" + args.method))
     if os.path.exists(tpath):
         try:
             traffic = json.load(open(tpath)).get("dram_bytes_per_launch")
         except Exception:
             traffic = None
     roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                "traffic": traffic, "peak_kind": peak_kind, "kernel": "k_sweep",
+                "traffic": traffic, "peak_kind": peak_kind, "kernel": kernel_name,
                 "algorithmic_bytes_per_site": alg_bytes_site, "design_bytes_per_site": design_bytes_site,
                 "achieved_design_GBs": design_bytes_site * N / (launch_ms * 1e-3) / 1e9,
                 "launch_ms": launch_ms}
@@ -308,13 +328,14 @@ def main():
         v, cores, desc, _, _ = time_oracle(c, target_s=15.0, crop=args.ref_crop)
         cpu = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc}
 
-    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+    metric = METRIC if args.method == "fire" else METRIC.replace("FIRE", {"gd": "gradient-descent", "nesterov": "Nesterov"}[args.method])
+    line = {"metric": metric, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
             "ms_per_step": ms_max / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic",
             "config": {"workload": c["name"], "lattice": [c["Lx"], c["Ly"], c["Lz"]], "n_simulated": nsim,
                        "elastic": "L1" if c["L2"] == 0 and c["L3"] == 0 else "L1+L2+L3",
                        "l2": "inputs_larger_than_L2" if 120.0 * N > 126e6 * 4 else "L2_resident_no_flush",
-                       "multi_gpu": "replicas only", "fire_path": args.fire_path},
+                       "multi_gpu": "replicas only", "fire_path": args.fire_path, "method": args.method},
             "clocks": clocks, "e2e": e2e, "gpu_launches": rep["launches"], "roofline": roofline,
             "cpu_baseline": cpu}
     print(json.dumps(line), flush=True)

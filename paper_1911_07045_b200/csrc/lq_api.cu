@@ -176,6 +176,7 @@ int lq_set_sites(lq_ctx *c, const uint8_t *mask, const uint8_t *anch_kind, const
     const LqGeom &g = c->g;
     cudaStream_t st = c->stream;
     lq_sweep_invalidate(c->sweep);
+    lq_descent_invalidate(c->descent);
     if (!mask) {
         c->flags_active = false; c->anch_active = false;
         c->n_class[0] = (unsigned long long)g.N; c->n_class[1] = c->n_class[2] = 0;
@@ -456,10 +457,10 @@ int lq_descent_minimize(lq_ctx *c, int method, long max_steps, double force_tol,
     LQ_CUDA(c, cudaEventCreate(&ev0));
     LQ_CUDA(c, cudaEventCreate(&ev1));
     LQ_CUDA(c, cudaEventRecord(ev0, st));
-    long launches = 0;
+    long launches = 0, sweeps = 0;
     int fin = 0;
-    rc = lq_descent_run(&c->descent, method, g, c->ph, fields_of(c), buf, nbuf, &fin, c->dsc, dp->eta, dp->mu, force_tol,
-                        max_steps, st, &launches, &h, c->err);
+    rc = lq_descent_run(&c->descent, method, c->fire_path == 1 ? 1 : 0, g, c->ph, fields_of(c), buf, nbuf, &fin, c->dsc,
+                        dp->eta, dp->mu, force_tol, max_steps, st, &launches, &sweeps, &h, c->err);
     if (rc == LQ_OK) {
         cudaEventRecord(ev1, st);
         cudaStreamSynchronize(st);
@@ -475,7 +476,7 @@ int lq_descent_minimize(lq_ctx *c, int method, long max_steps, double force_tol,
     out->steps = (long)h.step; out->converged = h.converged;
     out->Fmax = h.Fmax; out->Frms = nsim > 0 ? sqrt(h.FF / nsim) : 0.0;
     out->P = 0.0; out->dt = dp->eta; out->alpha = dp->mu;
-    out->launches = launches; out->sweep_launches = launches; out->gpu_ms = ms;
+    out->launches = launches; out->sweep_launches = sweeps; out->gpu_ms = ms;
     if (dp->report_energy) {
         rc = lq_energy(c, &out->energy);
         if (rc != LQ_OK) return rc;

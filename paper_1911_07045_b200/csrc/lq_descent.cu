@@ -171,46 +171,254 @@ __global__ void __launch_bounds__(DB) k_descent(const DescArgs a) {
     finish_descent<DB>(a, r, red, &s_last);
 }
 
+
+// ---------------------------------------------------------------- one-constant fast path (plain sites)
+// 7-point Laplacian with a fixed association and F of a pure-bulk one-constant site from its tensor and
+// Laplacian (Eq. 5 + Eq. 11), explicit roundings.
+__device__ __forceinline__ double lap7(double xl, double xr, double yu, double yd, double zm, double zp, double c) {
+    return __fma_rn(-6.0, c, __dadd_rn(__dadd_rn(__dadd_rn(xl, xr), __dadd_rn(yu, yd)), __dadd_rn(zm, zp)));
+}
+__device__ __forceinline__ void force1(const LqPhys &ph, const double q[5], const double lap[5], double F[5]) {
+    const double a = q[0], b = q[1], c = q[2], d = q[3], e = q[4], f = -(a + d);
+    const double aa = a * a, bb = b * b, cc = c * c, dd = d * d, ee = e * e, ff = f * f;
+    const double tr = __dadd_rn(__dadd_rn(__dadd_rn(aa, dd), ff), 2.0 * __dadd_rn(__dadd_rn(bb, cc), ee));
+    const double k = __fma_rn(ph.C, tr, ph.A);
+    const double bf = __dadd_rn(bb, -ff);
+    const double dxx = __dadd_rn(__dadd_rn(aa, -ee), bf);          // (Q^2)xx - (Q^2)zz
+    const double dyy = __dadd_rn(__dadd_rn(dd, -cc), bf);          // (Q^2)yy - (Q^2)zz
+    const double qxy = __fma_rn(c, e, __fma_rn(b, d, a * b));
+    const double qxz = __fma_rn(c, f, __fma_rn(b, e, a * c));
+    const double qyz = __fma_rn(e, f, __fma_rn(d, e, b * c));
+    const double L1 = ph.L1, L2x = 2.0 * ph.L1, mB = -ph.B, m2B = -2.0 * ph.B, m2k = -2.0 * k;
+    // Gxx - Gzz = k (a - f) + B dxx with a - f = 2a + d
+    F[0] = __fma_rn(L1, __fma_rn(2.0, lap[0], lap[3]), __fma_rn(mB, dxx, -k * __fma_rn(2.0, a, d)));
+    F[3] = __fma_rn(L1, __fma_rn(2.0, lap[3], lap[0]), __fma_rn(mB, dyy, -k * __fma_rn(2.0, d, a)));
+    F[1] = __fma_rn(L2x, lap[1], __fma_rn(m2B, qxy, m2k * b));
+    F[2] = __fma_rn(L2x, lap[2], __fma_rn(m2B, qxz, m2k * c));
+    F[4] = __fma_rn(L2x, lap[4], __fma_rn(m2B, qyz, m2k * e));
+}
+
+// CTA = 32 x 16 columns marching a z-chunk.  Per plane one elected thread issues one (GD) or two (Nesterov)
+// 4-D TMA boxes (36 x 18 x 1 x 5: tile + 1 halo; the innermost start coordinate must be 16-byte aligned, hence
+// x0-2) into an NS-slot mbarrier ring.  A thread keeps the look-ahead column y(z-1), y(z), y(z+1) of its site in
+// registers and reads the four in-plane neighbours from the landed boxes; y is formed on the fly.
+template <bool NEST, int NS_>
+struct DS {
+    static constexpr int TX = 32, TY = 16, NT = TX * TY, NS = NS_;
+    static constexpr int SW = TX + 4, SH = TY + 2, SPLANE = SW * SH;
+    static constexpr int BOX_BYTES = 5 * SPLANE * 8, BOX_STRIDE = (BOX_BYTES + 127) / 128 * 128;
+    static constexpr int NF = NEST ? 2 : 1;
+    static constexpr int SLOT = NF * BOX_STRIDE;
+    static constexpr int OFF_BAR = NS * SLOT;
+    static constexpr int OFF_RED = OFF_BAR + 8 * NS_ + (8 * NS_ % 16);
+    static constexpr int SMEM_BYTES = OFF_RED + 2 * (NT / 32) * 8 + 16;
+};
+
+template <bool NEST, bool MASKED, int NS>
+__global__ void __launch_bounds__(512, 1)
+k_descent_sweep(const __grid_constant__ CUtensorMap tq, const __grid_constant__ CUtensorMap tp, const DescArgs a,
+                const uint8_t *__restrict__ plain, int zc) {
+    using C = DS<NEST, NS>;
+    extern __shared__ __align__(1024) unsigned char smem[];
+    __shared__ unsigned s_last;
+    if (a.sc->converged) return;
+    uint64_t *full = reinterpret_cast<uint64_t *>(smem + C::OFF_BAR);
+    double *red = reinterpret_cast<double *>(smem + C::OFF_RED);
+    const int tid = threadIdx.x, tx = tid & 31, ty = tid >> 5;
+    const int x0 = blockIdx.x * C::TX, y0 = blockIdx.y * C::TY;
+    const int zb = blockIdx.z * zc, ze = min(a.g.Lz, zb + zc);
+    const int x = x0 + tx, y = y0 + ty;
+    const bool active = x < a.g.Lx && y < a.g.Ly;
+    const int nplanes = ze - zb + 2;              // planes zb-1 .. ze
+    const double mu = a.mu, eta = a.eta;
+
+    if (tid == 0) {
+#pragma unroll
+        for (int i = 0; i < NS; ++i) mbar_init(&full[i], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+    auto issue = [&](int j, int s) {               // plane zb-1+j -> slot s
+        unsigned char *dst = smem + s * C::SLOT;
+        const int cx = x0 + LQ_XO - 2, cy = y0 + LQ_GH - 1, cz = zb - 1 + j + LQ_GH;
+        mbar_expect_tx(&full[s], (uint32_t)(C::NF * C::BOX_BYTES));
+        tma_load_4d(dst, &tq, &full[s], cx, cy, cz, 0);
+        if (NEST) tma_load_4d(dst + C::BOX_STRIDE, &tp, &full[s], cx, cy, cz, 0);
+    };
+    if (tid == 0)
+        for (int j = 0; j < NS && j < nplanes; ++j) issue(j, j);
+
+    const int sidx = (ty + 1) * C::SW + tx + 2;    // own site in a staged box
+    auto Y = [&](const double *sq, int c, int off) -> double {
+        const double v = sq[c * C::SPLANE + sidx + off];
+        return NEST ? lookahead(v, sq[C::BOX_STRIDE / 8 + c * C::SPLANE + sidx + off], mu) : v;
+    };
+    double ym[5], yc[5], r[2] = {0.0, 0.0};
+#pragma unroll
+    for (int c = 0; c < 5; ++c) ym[c] = yc[c] = 0.0;
+    long long p = a.g.pidx(x, y, zb - 1);          // padded index of the plane handled now (k = zb + j - 2)
+    unsigned pb_next = 1u;
+    int s0 = 0, s1 = NS - 1;
+    uint32_t par = 0;
+    for (int j = 0; j < nplanes; ++j) {
+        const unsigned pb = pb_next;
+        pb_next = 1u;
+        if (MASKED && active && j >= 1 && j + 1 < nplanes) pb_next = plain[p + a.g.sz];
+        mbar_wait(&full[s0], par);
+        const double *sj = reinterpret_cast<const double *>(smem + s0 * C::SLOT);
+        double yn[5];
+#pragma unroll
+        for (int c = 0; c < 5; ++c) yn[c] = Y(sj, c, 0);
+        if (j >= 2 && active) {
+            const int k = zb + j - 2;
+            const double *sb = reinterpret_cast<const double *>(smem + s1 * C::SLOT);
+            if (!MASKED || pb == 1u) {
+                double lap[5], F[5], o[5];
+#pragma unroll
+                for (int c = 0; c < 5; ++c)
+                    lap[c] = lap7(Y(sb, c, -1), Y(sb, c, 1), Y(sb, c, -C::SW), Y(sb, c, C::SW), ym[c], yn[c], yc[c]);
+                force1(a.ph, yc, lap, F);
+#pragma unroll
+                for (int c = 0; c < 5; ++c) {
+                    o[c] = __fma_rn(eta, F[c], yc[c]);
+                    r[0] = __fma_rn(F[c], F[c], r[0]);
+                    r[1] = fmax(r[1], fabs(F[c]));
+                }
+                store_site(a.g, a.qo, p, x, y, k, o);
+            } else if (pb == 2u) {
+                store_site(a.g, a.qo, p, x, y, k, yc);     // object site: y == q, never moves
+            }                                              // pb == 0: left to k_descent on the non-plain list
+        }
+        if (j >= 1) p += a.g.sz;
+#pragma unroll
+        for (int c = 0; c < 5; ++c) { ym[c] = yc[c]; yc[c] = yn[c]; }
+        // plane j-1 (slot s1) has been read by every thread: refill it with plane j-1+NS
+        __syncthreads();
+        if (tid == 0 && j >= 1 && j - 1 + NS < nplanes) issue(j - 1 + NS, s1);
+        s1 = s0;
+        if (++s0 == NS) { s0 = 0; par ^= 1u; }
+    }
+    finish_descent<C::NT>(a, r, red, &s_last);
+}
+
 }  // namespace
 
 struct LqDescentPlan {
-    double *partials = nullptr;
+    double *partials = nullptr;       // k_descent blocks
     size_t cap = 0;
+    double *sweep_partials = nullptr; // k_descent_sweep CTAs
+    size_t sweep_cap = 0;
     unsigned int *counter = nullptr;
+    // one-constant fast path
+    CUtensorMap map[3];
+    double *mapped[3] = {nullptr, nullptr, nullptr};
+    uint8_t *plain = nullptr;         // per-site plain byte (masked lattices)
+    int *list = nullptr;              // index-ordered non-plain simulated sites
+    int n_list = 0;
+    const uint8_t *flags_seen = nullptr;
+    bool sites_dirty = true;
+    bool attr_set[8] = {false, false, false, false, false, false, false, false};
 };
 
 void lq_descent_destroy(LqDescentPlan *p) {
     if (!p) return;
     cudaFree(p->partials);
+    cudaFree(p->sweep_partials);
     cudaFree(p->counter);
+    cudaFree(p->plain);
+    cudaFree(p->list);
     delete p;
 }
+void lq_descent_invalidate(LqDescentPlan *p) {
+    if (p) p->sites_dirty = true;
+}
 
-// Runs up to max_steps steps, one launch per step (two on masked one-constant lattices once the sweep exists).
-// buf[0] holds q_0 with a valid ghost shell; nbuf = 2 (GD) or 3 (Nesterov) rotating buffers.  On return *final
-// is the index of the buffer that holds the last iterate and *h the scalars.
-int lq_descent_run(LqDescentPlan **planp, int method, const LqGeom &g, const LqPhys &ph, const LqFields &f,
+namespace {
+constexpr int NS_GD = 6, NS_NEST = 4;   // ring depth: 6 x 25.4 KB (GD), 4 x 50.8 KB (Nesterov)
+
+template <bool NEST, bool MASKED>
+cudaError_t launch_sweep(LqDescentPlan *pl, dim3 grid, const CUtensorMap &mq, const CUtensorMap &mp, const DescArgs &a,
+                         int zc, cudaStream_t st) {
+    constexpr int NS = NEST ? NS_NEST : NS_GD;
+    using C = DS<NEST, NS>;
+    const int v = (NEST ? 2 : 0) + (MASKED ? 1 : 0);
+    if (!pl->attr_set[v]) {
+        cudaError_t e = cudaFuncSetAttribute(k_descent_sweep<NEST, MASKED, NS>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                             C::SMEM_BYTES);
+        if (e != cudaSuccess) return e;
+        pl->attr_set[v] = true;
+    }
+    k_descent_sweep<NEST, MASKED, NS><<<grid, C::NT, C::SMEM_BYTES, st>>>(mq, mp, a, pl->plain, zc);
+    return cudaGetLastError();
+}
+}  // namespace
+
+// Runs up to max_steps steps.  buf[0] holds q_0 with a valid ghost shell; nbuf = 2 (GD) or 3 (Nesterov) rotating
+// buffers.  On return *final is the index of the buffer that holds the last iterate and *h the scalars.
+// path: 0 = fast path where it applies (one-constant: TMA sweep over plain sites + k_descent on the non-plain
+// list), 1 = k_descent over every site.
+int lq_descent_run(LqDescentPlan **planp, int method, int path, const LqGeom &g, const LqPhys &ph, const LqFields &f,
                    double *const *buf, int nbuf, int *final, LqFireScalars *dsc, double eta, double mu,
-                   double force_tol, long max_steps, cudaStream_t st, long *launches, LqFireScalars *h,
-                   std::string &err) {
+                   double force_tol, long max_steps, cudaStream_t st, long *launches, long *sweeps,
+                   LqFireScalars *h, std::string &err) {
     LqDescentPlan *pl = *planp;
     if (!pl) { pl = new LqDescentPlan(); *planp = pl; }
     const bool three = ph.L2 != 0.0 || ph.L3 != 0.0;
     const bool nest = method == LQ_MIN_NESTEROV;
-    const unsigned nblk = (unsigned)((g.N + DB - 1) / DB);
+    const bool masked = f.flags != nullptr;
+    const bool fast = path == 0 && !three;
+    cudaError_t e;
+#define DESC_CUDA(call) do { e = (call); if (e != cudaSuccess) { err = std::string("lq_descent: ") + cudaGetErrorString(e); return LQ_ERR_CUDA; } } while (0)
+
+    // fast path set-up: tensor maps of the rotating buffers, z-chunking, plain map + non-plain list
+    dim3 grid(1, 1, 1);
+    int zc = g.Lz;
+    if (fast) {
+        for (int i = 0; i < nbuf; ++i)
+            if (pl->mapped[i] != buf[i]) {
+                if (!lq_make_box_map(&pl->map[i], g, buf[i], 36, 18)) { err = "lq_descent: cuTensorMapEncodeTiled failed"; return LQ_ERR_CUDA; }
+                pl->mapped[i] = buf[i];
+            }
+        const int ntx = (g.Lx + 31) / 32, nty = (g.Ly + 15) / 16;
+        long long best = -1;
+        for (int nzc = 1; nzc <= (g.Lz + 7) / 8; ++nzc) {          // equal chunks, modelled makespan on 148 SMs
+            const int c = (g.Lz + nzc - 1) / nzc;
+            const long long ncta = (long long)ntx * nty * ((g.Lz + c - 1) / c);
+            const long long cost = ((ncta + 147) / 148) * (c + 4);
+            if (best < 0 || cost < best) { best = cost; zc = c; }
+        }
+        grid = dim3(ntx, nty, (g.Lz + zc - 1) / zc);
+        const size_t ncta = (size_t)grid.x * grid.y * grid.z;
+        if (pl->sweep_cap < 2 * ncta) {
+            cudaFree(pl->sweep_partials); pl->sweep_partials = nullptr; pl->sweep_cap = 0;
+            if (cudaMalloc(&pl->sweep_partials, 2 * ncta * sizeof(double)) != cudaSuccess) { err = "lq_descent: cudaMalloc failed"; return LQ_ERR_NOMEM; }
+            pl->sweep_cap = 2 * ncta;
+        }
+        if (masked && (pl->sites_dirty || pl->flags_seen != f.flags || !pl->plain)) {
+            if (!pl->plain && cudaMalloc(&pl->plain, (size_t)g.NP) != cudaSuccess) { err = "lq_descent: cudaMalloc failed"; return LQ_ERR_NOMEM; }
+            DESC_CUDA(cudaMemsetAsync(pl->plain, 0, (size_t)g.NP, st));
+            lq_launch_plain_map(g, f.flags, pl->plain, st);
+            *launches += 1;
+            if (lq_fixup_build_list(g, f.flags, pl->plain, &pl->list, &pl->n_list, st) != 0) { err = "lq_descent: building the non-plain site list failed"; return LQ_ERR_NOMEM; }
+            pl->sites_dirty = false;
+            pl->flags_seen = f.flags;
+        }
+    }
+    const long long nsites = fast ? (masked ? pl->n_list : 0) : g.N;
+    const unsigned nblk = (unsigned)((nsites + DB - 1) / DB);
     if (pl->cap < (size_t)2 * nblk) {
         cudaFree(pl->partials); pl->partials = nullptr; pl->cap = 0;
         if (cudaMalloc(&pl->partials, (size_t)2 * nblk * sizeof(double)) != cudaSuccess) { err = "lq_descent: cudaMalloc failed"; return LQ_ERR_NOMEM; }
         pl->cap = (size_t)2 * nblk;
     }
     if (!pl->counter && cudaMalloc(&pl->counter, sizeof(unsigned int)) != cudaSuccess) { err = "lq_descent: cudaMalloc failed"; return LQ_ERR_NOMEM; }
-    cudaError_t e = cudaMemsetAsync(pl->counter, 0, sizeof(unsigned int), st);
-    if (e != cudaSuccess) { err = cudaGetErrorString(e); return LQ_ERR_CUDA; }
+    DESC_CUDA(cudaMemsetAsync(pl->counter, 0, sizeof(unsigned int), st));
 
     DescArgs a;
     a.g = g; a.ph = ph; a.f = f; a.eta = eta; a.mu = nest ? mu : 0.0; a.force_tol = force_tol;
-    a.list = nullptr; a.n = 0; a.sc = dsc; a.partials = pl->partials; a.extra = nullptr; a.n_extra = 0;
-    a.counter = pl->counter; a.finish = 1;
+    a.sc = dsc; a.counter = pl->counter;
+    const bool second = nblk > 0;                  // a k_descent launch closes the step
+    const int per_step = (fast ? 1 : 0) + (second ? 1 : 0);
     const long chunk = force_tol > 0.0 ? 100 : (1L << 30);
     long done = 0;
     while (done < max_steps) {
@@ -219,28 +427,41 @@ int lq_descent_run(LqDescentPlan **planp, int method, const LqGeom &g, const LqP
             const long k = done + i;
             const int in = (int)(k % nbuf), out = (int)((k + 1) % nbuf), prev = k == 0 ? in : (int)((k - 1) % nbuf);
             a.q = buf[in]; a.qp = buf[prev]; a.qo = buf[out];
-            if (three) {
-                if (nest) k_descent<true, true><<<nblk, DB, 0, st>>>(a);
-                else k_descent<true, false><<<nblk, DB, 0, st>>>(a);
-            } else {
-                if (nest) k_descent<false, true><<<nblk, DB, 0, st>>>(a);
-                else k_descent<false, false><<<nblk, DB, 0, st>>>(a);
+            if (fast) {
+                a.list = nullptr; a.n = 0; a.partials = pl->sweep_partials; a.extra = nullptr; a.n_extra = 0;
+                a.finish = second ? 0 : 1;
+                if (nest) e = masked ? launch_sweep<true, true>(pl, grid, pl->map[in], pl->map[prev], a, zc, st)
+                                     : launch_sweep<true, false>(pl, grid, pl->map[in], pl->map[prev], a, zc, st);
+                else e = masked ? launch_sweep<false, true>(pl, grid, pl->map[in], pl->map[in], a, zc, st)
+                                : launch_sweep<false, false>(pl, grid, pl->map[in], pl->map[in], a, zc, st);
+                DESC_CUDA(e);
             }
-            e = cudaGetLastError();
-            if (e != cudaSuccess) { err = std::string("lq_descent launch: ") + cudaGetErrorString(e); return LQ_ERR_CUDA; }
+            if (second) {
+                a.list = fast ? pl->list : nullptr; a.n = fast ? pl->n_list : 0; a.partials = pl->partials;
+                a.extra = fast ? pl->sweep_partials : nullptr; a.n_extra = fast ? (int)(grid.x * grid.y * grid.z) : 0;
+                a.finish = 1;
+                if (three) {
+                    if (nest) k_descent<true, true><<<nblk, DB, 0, st>>>(a);
+                    else k_descent<true, false><<<nblk, DB, 0, st>>>(a);
+                } else {
+                    if (nest) k_descent<false, true><<<nblk, DB, 0, st>>>(a);
+                    else k_descent<false, false><<<nblk, DB, 0, st>>>(a);
+                }
+                DESC_CUDA(cudaGetLastError());
+            }
         }
         done += n;
-        *launches += n;
+        *launches += per_step * n;
+        *sweeps += n;
         if (force_tol > 0.0) {
-            e = cudaMemcpyAsync(h, dsc, sizeof(*h), cudaMemcpyDeviceToHost, st);
-            if (e == cudaSuccess) e = cudaStreamSynchronize(st);
-            if (e != cudaSuccess) { err = std::string("lq_descent: ") + cudaGetErrorString(e); return LQ_ERR_CUDA; }
+            DESC_CUDA(cudaMemcpyAsync(h, dsc, sizeof(*h), cudaMemcpyDeviceToHost, st));
+            DESC_CUDA(cudaStreamSynchronize(st));
             if (h->converged) break;
         }
     }
-    e = cudaMemcpyAsync(h, dsc, sizeof(*h), cudaMemcpyDeviceToHost, st);
-    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
-    if (e != cudaSuccess) { err = std::string("lq_descent: ") + cudaGetErrorString(e); return LQ_ERR_CUDA; }
+    DESC_CUDA(cudaMemcpyAsync(h, dsc, sizeof(*h), cudaMemcpyDeviceToHost, st));
+    DESC_CUDA(cudaStreamSynchronize(st));
+#undef DESC_CUDA
     *final = (int)(h->step % nbuf);
     return LQ_OK;
 }

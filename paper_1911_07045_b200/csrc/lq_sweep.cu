@@ -266,6 +266,8 @@ bool make_map(CUtensorMap *m, const LqGeom &g, double *base, int bxw, int byh) {
 
 }  // namespace
 
+bool lq_make_box_map(CUtensorMap *m, const LqGeom &g, double *base, int bxw, int byh) { return make_map(m, g, base, bxw, byh); }
+
 struct LqSweepPlan {
     CUtensorMap mq[2], mv[2], mF[2];
     double *bq[2] = {nullptr, nullptr}, *bv[2] = {nullptr, nullptr}, *bF[2] = {nullptr, nullptr};

@@ -20,13 +20,17 @@ int lq_sweep_run(LqSweepPlan **plan, bool stored_F, const LqGeom &g, const LqPhy
 // gradient descent / Nesterov (lq_descent.cu): one launch per step; buf[0] holds q_0, nbuf rotating buffers
 struct LqDescentPlan;
 void lq_descent_destroy(LqDescentPlan *plan);
-int lq_descent_run(LqDescentPlan **plan, int method, const LqGeom &g, const LqPhys &ph, const LqFields &f,
+int lq_descent_run(LqDescentPlan **plan, int method, int path, const LqGeom &g, const LqPhys &ph, const LqFields &f,
                    double *const *buf, int nbuf, int *final, LqFireScalars *dsc, double eta, double mu,
-                   double force_tol, long max_steps, cudaStream_t st, long *launches, LqFireScalars *h,
-                   std::string &err);
+                   double force_tol, long max_steps, cudaStream_t st, long *launches, long *sweeps,
+                   LqFireScalars *h, std::string &err);
+
+#include <cuda.h>
+// 4-D tensor map (x, y, z, component) over a padded field with a bxw x byh x 1 x 5 box (lq_sweep.cu)
+bool lq_make_box_map(CUtensorMap *m, const LqGeom &g, double *base, int bxw, int byh);
+void lq_descent_invalidate(LqDescentPlan *plan);   // geometry / anchoring arrays changed
 
 // recompute-F kernel (lq_sweep_rc.cu)
-#include <cuda.h>
 namespace lqsw { struct SweepArgs; }
 int lq_sweep_rc_box(int which, int dim);
 int lq_sweep_rc_tile(int dim);

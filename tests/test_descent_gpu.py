@@ -64,6 +64,27 @@ def test_q_after_K_steps(case, lq, method):
         assert np.array_equal(q.reshape(5, -1)[:, obj], np.asarray(c["q"]).reshape(5, -1)[:, obj])
 
 
+@pytest.mark.parametrize("method", [0, 1])
+def test_general_kernel_path_matches_too(lq, oracle_mod, method):
+    """fire_path = 1 runs k_descent over every site (no TMA sweep): same oracle, same tolerance; and the two GPU
+    paths agree with each other far below it"""
+    for name in ("masked_70x35x9_L1only", "replica5p"):
+        build, K = CASES[name]
+        c = build()
+        o = make_oracle(oracle_mod, c)
+        qref, _ = o.descent(c["q"], method, K, 0.0, ETA, MU)
+        got = []
+        for path in (1, 0):
+            ctx = lq.create_from_config(c)
+            lq.lq_set_option(ctx, "fire_path", path)
+            rep = lq.lq_descent_minimize(ctx, method, K, 0.0, ETA, MU)
+            assert rep["steps"] == K
+            got.append(lq.lq_get_Q(ctx))
+            lq.lq_destroy(ctx)
+            assert np.abs(got[-1] - qref).max() <= 1e-8
+        assert np.abs(got[0] - got[1]).max() <= 1e-12
+
+
 def test_first_step_is_q_plus_eta_F(case, lq):
     """one GD step against the force entry point of the same library and the oracle's force"""
     name, c, ctx, o, K = case

@@ -129,23 +129,30 @@ def crop_config(c, L):
     return d
 
 
-def time_oracle(c, target_s=15.0, crop=128):
-    """oracle FIRE steps on a crop; returns (site-updates/s, cores, sample description)"""
+def oracle_steps(o, s, q, steps, method="fire", eta=0.004, mu=0.8):
+    """the oracle's minimiser for `method`, as it stands; returns the final q"""
+    if method == "fire":
+        return o.fire(q, steps, 0.0, s["fire"], variant=1)[0]
+    return o.descent(q, 0 if method == "gd" else 1, steps, 0.0, eta, mu, variant=1)[0]
+
+
+def time_oracle(c, target_s=15.0, crop=128, method="fire", eta=0.004, mu=0.8):
+    """oracle minimiser steps on a crop; returns (site-updates/s, cores, sample description)"""
     import oracle
     oracle.build_oracle()
     s = crop_config(c, crop)
     o = oracle_problem(s)
     nsim = s["N"] if s["mask"] is None else int(np.sum(s["mask"] == 0))
     t0 = time.perf_counter()
-    o.fire(s["q"], 1, 0.0, s["fire"], variant=1)
+    oracle_steps(o, s, s["q"], 1, method, eta, mu)
     t1 = time.perf_counter() - t0                      # 1 step (+ the initial force evaluation)
     steps = int(max(2, min(200, target_s / max(t1 / 2.0, 1e-4))))
     t0 = time.perf_counter()
-    o.fire(s["q"], steps, 0.0, s["fire"], variant=1)
+    oracle_steps(o, s, s["q"], steps, method, eta, mu)
     dt = time.perf_counter() - t0
     val = nsim * steps / dt
-    desc = "%dx%dx%d corner crop of %s, %d FIRE steps, oracle variant=factorised+OpenMP, %.1f s" % (
-        s["Lx"], s["Ly"], s["Lz"], c["name"], steps, dt)
+    desc = "%dx%dx%d corner crop of %s, %d %s steps, oracle variant=factorised+OpenMP, %.1f s" % (
+        s["Lx"], s["Ly"], s["Lz"], c["name"], steps, method, dt)
     return val, oracle.num_threads(), desc, dt, steps
 
 
@@ -163,14 +170,15 @@ def run_reference(args):
     nsim = s["N"] if s["mask"] is None else int(np.sum(s["mask"] == 0))
     q = s["q"]
     for _ in range(args.warmup if args.warmup is not None else 1):
-        q, _ = o.fire(q, 1, 0.0, s["fire"], variant=1)
+        q = oracle_steps(o, s, q, 1, args.method, args.eta, args.mu)
     K = args.steps if args.steps is not None else 5
     t0 = time.perf_counter()
-    q, _ = o.fire(q, K, 0.0, s["fire"], variant=1)
+    q = oracle_steps(o, s, q, K, args.method, args.eta, args.mu)
     dt = time.perf_counter() - t0
     val = nsim * K / dt
-    sample = "%dx%dx%d corner crop of %s, %d FIRE steps per timed call" % (s["Lx"], s["Ly"], s["Lz"], c["name"], K)
-    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": K,
+    sample = "%dx%dx%d corner crop of %s, %d %s steps per timed call" % (s["Lx"], s["Ly"], s["Lz"], c["name"], K, args.method)
+    metric = METRIC if args.method == "fire" else METRIC.replace("FIRE", {"gd": "gradient-descent", "nesterov": "Nesterov"}[args.method])
+    line = {"impl": "reference", "metric": metric, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": K,
             "warmup": args.warmup if args.warmup is not None else 1, "ms_per_step": 1e3 * dt / K,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": c["name"], "sample": sample},
@@ -325,7 +333,7 @@ def main():
 
     cpu = None
     if not args.no_cpu_baseline:
-        v, cores, desc, _, _ = time_oracle(c, target_s=15.0, crop=args.ref_crop)
+        v, cores, desc, _, _ = time_oracle(c, target_s=15.0, crop=args.ref_crop, method=args.method, eta=args.eta, mu=args.mu)
         cpu = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc}
 
     metric = METRIC if args.method == "fire" else METRIC.replace("FIRE", {"gd": "gradient-descent", "nesterov": "Nesterov"}[args.method])

@@ -136,6 +136,15 @@ typedef struct {
 int lq_fire_minimize(lq_ctx *ctx, long max_steps, double force_tol,
                      const lq_fire_params *params, lq_fire_report *out);
 
+/* Uniform external magnetic / electric fields, Eq. 13:
+ *     f_external = -(1/3) chi H_i Q_ij H_j - (1/3) eps E_i Q_ij E_j        at every simulated site,
+ * chi = mu0 Delta-chi and eps = eps0 Delta-eps in the context's nondimensional units (positive values favour
+ * alignment of the director with the field).  H, E: host double[3] (NULL = zero vector).  The term enters
+ * lq_energy (reported inside the bulk term of lq_energy_terms), lq_forces and every minimiser; it costs no extra
+ * instruction in the kernels (a constant folded into existing FMAs).  Calling it again replaces the fields;
+ * all-zero arguments switch the term off.  Errors: LQ_ERR_ARG on non-finite values. */
+int lq_set_field(lq_ctx *ctx, const double *H, double chi, const double *E, double eps);
+
 /* Other first-order minimisers on the same force.  The paper compares FIRE with gradient
  * descent and offers Nesterov's accelerated gradient as its second minimiser
  * without printing either update; the fixed-step textbook forms are used

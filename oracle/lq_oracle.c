@@ -56,6 +56,8 @@ typedef struct {
     const uint8_t *kind;     /* [N] 0 none, 1 oriented (Eq.14), 2 degenerate planar (Eq.15); NULL = none */
     const double *W;         /* [N] anchoring strength of Eq. 14/15; NULL if kind NULL */
     const double *axis;      /* [3][N] unit vector n0 (kind 1) or nu (kind 2)  */
+    /* external fields, Eq. 13: uniform H and E; chi = mu0 Delta-chi, eps = eps0 Delta-eps */
+    double H[3], chi, E[3], eps;
 } lqo_problem;
 
 typedef struct { double dt0, dtmax, alpha0, finc, fdec, falpha; int Nmin; int integrator; } lqo_fire_params;
@@ -160,6 +162,23 @@ static double bulk_energy(const lqo_problem *p, const double Q[3][3])
             for (int k = 0; k < 3; ++k) tr3 += Q[i][j] * Q[j][k] * Q[k][i];
         }
     return 0.5 * p->A * tr2 + p->B / 3.0 * tr3 + 0.25 * p->C * tr2 * tr2;
+}
+
+/* Eq. 13: f_external = -(1/3) chi H_i Q_ij H_j - (1/3) eps E_i Q_ij E_j */
+static double field_energy(const lqo_problem *p, const double Q[3][3])
+{
+    double e = 0.0;
+    for (int i = 0; i < 3; ++i)
+        for (int j = 0; j < 3; ++j)
+            e -= (p->chi * p->H[i] * Q[i][j] * p->H[j] + p->eps * p->E[i] * Q[i][j] * p->E[j]) / 3.0;
+    return e;
+}
+/* d(f_external)/dQ_ab, entries independent: linear in Q, so a constant tensor */
+static void field_grad_add(const lqo_problem *p, double G[3][3])
+{
+    for (int a = 0; a < 3; ++a)
+        for (int b = 0; b < 3; ++b)
+            G[a][b] -= (p->chi * p->H[a] * p->H[b] + p->eps * p->E[a] * p->E[b]) / 3.0;
 }
 
 /* d(bulk)/dQ_ab with entries independent:
@@ -304,8 +323,8 @@ static double site_literal(const lqo_problem *p, const double *q, int x, int y, 
     double G9[7][3][3];
     memset(G9, 0, sizeof(G9));
 
-    double eb = bulk_energy(p, Q);
-    if (g) bulk_grad(p, Q, G9[0]);
+    double eb = bulk_energy(p, Q) + field_energy(p, Q);      /* the "bulk" slot carries Eq. 13 too */
+    if (g) { bulk_grad(p, Q, G9[0]); field_grad_add(p, G9[0]); }
 
     int nopt[3], opt[3][2];
     allowed_signs(p, x, y, z, nopt, opt);
@@ -420,7 +439,7 @@ static double site_factorised(const lqo_problem *p, const double *q, int x, int 
                 }
             }
 
-    double eb = bulk_energy(p, Q);
+    double eb = bulk_energy(p, Q) + field_energy(p, Q);      /* the "bulk" slot carries Eq. 13 too */
     double Ga[3][3];
     double ea = anchoring(p, N, s, Q, g ? Ga : NULL);
 
@@ -428,6 +447,7 @@ static double site_factorised(const lqo_problem *p, const double *q, int x, int 
         double G9[7][3][3];
         memset(G9, 0, sizeof(G9));
         bulk_grad(p, Q, G9[0]);
+        field_grad_add(p, G9[0]);
         for (int i = 0; i < 3; ++i)
             for (int j = 0; j < 3; ++j) G9[0][i][j] += Ga[i][j];
         for (int k = 0; k < 3; ++k)

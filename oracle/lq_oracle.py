@@ -38,7 +38,8 @@ class _Problem(C.Structure):
     _fields_ = [("Lx", C.c_int), ("Ly", C.c_int), ("Lz", C.c_int),
                 ("A", C.c_double), ("B", C.c_double), ("C", C.c_double),
                 ("L1", C.c_double), ("L2", C.c_double), ("L3", C.c_double),
-                ("mask", C.c_void_p), ("kind", C.c_void_p), ("W", C.c_void_p), ("axis", C.c_void_p)]
+                ("mask", C.c_void_p), ("kind", C.c_void_p), ("W", C.c_void_p), ("axis", C.c_void_p),
+                ("H", C.c_double * 3), ("chi", C.c_double), ("E", C.c_double * 3), ("eps", C.c_double)]
 
 
 class _FireParams(C.Structure):
@@ -108,7 +109,7 @@ class Oracle:
     """One lattice problem held as host numpy arrays; every method calls C."""
 
     def __init__(self, Lx, Ly, Lz, A, B, Cc, L1, L2=0.0, L3=0.0,
-                 mask=None, kind=None, W=None, axis=None):
+                 mask=None, kind=None, W=None, axis=None, H=(0.0, 0.0, 0.0), chi=0.0, E=(0.0, 0.0, 0.0), eps=0.0):
         self.lib = _load()
         self.shape = (int(Lx), int(Ly), int(Lz))
         self.N = int(Lx) * int(Ly) * int(Lz)
@@ -120,7 +121,9 @@ class Oracle:
         if self.kind is not None and (self.W is None or self.axis is None):
             raise ValueError("kind given without W/axis")
         self.p = _Problem(int(Lx), int(Ly), int(Lz), A, B, Cc, L1, L2, L3,
-                          _ptr(self.mask), _ptr(self.kind), _ptr(self.W), _ptr(self.axis))
+                          _ptr(self.mask), _ptr(self.kind), _ptr(self.W), _ptr(self.axis),
+                          (C.c_double * 3)(*[float(h) for h in H]), float(chi),
+                          (C.c_double * 3)(*[float(e) for e in E]), float(eps))
 
     def _q(self, q):
         q = np.ascontiguousarray(q, dtype=np.float64)

@@ -23,7 +23,7 @@ _lib = None
 
 # every symbol include/lq.h declares (checked by tests/test_abi.py against the header)
 SYMBOLS = ["lq_create", "lq_destroy", "lq_set_stream", "lq_set_sites", "lq_get_flags", "lq_set_Q", "lq_get_Q",
-           "lq_get_velocity", "lq_energy", "lq_energy_terms", "lq_forces", "lq_fire_minimize", "lq_descent_minimize", "lq_get_S0",
+           "lq_get_velocity", "lq_set_field", "lq_energy", "lq_energy_terms", "lq_forces", "lq_fire_minimize", "lq_descent_minimize", "lq_get_S0",
            "lq_set_option", "lq_get_info", "lq_last_error", "lq_version"]
 
 
@@ -79,6 +79,7 @@ def load():
     L.lq_energy_terms.argtypes = [vp, dp]
     L.lq_forces.argtypes = [vp, vp, ip]
     L.lq_fire_minimize.argtypes = [vp, C.c_long, C.c_double, C.POINTER(lq_fire_params), C.POINTER(lq_fire_report)]
+    L.lq_set_field.argtypes = [vp, dp, C.c_double, dp, C.c_double]
     L.lq_descent_minimize.argtypes = [vp, ip, C.c_long, C.c_double, C.POINTER(lq_descent_params), C.POINTER(lq_fire_report)]
     L.lq_get_S0.argtypes = [vp, dp]
     L.lq_set_option.argtypes = [vp, C.c_char_p, C.c_double]
@@ -236,6 +237,13 @@ def lq_fire_minimize(ctx, max_steps, force_tol, params: dict, report_energy=Fals
     rep = lq_fire_report()
     _check(ctx.handle, load().lq_fire_minimize(ctx.handle, int(max_steps), float(force_tol), C.byref(fp), C.byref(rep)))
     return {k: getattr(rep, k) for k, _ in lq_fire_report._fields_}
+
+
+def lq_set_field(ctx, H=None, chi=0.0, E=None, eps=0.0) -> None:
+    """uniform external fields of Eq. 13: H, E sequences of 3 floats (None = zero)"""
+    def vec(v):
+        return None if v is None else (C.c_double * 3)(*[float(t) for t in v])
+    _check(ctx.handle, load().lq_set_field(ctx.handle, vec(H), float(chi), vec(E), float(eps)))
 
 
 def lq_descent_minimize(ctx, method, max_steps, force_tol, eta, mu=0.0, report_energy=False) -> dict:

@@ -433,6 +433,24 @@ int lq_fire_minimize(lq_ctx *c, long max_steps, double force_tol, const lq_fire_
 }
 
 
+int lq_set_field(lq_ctx *c, const double *H, double chi, const double *E, double eps) {
+    if (!c) return LQ_ERR_ARG;
+    double h[3] = {0.0, 0.0, 0.0}, e[3] = {0.0, 0.0, 0.0};
+    for (int i = 0; i < 3; ++i) {
+        if (H) h[i] = H[i];
+        if (E) e[i] = E[i];
+        if (!std::isfinite(h[i]) || !std::isfinite(e[i])) return fail(c, LQ_ERR_ARG, "lq_set_field: non-finite field");
+    }
+    if (!std::isfinite(chi) || !std::isfinite(eps)) return fail(c, LQ_ERR_ARG, "lq_set_field: non-finite coefficient");
+    const int ia[6] = {0, 0, 0, 1, 1, 2}, ib[6] = {0, 1, 2, 1, 2, 2};      // (xx, xy, xz, yy, yz, zz)
+    double *T = c->ph.T;
+    for (int k = 0; k < 6; ++k) T[k] = (chi * h[ia[k]] * h[ib[k]] + eps * e[ia[k]] * e[ib[k]]) / 3.0;
+    // F = -(Gxx - Gzz, 2 Gxy, 2 Gxz, Gyy - Gzz, 2 Gyz) with G_ab = -T_ab
+    c->ph.Fx[0] = T[0] - T[5]; c->ph.Fx[1] = 2.0 * T[1]; c->ph.Fx[2] = 2.0 * T[2];
+    c->ph.Fx[3] = T[3] - T[5]; c->ph.Fx[4] = 2.0 * T[4];
+    return LQ_OK;
+}
+
 int lq_descent_minimize(lq_ctx *c, int method, long max_steps, double force_tol, const lq_descent_params *dp,
                         lq_fire_report *out) {
     if (!c) return LQ_ERR_ARG;

@@ -191,11 +191,12 @@ __device__ __forceinline__ void force1(const LqPhys &ph, const double q[5], cons
     const double qyz = __fma_rn(e, f, __fma_rn(d, e, b * c));
     const double L1 = ph.L1, L2x = 2.0 * ph.L1, mB = -ph.B, m2B = -2.0 * ph.B, m2k = -2.0 * k;
     // Gxx - Gzz = k (a - f) + B dxx with a - f = 2a + d
-    F[0] = __fma_rn(L1, __fma_rn(2.0, lap[0], lap[3]), __fma_rn(mB, dxx, -k * __fma_rn(2.0, a, d)));
-    F[3] = __fma_rn(L1, __fma_rn(2.0, lap[3], lap[0]), __fma_rn(mB, dyy, -k * __fma_rn(2.0, d, a)));
-    F[1] = __fma_rn(L2x, lap[1], __fma_rn(m2B, qxy, m2k * b));
-    F[2] = __fma_rn(L2x, lap[2], __fma_rn(m2B, qxz, m2k * c));
-    F[4] = __fma_rn(L2x, lap[4], __fma_rn(m2B, qyz, m2k * e));
+    // + Fx: constant external-field force (Eq. 13), folded into the FMAs
+    F[0] = __fma_rn(L1, __fma_rn(2.0, lap[0], lap[3]), __fma_rn(mB, dxx, __fma_rn(-k, __fma_rn(2.0, a, d), ph.Fx[0])));
+    F[3] = __fma_rn(L1, __fma_rn(2.0, lap[3], lap[0]), __fma_rn(mB, dyy, __fma_rn(-k, __fma_rn(2.0, d, a), ph.Fx[3])));
+    F[1] = __fma_rn(L2x, lap[1], __fma_rn(m2B, qxy, __fma_rn(m2k, b, ph.Fx[1])));
+    F[2] = __fma_rn(L2x, lap[2], __fma_rn(m2B, qxz, __fma_rn(m2k, c, ph.Fx[2])));
+    F[4] = __fma_rn(L2x, lap[4], __fma_rn(m2B, qyz, __fma_rn(m2k, e, ph.Fx[4])));
 }
 
 // CTA = 32 x 16 columns marching a z-chunk.  Per plane one elected thread issues one (GD) or two (Nesterov)

@@ -28,6 +28,9 @@ struct LqGeom {
 
 struct LqPhys {
     double A, B, C, L1, L2, L3, S0;
+    // external fields, Eq. 13: T_ab = (chi H_a H_b + eps E_a E_b) / 3 in (xx,xy,xz,yy,yz,zz) order,
+    // f_external = -T_ab Q_ab; Fx = the constant force it adds in the five stored variables (all 0 without a field)
+    double T[6], Fx[5];
 };
 
 // FIRE state that lives on the device (Algorithm 1).

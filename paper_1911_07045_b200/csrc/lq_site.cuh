@@ -81,8 +81,10 @@ __device__ __forceinline__ void bulk_G(const LqPhys &ph, const double Q[6], doub
     const double q2xx = a * a + b * b + c * c, q2xy = a * b + b * d + c * e, q2xz = a * c + b * e + c * f;
     const double q2yy = b * b + d * d + e * e, q2yz = b * c + d * e + e * f, q2zz = c * c + e * e + f * f;
     const double k = ph.A + ph.C * (q2xx + q2yy + q2zz);
-    G[0][0] = k * a + ph.B * q2xx; G[0][1] = G[1][0] = k * b + ph.B * q2xy; G[0][2] = G[2][0] = k * c + ph.B * q2xz;
-    G[1][1] = k * d + ph.B * q2yy; G[1][2] = G[2][1] = k * e + ph.B * q2yz; G[2][2] = k * f + ph.B * q2zz;
+    // - T_ab: the external-field term of Eq. 13 (constant; folds into the FMAs, exact no-op when T = 0)
+    G[0][0] = k * a + (ph.B * q2xx - ph.T[0]); G[0][1] = G[1][0] = k * b + (ph.B * q2xy - ph.T[1]);
+    G[0][2] = G[2][0] = k * c + (ph.B * q2xz - ph.T[2]); G[1][1] = k * d + (ph.B * q2yy - ph.T[3]);
+    G[1][2] = G[2][1] = k * e + (ph.B * q2yz - ph.T[4]); G[2][2] = k * f + (ph.B * q2zz - ph.T[5]);
 }
 
 __device__ __forceinline__ double bulk_E(const LqPhys &ph, const double Q[6]) {
@@ -91,7 +93,8 @@ __device__ __forceinline__ double bulk_E(const LqPhys &ph, const double Q[6]) {
     const double q2yy = b * b + d * d + e * e, q2yz = b * c + d * e + e * f, q2zz = c * c + e * e + f * f;
     const double tr2 = q2xx + q2yy + q2zz;
     const double tr3 = q2xx * a + q2yy * d + q2zz * f + 2.0 * (q2xy * b + q2xz * c + q2yz * e);
-    return 0.5 * ph.A * tr2 + ph.B * (1.0 / 3.0) * tr3 + 0.25 * ph.C * tr2 * tr2;
+    const double fext = -(ph.T[0] * a + ph.T[3] * d + ph.T[5] * f + 2.0 * (ph.T[1] * b + ph.T[2] * c + ph.T[4] * e));   // Eq. 13
+    return 0.5 * ph.A * tr2 + ph.B * (1.0 / 3.0) * tr3 + 0.25 * ph.C * tr2 * tr2 + fext;
 }
 
 // anchoring: adds to G (if G != nullptr) and returns the energy

@@ -131,6 +131,11 @@ def crop_config(c, L):
 
 def oracle_steps(o, s, q, steps, method="fire", eta=0.004, mu=0.8):
     """the oracle's minimiser for `method`, as it stands; returns the final q"""
+    if method == "analyze":
+        import oracle
+        for _ in range(steps):
+            oracle.analyze(q, s["mask"], 0.4)
+        return q
     if method == "fire":
         return o.fire(q, steps, 0.0, s["fire"], variant=1)[0]
     return o.descent(q, 0 if method == "gd" else 1, steps, 0.0, eta, mu, variant=1)[0]
@@ -151,8 +156,9 @@ def time_oracle(c, target_s=15.0, crop=128, method="fire", eta=0.004, mu=0.8):
     oracle_steps(o, s, s["q"], steps, method, eta, mu)
     dt = time.perf_counter() - t0
     val = nsim * steps / dt
-    desc = "%dx%dx%d corner crop of %s, %d %s steps, oracle variant=factorised+OpenMP, %.1f s" % (
-        s["Lx"], s["Ly"], s["Lz"], c["name"], steps, method, dt)
+    how = "numpy.linalg.eigh per site" if method == "analyze" else "oracle variant=factorised+OpenMP"
+    desc = "%dx%dx%d corner crop of %s, %d %s steps, %s, %.1f s" % (
+        s["Lx"], s["Ly"], s["Lz"], c["name"], steps, method, how, dt)
     return val, oracle.num_threads(), desc, dt, steps
 
 
@@ -177,7 +183,7 @@ def run_reference(args):
     dt = time.perf_counter() - t0
     val = nsim * K / dt
     sample = "%dx%dx%d corner crop of %s, %d %s steps per timed call" % (s["Lx"], s["Ly"], s["Lz"], c["name"], K, args.method)
-    metric = METRIC if args.method == "fire" else METRIC.replace("FIRE", {"gd": "gradient-descent", "nesterov": "Nesterov"}[args.method])
+    metric = METRIC if args.method == "fire" else METRIC.replace("FIRE", {"gd": "gradient-descent", "nesterov": "Nesterov", "analyze": "director/S/defect analysis"}[args.method])
     line = {"impl": "reference", "metric": metric, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": K,
             "warmup": args.warmup if args.warmup is not None else 1, "ms_per_step": 1e3 * dt / K,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
@@ -212,7 +218,7 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--fire-path", type=int, default=0)
-    ap.add_argument("--method", default="fire", choices=["fire", "gd", "nesterov"],
+    ap.add_argument("--method", default="fire", choices=["fire", "gd", "nesterov", "analyze"],
                     help="minimiser whose step is timed (default: FIRE, the headline metric; gd / nesterov: SURVEY 8(f1))")
     ap.add_argument("--eta", type=float, default=0.004)
     ap.add_argument("--mu", type=float, default=0.8)
@@ -256,6 +262,17 @@ def main():
     if args.method == "fire":
         def minimize(steps):
             return lq.lq_fire_minimize(ctx, steps, 0.0, c["fire"])
+    elif args.method == "analyze":
+        # a "step" = one pass of the director / S / defect-mask kernel over the lattice
+        aS = torch.empty(N, dtype=torch.float64, device="cuda")
+        aD = torch.empty((3, N), dtype=torch.float64, device="cuda")
+        aM = torch.empty(N, dtype=torch.uint8, device="cuda")
+        thr = 0.8 * lq.lq_get_S0(ctx)
+
+        def minimize(steps):
+            for _ in range(steps):
+                lq.lq_analyze_device(ctx, thr, aS, aD, aM)
+            return {"steps": steps, "sweep_launches": steps, "launches": steps}
     else:
         meth = lq.LQ_MIN_GD if args.method == "gd" else lq.LQ_MIN_NESTEROV
 
@@ -309,12 +326,14 @@ def main():
     peak, peak_kind = measured_hbm_peak()
     flag_byte = 1.0 if lq.lq_get_info(ctx, "n_object") > 0 else 0.0
     # FIRE reads + writes q and v (+ flag byte).  GD: read q, write q; Nesterov: read q_k, q_{k-1}, write q_{k+1}
-    alg_bytes_site = {"fire": 160.0, "gd": 80.0, "nesterov": 120.0}[args.method] + flag_byte
+    alg_bytes_site = {"fire": 160.0, "gd": 80.0, "nesterov": 120.0, "analyze": 73.0}[args.method] + flag_byte
     launch_ms = ms / max(rep["sweep_launches"], 1)           # average launch duration over the timed region
     achieved = alg_bytes_site * N / (launch_ms * 1e-3) / 1e9
     design_bytes_site = lq.lq_get_info(ctx, "sweep_bytes_per_site") if args.method == "fire" else alg_bytes_site
     three = c["L2"] != 0 or c["L3"] != 0
-    if args.method != "fire":
+    if args.method == "analyze":
+        kernel_name = "k_analyze"
+    elif args.method != "fire":
         kernel_name = "k_descent" if (three or args.fire_path == 1) else "k_descent_sweep"
     else:
         kernel_name = {1: "k_fire1_force"}.get(args.fire_path, "k_sweep" if (three or args.fire_path == 2) else "k_sweep_rc")
@@ -336,7 +355,7 @@ def main():
         v, cores, desc, _, _ = time_oracle(c, target_s=15.0, crop=args.ref_crop, method=args.method, eta=args.eta, mu=args.mu)
         cpu = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc}
 
-    metric = METRIC if args.method == "fire" else METRIC.replace("FIRE", {"gd": "gradient-descent", "nesterov": "Nesterov"}[args.method])
+    metric = METRIC if args.method == "fire" else METRIC.replace("FIRE", {"gd": "gradient-descent", "nesterov": "Nesterov", "analyze": "director/S/defect analysis"}[args.method])
     line = {"metric": metric, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
             "ms_per_step": ms_max / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic",

@@ -166,6 +166,17 @@ typedef struct {
 int lq_descent_minimize(lq_ctx *ctx, int method, long max_steps, double force_tol,
                         const lq_descent_params *params, lq_fire_report *out);
 
+/* Per-site analysis of the current Q: "The nematic director can be recovered as the eigenvector
+ * corresponding to the largest eigenvalue of Q, which equals S" (Eq. 2); defects are "regions where
+ * the largest eigenvalue of Q falls below some threshold".  Outputs are dense (unpadded) arrays in
+ * lattice order s = x + Lx (y + Ly z), each may be NULL: S [N]; director [3][N] SoA, unit length, the component of
+ * largest magnitude positive (first such on ties; the director is headless); defect [N] bytes, 1 where
+ * S < S_threshold; *n_defect (host long) = number of such sites.  Object sites get S = 0, director = 0, defect = 0.
+ * Where the largest eigenvalue is degenerate the director is any unit vector of its eigenspace.
+ * One streaming kernel launch.  Errors: LQ_ERR_STATE before lq_set_Q, LQ_ERR_ARG on a bad `where`. */
+int lq_analyze(lq_ctx *ctx, double S_threshold, double *S, double *director, uint8_t *defect, long *n_defect,
+               int where);
+
 /* S0 of Eq. 7 for the context's A, B, C (host double). */
 int lq_get_S0(lq_ctx *ctx, double *S0);
 

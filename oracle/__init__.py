@@ -7,6 +7,7 @@ citations and the list of pins.
 """
 from .lq_oracle import (  # noqa: F401
     Oracle,
+    analyze,
     build_oracle,
     oracle_lib_path,
     q0_of,

@@ -192,3 +192,33 @@ class Oracle:
             raise MemoryError("lqo_descent rc=%d" % rc)
         report = {k: getattr(rep, k) for k, _ in _FireReport._fields_}
         return (q, report, tr[: report["steps"]]) if trace else (q, report)
+
+
+def analyze(q, mask=None, threshold=0.0):
+    """Director, degree of order and defect mask of a Q field, the plain definition:
+    "The nematic director can be recovered as the eigenvector corresponding to the largest eigenvalue of Q, which
+    equals S" (Eq. 2) and defects are "regions where the largest eigenvalue of Q falls below some
+    threshold".  numpy.linalg.eigh per site (a library routine as the one step).
+    q [5][N] (xx, xy, xz, yy, yz); mask [N] or None.  Returns S [N], n [3][N] (unit, sign: largest-|.| component
+    positive, first such component on ties), defect [N] uint8 (S < threshold); object sites get S = 0, n = 0, 0."""
+    q = np.ascontiguousarray(q, dtype=np.float64)
+    N = q.size // 5
+    q = q.reshape(5, N)
+    Q = np.empty((N, 3, 3))
+    Q[:, 0, 0], Q[:, 0, 1], Q[:, 0, 2] = q[0], q[1], q[2]
+    Q[:, 1, 0], Q[:, 1, 1], Q[:, 1, 2] = q[1], q[3], q[4]
+    Q[:, 2, 0], Q[:, 2, 1], Q[:, 2, 2] = q[2], q[4], -q[0] - q[3]
+    w, v = np.linalg.eigh(Q)                     # ascending eigenvalues
+    S = w[:, 2].copy()
+    n = v[:, :, 2].T.copy()                      # [3][N]
+    k = np.argmax(np.abs(n), axis=0)
+    sgn = np.sign(n[k, np.arange(N)])
+    sgn[sgn == 0] = 1.0
+    n *= sgn
+    defect = (S < threshold).astype(np.uint8)
+    if mask is not None:
+        obj = np.asarray(mask).reshape(N) != 0
+        S[obj] = 0.0
+        n[:, obj] = 0.0
+        defect[obj] = 0
+    return S, n, defect

@@ -23,7 +23,7 @@ _lib = None
 
 # every symbol include/lq.h declares (checked by tests/test_abi.py against the header)
 SYMBOLS = ["lq_create", "lq_destroy", "lq_set_stream", "lq_set_sites", "lq_get_flags", "lq_set_Q", "lq_get_Q",
-           "lq_get_velocity", "lq_set_field", "lq_energy", "lq_energy_terms", "lq_forces", "lq_fire_minimize", "lq_descent_minimize", "lq_get_S0",
+           "lq_get_velocity", "lq_set_field", "lq_analyze", "lq_energy", "lq_energy_terms", "lq_forces", "lq_fire_minimize", "lq_descent_minimize", "lq_get_S0",
            "lq_set_option", "lq_get_info", "lq_last_error", "lq_version"]
 
 
@@ -79,6 +79,7 @@ def load():
     L.lq_energy_terms.argtypes = [vp, dp]
     L.lq_forces.argtypes = [vp, vp, ip]
     L.lq_fire_minimize.argtypes = [vp, C.c_long, C.c_double, C.POINTER(lq_fire_params), C.POINTER(lq_fire_report)]
+    L.lq_analyze.argtypes = [vp, C.c_double, vp, vp, vp, C.POINTER(C.c_long), ip]
     L.lq_set_field.argtypes = [vp, dp, C.c_double, dp, C.c_double]
     L.lq_descent_minimize.argtypes = [vp, ip, C.c_long, C.c_double, C.POINTER(lq_descent_params), C.POINTER(lq_fire_report)]
     L.lq_get_S0.argtypes = [vp, dp]
@@ -237,6 +238,32 @@ def lq_fire_minimize(ctx, max_steps, force_tol, params: dict, report_energy=Fals
     rep = lq_fire_report()
     _check(ctx.handle, load().lq_fire_minimize(ctx.handle, int(max_steps), float(force_tol), C.byref(fp), C.byref(rep)))
     return {k: getattr(rep, k) for k, _ in lq_fire_report._fields_}
+
+
+def lq_analyze(ctx, threshold=0.0, want_S=True, want_director=True, want_defect=True):
+    """director / S / defect mask of the current Q into fresh host arrays.
+    Returns dict(S [N], director [3][N], defect [N] uint8, n_defect)."""
+    N = ctx.N
+    S = np.empty(N, dtype=np.float64) if want_S else None
+    d = np.empty((3, N), dtype=np.float64) if want_director else None
+    m = np.empty(N, dtype=np.uint8) if want_defect else None
+    cnt = C.c_long()
+
+    def ptr(a):
+        return None if a is None else C.c_void_p(a.ctypes.data)
+    _check(ctx.handle, load().lq_analyze(ctx.handle, float(threshold), ptr(S), ptr(d), ptr(m), C.byref(cnt), LQ_HOST))
+    return {"S": S, "director": d, "defect": m, "n_defect": cnt.value}
+
+
+def lq_analyze_device(ctx, threshold, S=None, director=None, defect=None) -> int:
+    """same, into caller-owned CUDA tensors (float64 [N], float64 [3][N], uint8 [N]; any may be None)"""
+    cnt = C.c_long()
+
+    def ptr(t):
+        return None if t is None else C.c_void_p(t.data_ptr())
+    _check(ctx.handle, load().lq_analyze(ctx.handle, float(threshold), ptr(S), ptr(director), ptr(defect), C.byref(cnt),
+                                         LQ_DEVICE))
+    return cnt.value
 
 
 def lq_set_field(ctx, H=None, chi=0.0, E=None, eps=0.0) -> None:

@@ -433,6 +433,41 @@ int lq_fire_minimize(lq_ctx *c, long max_steps, double force_tol, const lq_fire_
 }
 
 
+int lq_analyze(lq_ctx *c, double thr, double *S, double *dir, uint8_t *defect, long *n_defect, int where) {
+    if (!c) return LQ_ERR_ARG;
+    if (bad_where(where)) return fail(c, LQ_ERR_ARG, "lq_analyze: bad `where`");
+    if (!c->has_Q) return fail(c, LQ_ERR_STATE, "lq_analyze: call lq_set_Q first");
+    const LqGeom &g = c->g;
+    cudaStream_t st = c->stream;
+    const size_t N = (size_t)g.N;
+    double *dS = S, *dD = dir;
+    uint8_t *dF = defect;
+    void *tmp[3] = {nullptr, nullptr, nullptr};
+    auto cleanup = [&]() { for (void *p : tmp) if (p) cudaFree(p); };
+    if (where == LQ_HOST) {                     // stage through device scratch
+        if (S) { if (cudaMalloc(&tmp[0], N * sizeof(double)) != cudaSuccess) { cleanup(); return fail(c, LQ_ERR_NOMEM, "lq_analyze: cudaMalloc"); } dS = (double *)tmp[0]; }
+        if (dir) { if (cudaMalloc(&tmp[1], 3 * N * sizeof(double)) != cudaSuccess) { cleanup(); return fail(c, LQ_ERR_NOMEM, "lq_analyze: cudaMalloc"); } dD = (double *)tmp[1]; }
+        if (defect) { if (cudaMalloc(&tmp[2], N) != cudaSuccess) { cleanup(); return fail(c, LQ_ERR_NOMEM, "lq_analyze: cudaMalloc"); } dF = (uint8_t *)tmp[2]; }
+    }
+    cudaError_t e = cudaMemsetAsync(c->dcounts, 0, sizeof(unsigned long long), st);
+    if (e == cudaSuccess) {
+        lq_launch_analyze(g, c->q[c->cur], c->flags_active ? c->flags : nullptr, thr, dS, dD, dF, c->dcounts, st);
+        e = cudaGetLastError();
+    }
+    unsigned long long cnt = 0;
+    if (e == cudaSuccess) e = cudaMemcpyAsync(&cnt, c->dcounts, sizeof(cnt), cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess && where == LQ_HOST) {
+        if (S) e = cudaMemcpyAsync(S, dS, N * sizeof(double), cudaMemcpyDeviceToHost, st);
+        if (e == cudaSuccess && dir) e = cudaMemcpyAsync(dir, dD, 3 * N * sizeof(double), cudaMemcpyDeviceToHost, st);
+        if (e == cudaSuccess && defect) e = cudaMemcpyAsync(defect, dF, N, cudaMemcpyDeviceToHost, st);
+    }
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    cleanup();
+    if (e != cudaSuccess) return fail(c, LQ_ERR_CUDA, std::string("lq_analyze: ") + cudaGetErrorString(e));
+    if (n_defect) *n_defect = (long)cnt;
+    return LQ_OK;
+}
+
 int lq_set_field(lq_ctx *c, const double *H, double chi, const double *E, double eps) {
     if (!c) return LQ_ERR_ARG;
     double h[3] = {0.0, 0.0, 0.0}, e[3] = {0.0, 0.0, 0.0};

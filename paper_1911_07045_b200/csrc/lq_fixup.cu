@@ -36,8 +36,11 @@ struct FixArgs {
     unsigned int *counter;
 };
 
+#ifndef LQ_FIX_MINB
+#define LQ_FIX_MINB 4
+#endif
 template <bool THREE>
-__global__ void __launch_bounds__(FB) k_fixup(const FixArgs a) {
+__global__ void __launch_bounds__(FB, LQ_FIX_MINB) k_fixup(const FixArgs a) {
     const LqFireScalars sc = *a.sc;
     if (sc.converged) return;
     const int i = blockIdx.x * FB + threadIdx.x;

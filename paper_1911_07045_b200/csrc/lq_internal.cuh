@@ -102,6 +102,8 @@ void lq_launch_fire1_force(const LqGeom &g, const LqPhys &ph, const LqFields &f,
 void lq_launch_fire_update(const double *partials, int nblocks, LqFireScalars *sc_in_out, LqFireConsts fc,
                            int first, cudaStream_t st);
 void lq_launch_zero_object_sites(const LqGeom &g, const uint8_t *flags, double *field, cudaStream_t st);
+void lq_launch_analyze(const LqGeom &g, const double *q, const uint8_t *flags, double thr, double *S, double *dir,
+                       uint8_t *defect, unsigned long long *count, cudaStream_t st);
 void lq_launch_plain_map(const LqGeom &g, const uint8_t *flags, uint8_t *plain, cudaStream_t st);
 void lq_launch_tile_summary(const LqGeom &g, const uint8_t *plain, uint8_t *tsum, int TX, int TY, int ntx, int nty,
                             cudaStream_t st);

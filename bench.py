@@ -334,7 +334,7 @@ def main():
     if args.method == "analyze":
         kernel_name = "k_analyze"
     elif args.method != "fire":
-        kernel_name = "k_descent" if (three or args.fire_path == 1) else "k_descent_sweep"
+        kernel_name = "k_descent" if args.fire_path == 1 else "k_descent_sweep"
     else:
         kernel_name = {1: "k_fire1_force"}.get(args.fire_path, "k_sweep" if (three or args.fire_path == 2) else "k_sweep_rc")
     traffic = None

@@ -185,7 +185,7 @@ int lq_get_S0(lq_ctx *ctx, double *S0);
  *                      state (q, v); L2/L3 != 0: force stored, state (q, v, F)), 1 = unfused four-kernel
  *                      path, 2 = fused sweep with the force stored (any constants).
  *                      lq_descent_minimize: 0 = TMA sweep over the constant-weight sites + list kernel for the
- *                      rest (one-constant; L2/L3 != 0 use the general kernel), 1 = general kernel on every site
+ *                      rest, 1 = general kernel on every site
  *   "sweep_bytes_per_site" (get): algorithmic HBM bytes one sweep moves per site
  *   "n_simulated" (get), "n_boundary" (get), "n_object" (get)
  * Unknown key: LQ_ERR_ARG. */

@@ -215,7 +215,9 @@ struct DS {
     static constexpr int SMEM_BYTES = OFF_RED + 2 * (NT / 32) * 8 + 16;
 };
 
-template <bool NEST, bool MASKED, int NS>
+// THREE: L2/L3 != 0 -- the 19-point constant-weight stencil (lqs::bulk_force_threeconst) reads planes k-1, k, k+1
+// from the ring (three live slots instead of two).
+template <bool NEST, bool MASKED, bool THREE, int NS>
 __global__ void __launch_bounds__(512, 1)
 k_descent_sweep(const __grid_constant__ CUtensorMap tq, const __grid_constant__ CUtensorMap tp, const DescArgs a,
                 const uint8_t *__restrict__ plain, int zc) {
@@ -259,7 +261,7 @@ k_descent_sweep(const __grid_constant__ CUtensorMap tq, const __grid_constant__ 
     for (int c = 0; c < 5; ++c) ym[c] = yc[c] = 0.0;
     long long p = a.g.pidx(x, y, zb - 1);          // padded index of the plane handled now (k = zb + j - 2)
     unsigned pb_next = 1u;
-    int s0 = 0, s1 = NS - 1;
+    int s0 = 0, s1 = NS - 1, s2 = NS - 2;        // ring slots of planes j, j-1, j-2
     uint32_t par = 0;
     for (int j = 0; j < nplanes; ++j) {
         const unsigned pb = pb_next;
@@ -274,11 +276,21 @@ k_descent_sweep(const __grid_constant__ CUtensorMap tq, const __grid_constant__ 
             const int k = zb + j - 2;
             const double *sb = reinterpret_cast<const double *>(smem + s1 * C::SLOT);
             if (!MASKED || pb == 1u) {
-                double lap[5], F[5], o[5];
+                double F[5], o[5];
+                if (!THREE) {
+                    double lap[5];
 #pragma unroll
-                for (int c = 0; c < 5; ++c)
-                    lap[c] = lap7(Y(sb, c, -1), Y(sb, c, 1), Y(sb, c, -C::SW), Y(sb, c, C::SW), ym[c], yn[c], yc[c]);
-                force1(a.ph, yc, lap, F);
+                    for (int c = 0; c < 5; ++c)
+                        lap[c] = lap7(Y(sb, c, -1), Y(sb, c, 1), Y(sb, c, -C::SW), Y(sb, c, C::SW), ym[c], yn[c], yc[c]);
+                    force1(a.ph, yc, lap, F);
+                } else {
+                    const double *sa = reinterpret_cast<const double *>(smem + s2 * C::SLOT);
+                    auto get = [&](int c, int dx, int dy, int dz) -> double {
+                        if (dz != 0 && dx == 0 && dy == 0) return dz < 0 ? ym[c] : yn[c];
+                        return Y(dz < 0 ? sa : (dz > 0 ? sj : sb), c, dy * C::SW + dx);
+                    };
+                    lqs::bulk_force_threeconst(a.ph, get, yc, F);
+                }
 #pragma unroll
                 for (int c = 0; c < 5; ++c) {
                     o[c] = __fma_rn(eta, F[c], yc[c]);
@@ -293,9 +305,11 @@ k_descent_sweep(const __grid_constant__ CUtensorMap tq, const __grid_constant__ 
         if (j >= 1) p += a.g.sz;
 #pragma unroll
         for (int c = 0; c < 5; ++c) { ym[c] = yc[c]; yc[c] = yn[c]; }
-        // plane j-1 (slot s1) has been read by every thread: refill it with plane j-1+NS
+        // the oldest live plane (j-1, or j-2 for the 19-point stencil) has been read by every thread: refill its slot
         __syncthreads();
-        if (tid == 0 && j >= 1 && j - 1 + NS < nplanes) issue(j - 1 + NS, s1);
+        constexpr int DEAD = THREE ? 2 : 1;
+        if (tid == 0 && j >= DEAD && j - DEAD + NS < nplanes) issue(j - DEAD + NS, THREE ? s2 : s1);
+        s2 = s1;
         s1 = s0;
         if (++s0 == NS) { s0 = 0; par ^= 1u; }
     }
@@ -337,20 +351,26 @@ void lq_descent_invalidate(LqDescentPlan *p) {
 namespace {
 constexpr int NS_GD = 6, NS_NEST = 4;   // ring depth: 6 x 25.4 KB (GD), 4 x 50.8 KB (Nesterov)
 
-template <bool NEST, bool MASKED>
-cudaError_t launch_sweep(LqDescentPlan *pl, dim3 grid, const CUtensorMap &mq, const CUtensorMap &mp, const DescArgs &a,
-                         int zc, cudaStream_t st) {
+template <bool NEST, bool MASKED, bool THREE>
+cudaError_t launch_sweep_t(LqDescentPlan *pl, dim3 grid, const CUtensorMap &mq, const CUtensorMap &mp, const DescArgs &a,
+                           int zc, cudaStream_t st) {
     constexpr int NS = NEST ? NS_NEST : NS_GD;
     using C = DS<NEST, NS>;
-    const int v = (NEST ? 2 : 0) + (MASKED ? 1 : 0);
+    const int v = (THREE ? 4 : 0) + (NEST ? 2 : 0) + (MASKED ? 1 : 0);
     if (!pl->attr_set[v]) {
-        cudaError_t e = cudaFuncSetAttribute(k_descent_sweep<NEST, MASKED, NS>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                             C::SMEM_BYTES);
+        cudaError_t e = cudaFuncSetAttribute(k_descent_sweep<NEST, MASKED, THREE, NS>,
+                                             cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES);
         if (e != cudaSuccess) return e;
         pl->attr_set[v] = true;
     }
-    k_descent_sweep<NEST, MASKED, NS><<<grid, C::NT, C::SMEM_BYTES, st>>>(mq, mp, a, pl->plain, zc);
+    k_descent_sweep<NEST, MASKED, THREE, NS><<<grid, C::NT, C::SMEM_BYTES, st>>>(mq, mp, a, pl->plain, zc);
     return cudaGetLastError();
+}
+template <bool NEST, bool MASKED>
+cudaError_t launch_sweep(bool three, LqDescentPlan *pl, dim3 grid, const CUtensorMap &mq, const CUtensorMap &mp,
+                         const DescArgs &a, int zc, cudaStream_t st) {
+    return three ? launch_sweep_t<NEST, MASKED, true>(pl, grid, mq, mp, a, zc, st)
+                 : launch_sweep_t<NEST, MASKED, false>(pl, grid, mq, mp, a, zc, st);
 }
 }  // namespace
 
@@ -367,7 +387,7 @@ int lq_descent_run(LqDescentPlan **planp, int method, int path, const LqGeom &g,
     const bool three = ph.L2 != 0.0 || ph.L3 != 0.0;
     const bool nest = method == LQ_MIN_NESTEROV;
     const bool masked = f.flags != nullptr;
-    const bool fast = path == 0 && !three;
+    const bool fast = path == 0;
     cudaError_t e;
 #define DESC_CUDA(call) do { e = (call); if (e != cudaSuccess) { err = std::string("lq_descent: ") + cudaGetErrorString(e); return LQ_ERR_CUDA; } } while (0)
 
@@ -385,7 +405,7 @@ int lq_descent_run(LqDescentPlan **planp, int method, int path, const LqGeom &g,
         for (int nzc = 1; nzc <= (g.Lz + 7) / 8; ++nzc) {          // equal chunks, modelled makespan on 148 SMs
             const int c = (g.Lz + nzc - 1) / nzc;
             const long long ncta = (long long)ntx * nty * ((g.Lz + c - 1) / c);
-            const long long cost = ((ncta + 147) / 148) * (c + 4);
+            const long long cost = ((ncta + 147) / 148) * (c + (three ? 5 : 4));
             if (best < 0 || cost < best) { best = cost; zc = c; }
         }
         grid = dim3(ntx, nty, (g.Lz + zc - 1) / zc);
@@ -431,10 +451,10 @@ int lq_descent_run(LqDescentPlan **planp, int method, int path, const LqGeom &g,
             if (fast) {
                 a.list = nullptr; a.n = 0; a.partials = pl->sweep_partials; a.extra = nullptr; a.n_extra = 0;
                 a.finish = second ? 0 : 1;
-                if (nest) e = masked ? launch_sweep<true, true>(pl, grid, pl->map[in], pl->map[prev], a, zc, st)
-                                     : launch_sweep<true, false>(pl, grid, pl->map[in], pl->map[prev], a, zc, st);
-                else e = masked ? launch_sweep<false, true>(pl, grid, pl->map[in], pl->map[in], a, zc, st)
-                                : launch_sweep<false, false>(pl, grid, pl->map[in], pl->map[in], a, zc, st);
+                if (nest) e = masked ? launch_sweep<true, true>(three, pl, grid, pl->map[in], pl->map[prev], a, zc, st)
+                                     : launch_sweep<true, false>(three, pl, grid, pl->map[in], pl->map[prev], a, zc, st);
+                else e = masked ? launch_sweep<false, true>(three, pl, grid, pl->map[in], pl->map[in], a, zc, st)
+                                : launch_sweep<false, false>(three, pl, grid, pl->map[in], pl->map[in], a, zc, st);
                 DESC_CUDA(e);
             }
             if (second) {

@@ -68,7 +68,7 @@ def test_q_after_K_steps(case, lq, method):
 def test_general_kernel_path_matches_too(lq, oracle_mod, method):
     """fire_path = 1 runs k_descent over every site (no TMA sweep): same oracle, same tolerance; and the two GPU
     paths agree with each other far below it"""
-    for name in ("masked_70x35x9_L1only", "replica5p"):
+    for name in ("masked_70x35x9_L1only", "replica5p", "replica3", "masked_37x21x11"):
         build, K = CASES[name]
         c = build()
         o = make_oracle(oracle_mod, c)

@@ -58,6 +58,7 @@ typedef struct {
     const double *axis;      /* [3][N] unit vector n0 (kind 1) or nu (kind 2)  */
     /* external fields, Eq. 13: uniform H and E; chi = mu0 Delta-chi, eps = eps0 Delta-eps */
     double H[3], chi, E[3], eps;
+    double L4;               /* chiral distortion constant of Eq. 10 */
 } lqo_problem;
 
 typedef struct { double dt0, dtmax, alpha0, finc, fdec, falpha; int Nmin; int integrator; } lqo_fire_params;
@@ -274,13 +275,34 @@ static void allowed_signs(const lqo_problem *p, int x, int y, int z, int nopt[3]
     }
 }
 
-/* Eq. 10 with L4 = L6 = 0 for one choice of difference tensors
- * D[k][i][j] ~ dQ_ij/dx_k; index loops exactly as printed.  If gD != NULL it
- * receives d f / d D[k][i][j] by the product rule applied term by term.       */
-static double f_distortion(const lqo_problem *p, const double D[3][3][3], double gD[3][3][3])
+/* Levi-Civita symbol */
+static inline double eps3(int i, int j, int k) { return (double)((i - j) * (j - k) * (k - i)) / 2.0; }
+
+/* Eq. 10 with L6 = 0 for one choice of difference tensors
+ * D[k][i][j] ~ dQ_ij/dx_k and the site's own tensor Q (the chiral term
+ * L4/2 eps_lik Q_lj dQ_ij/dx_k carries an undifferentiated Q); index loops
+ * exactly as printed.  If gD != NULL it receives d f / d D[k][i][j] and gQ
+ * d f / d Q[l][j] (entries independent) by the product rule term by term.     */
+static double f_distortion(const lqo_problem *p, const double Q[3][3], const double D[3][3][3],
+                           double gD[3][3][3], double gQ[3][3])
 {
     double f = 0.0;
-    if (gD) memset(gD, 0, 27 * sizeof(double));
+    if (gD) { memset(gD, 0, 27 * sizeof(double)); memset(gQ, 0, 9 * sizeof(double)); }
+    if (p->L4 != 0.0)
+        for (int l = 0; l < 3; ++l)
+            for (int i = 0; i < 3; ++i)
+                for (int k = 0; k < 3; ++k) {
+                    const double e = eps3(l, i, k);
+                    if (e == 0.0) continue;
+                    for (int j = 0; j < 3; ++j) {
+                        /* L4/2 eps_lik Q_lj dQij/dxk */
+                        f += 0.5 * p->L4 * e * Q[l][j] * D[k][i][j];
+                        if (gD) {
+                            gD[k][i][j] += 0.5 * p->L4 * e * Q[l][j];
+                            gQ[l][j] += 0.5 * p->L4 * e * D[k][i][j];
+                        }
+                    }
+                }
     for (int i = 0; i < 3; ++i)
         for (int j = 0; j < 3; ++j)
             for (int k = 0; k < 3; ++k) {
@@ -334,7 +356,7 @@ static double site_literal(const lqo_problem *p, const double *q, int x, int y, 
         for (int b = 0; b < nopt[1]; ++b)
             for (int c = 0; c < nopt[2]; ++c) {
                 const int sg[3] = { opt[0][a], opt[1][b], opt[2][c] };
-                double D[3][3][3], gD[3][3][3];
+                double D[3][3][3], gD[3][3][3], gQ[3][3];
                 for (int k = 0; k < 3; ++k)
                     for (int i = 0; i < 3; ++i)
                         for (int j = 0; j < 3; ++j) {
@@ -343,7 +365,10 @@ static double site_literal(const lqo_problem *p, const double *q, int x, int y, 
                             else if (sg[k] < 0) D[k][i][j] = Q[i][j] - Qn[k][1][i][j];
                             else D[k][i][j] = 0.0;
                         }
-                ed += f_distortion(p, D, g ? gD : NULL) / ncombo;
+                ed += f_distortion(p, Q, D, g ? gD : NULL, gQ) / ncombo;
+                if (g)
+                    for (int i = 0; i < 3; ++i)
+                        for (int j = 0; j < 3; ++j) G9[0][i][j] += gQ[i][j] / ncombo;
                 if (g)
                     for (int k = 0; k < 3; ++k) {
                         if (sg[k] == 0) continue;
@@ -439,6 +464,23 @@ static double site_factorised(const lqo_problem *p, const double *q, int x, int 
                 }
             }
 
+    /* chiral term: linear in the differences, so its mean over the sign combinations is the same expression
+     * on the mean differences Dbar */
+    double gQ4[3][3];
+    memset(gQ4, 0, sizeof(gQ4));
+    if (p->L4 != 0.0)
+        for (int l = 0; l < 3; ++l)
+            for (int i = 0; i < 3; ++i)
+                for (int k = 0; k < 3; ++k) {
+                    const double e = eps3(l, i, k);
+                    if (e == 0.0) continue;
+                    for (int j = 0; j < 3; ++j) {
+                        ed += 0.5 * p->L4 * e * Q[l][j] * Dbar[k][i][j];
+                        gDbar[k][i][j] += 0.5 * p->L4 * e * Q[l][j];
+                        gQ4[l][j] += 0.5 * p->L4 * e * Dbar[k][i][j];
+                    }
+                }
+
     double eb = bulk_energy(p, Q) + field_energy(p, Q);      /* the "bulk" slot carries Eq. 13 too */
     double Ga[3][3];
     double ea = anchoring(p, N, s, Q, g ? Ga : NULL);
@@ -448,6 +490,8 @@ static double site_factorised(const lqo_problem *p, const double *q, int x, int 
         memset(G9, 0, sizeof(G9));
         bulk_grad(p, Q, G9[0]);
         field_grad_add(p, G9[0]);
+        for (int i = 0; i < 3; ++i)
+            for (int j = 0; j < 3; ++j) G9[0][i][j] += gQ4[i][j];
         for (int i = 0; i < 3; ++i)
             for (int j = 0; j < 3; ++j) G9[0][i][j] += Ga[i][j];
         for (int k = 0; k < 3; ++k)

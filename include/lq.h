@@ -145,6 +145,15 @@ int lq_fire_minimize(lq_ctx *ctx, long max_steps, double force_tol,
  * all-zero arguments switch the term off.  Errors: LQ_ERR_ARG on non-finite values. */
 int lq_set_field(lq_ctx *ctx, const double *H, double chi, const double *E, double eps);
 
+/* Chiral distortion constant L4 of Eq. 10: adds
+ *     L4/2 eps_lik Q_lj dQ_ij/dx_k      (in the uniaxial limit L4 = -(8 / 9 S^2) q0 K2)
+ * to the distortion energy of every simulated site, with the same averaged one-sided differences as the other terms
+ * (the term is linear in the derivative, so the average over the allowed sign combinations is the expression on the
+ * mean differences).  With L4 != 0 every minimiser runs the general one-thread-per-site kernels (the fused sweeps'
+ * constant-weight stencils do not carry the term yet).
+ * L4 = 0 switches the term off.  Errors: LQ_ERR_ARG on a non-finite value. */
+int lq_set_chiral(lq_ctx *ctx, double L4);
+
 /* Other first-order minimisers on the same force.  The paper compares FIRE with gradient
  * descent and offers Nesterov's accelerated gradient as its second minimiser
  * without printing either update; the fixed-step textbook forms are used

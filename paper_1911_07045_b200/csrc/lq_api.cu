@@ -336,7 +336,7 @@ int lq_get_info(lq_ctx *c, const char *key, double *value) {
     if (!strcmp(key, "n_object")) { *value = c->flags_active ? (double)c->n_class[2] : 0.0; return LQ_OK; }
     if (!strcmp(key, "sweep_bytes_per_site")) {
         // fused sweep: read + write q, v (and F when it is stored), 5 fp64 each, + the flag byte where objects exist
-        const bool three = c->ph.L2 != 0.0 || c->ph.L3 != 0.0;
+        const bool three = lq_three(c->ph);
         const double fields = (three || c->fire_path == 2) ? 6.0 : 4.0;
         *value = c->fire_path == 1 ? 0.0 : fields * 40.0 + (c->flags_active ? 1.0 : 0.0);
         return LQ_OK;
@@ -358,8 +358,9 @@ int lq_fire_minimize(lq_ctx *c, long max_steps, double force_tol, const lq_fire_
     int rc;
     if ((rc = ensure_field(c, &c->v[c->cur])) != LQ_OK) return rc;
     if ((rc = ensure_field(c, &c->F[c->cur])) != LQ_OK) return rc;
-    const bool fused = c->fire_path != 1;
-    const bool three = c->ph.L2 != 0.0 || c->ph.L3 != 0.0;
+    // the fused sweeps' constant-weight stencils do not carry the chiral term: L4 != 0 runs the general kernels
+    const bool fused = c->fire_path != 1 && c->ph.L4 == 0.0;
+    const bool three = lq_three(c->ph);
     const bool stored_F = three || c->fire_path == 2;   // recompute-F sweep: one-constant only
     if (fused) {
         if ((rc = ensure_field(c, &c->q[c->cur ^ 1])) != LQ_OK) return rc;
@@ -468,6 +469,13 @@ int lq_analyze(lq_ctx *c, double thr, double *S, double *dir, uint8_t *defect, l
     return LQ_OK;
 }
 
+int lq_set_chiral(lq_ctx *c, double L4) {
+    if (!c) return LQ_ERR_ARG;
+    if (!std::isfinite(L4)) return fail(c, LQ_ERR_ARG, "lq_set_chiral: non-finite L4");
+    c->ph.L4 = L4;
+    return LQ_OK;
+}
+
 int lq_set_field(lq_ctx *c, const double *H, double chi, const double *E, double eps) {
     if (!c) return LQ_ERR_ARG;
     double h[3] = {0.0, 0.0, 0.0}, e[3] = {0.0, 0.0, 0.0};
@@ -512,7 +520,7 @@ int lq_descent_minimize(lq_ctx *c, int method, long max_steps, double force_tol,
     LQ_CUDA(c, cudaEventRecord(ev0, st));
     long launches = 0, sweeps = 0;
     int fin = 0;
-    rc = lq_descent_run(&c->descent, method, c->fire_path == 1 ? 1 : 0, g, c->ph, fields_of(c), buf, nbuf, &fin, c->dsc,
+    rc = lq_descent_run(&c->descent, method, (c->fire_path == 1 || c->ph.L4 != 0.0) ? 1 : 0, g, c->ph, fields_of(c), buf, nbuf, &fin, c->dsc,
                         dp->eta, dp->mu, force_tol, max_steps, st, &launches, &sweeps, &h, c->err);
     if (rc == LQ_OK) {
         cudaEventRecord(ev1, st);

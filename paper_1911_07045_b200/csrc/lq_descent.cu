@@ -384,7 +384,7 @@ int lq_descent_run(LqDescentPlan **planp, int method, int path, const LqGeom &g,
                    LqFireScalars *h, std::string &err) {
     LqDescentPlan *pl = *planp;
     if (!pl) { pl = new LqDescentPlan(); *planp = pl; }
-    const bool three = ph.L2 != 0.0 || ph.L3 != 0.0;
+    const bool three = lq_three(ph);
     const bool nest = method == LQ_MIN_NESTEROV;
     const bool masked = f.flags != nullptr;
     const bool fast = path == 0;

@@ -31,7 +31,10 @@ struct LqPhys {
     // external fields, Eq. 13: T_ab = (chi H_a H_b + eps E_a E_b) / 3 in (xx,xy,xz,yy,yz,zz) order,
     // f_external = -T_ab Q_ab; Fx = the constant force it adds in the five stored variables (all 0 without a field)
     double T[6], Fx[5];
+    double L4;   // chiral distortion constant of Eq. 10; 0 = off
 };
+// the 19-point / general mixed-derivative code paths are needed as soon as any of L2, L3, L4 is non-zero
+__host__ __device__ inline bool lq_three(const LqPhys &ph) { return ph.L2 != 0.0 || ph.L3 != 0.0 || ph.L4 != 0.0; }
 
 // FIRE state that lives on the device (Algorithm 1).
 // mix_a, mix_b: the velocity rescale of the step just reduced, v <- mix_a*v + mix_b*F

@@ -321,7 +321,7 @@ void lq_launch_check_u8_max(const LqGeom &g, const uint8_t *arr_p, int maxval, i
 }
 void lq_launch_forces(const LqGeom &g, const LqPhys &ph, const LqFields &f, const double *q, double *F,
                       cudaStream_t st) {
-    if (ph.L2 != 0.0 || ph.L3 != 0.0) k_forces<true><<<site_grid(g), dim3(BX, BY), 0, st>>>(g, ph, f, q, F);
+    if (lq_three(ph)) k_forces<true><<<site_grid(g), dim3(BX, BY), 0, st>>>(g, ph, f, q, F);
     else k_forces<false><<<site_grid(g), dim3(BX, BY), 0, st>>>(g, ph, f, q, F);
 }
 int lq_energy_num_blocks(const LqGeom &g) {
@@ -330,7 +330,7 @@ int lq_energy_num_blocks(const LqGeom &g) {
 }
 void lq_launch_energy(const LqGeom &g, const LqPhys &ph, const LqFields &f, const double *q, double *partials,
                       double *out3, cudaStream_t st) {
-    if (ph.L2 != 0.0 || ph.L3 != 0.0) k_energy<true><<<site_grid(g), dim3(BX, BY), 0, st>>>(g, ph, f, q, partials);
+    if (lq_three(ph)) k_energy<true><<<site_grid(g), dim3(BX, BY), 0, st>>>(g, ph, f, q, partials);
     else k_energy<false><<<site_grid(g), dim3(BX, BY), 0, st>>>(g, ph, f, q, partials);
     k_final_sum<3><<<1, 256, 0, st>>>(partials, lq_energy_num_blocks(g), out3);
 }
@@ -341,7 +341,7 @@ void lq_launch_fire1_drift(const LqGeom &g, const LqFields &f, double *q, double
 }
 void lq_launch_fire1_force(const LqGeom &g, const LqPhys &ph, const LqFields &f, const double *q, double *v,
                            double *F, const LqFireScalars *sc, double *partials, cudaStream_t st) {
-    if (ph.L2 != 0.0 || ph.L3 != 0.0)
+    if (lq_three(ph))
         k_fire1_force<true><<<site_grid(g), dim3(BX, BY), 0, st>>>(g, ph, f, q, v, F, sc, partials);
     else
         k_fire1_force<false><<<site_grid(g), dim3(BX, BY), 0, st>>>(g, ph, f, q, v, F, sc, partials);

@@ -203,6 +203,24 @@ __device__ __forceinline__ void site_force(const LqPhys &ph, const Acc &acc, uns
                     G[a][m1] += coef * ph.L3 * D1[m6(a, c)];
                     G[a][m2] += coef * ph.L3 * D2[m6(a, c)];
                 }
+                // chiral term: H^(c)_ab(y) = d f4(y) / d(Dbar_c Q_ab) = L4/2 eps_lac Q_lb(y)
+#pragma unroll
+                for (int b = 0; b < 3; ++b) {
+                    G[m2][b] += coef * 0.5 * ph.L4 * Qy[m6(m1, b)];
+                    G[m1][b] -= coef * 0.5 * ph.L4 * Qy[m6(m2, b)];
+                }
+            }
+        }
+        if (ph.L4 != 0.0) {
+            // ... and its undifferentiated factor: d f4(x) / dQ_ab(x) = L4/2 eps_aik Dbar_k Q_ib(x)
+            double Dk[3][6];
+#pragma unroll
+            for (int k = 0; k < 3; ++k) dbar(acc, 0, 0, 0, fl, Qx, k, Dk[k]);
+#pragma unroll
+            for (int a = 0; a < 3; ++a) {
+                const int a1 = (a + 1) % 3, a2 = (a + 2) % 3;
+#pragma unroll
+                for (int b = 0; b < 3; ++b) G[a][b] += 0.5 * ph.L4 * (Dk[a2][m6(a1, b)] - Dk[a1][m6(a2, b)]);
             }
         }
     }
@@ -256,6 +274,14 @@ __device__ __forceinline__ void site_energy(const LqPhys &ph, const Acc &acc, un
                     ed += ph.L2 * Db[j][m6(i, j)] * Db[k][m6(i, k)];
                     ed += ph.L3 * Db[j][m6(i, k)] * Db[k][m6(i, j)];
                 }
+        // chiral term L4/2 eps_lik Q_lj Dbar_k Q_ij: for axis k the pairs (l, i) = (k+1, k+2) [+1] and (k+2, k+1) [-1]
+#pragma unroll
+        for (int k = 0; k < 3; ++k) {
+            const int k1 = (k + 1) % 3, k2 = (k + 2) % 3;
+#pragma unroll
+            for (int j = 0; j < 3; ++j)
+                ed += 0.5 * ph.L4 * (Qx[m6(k1, j)] * Db[k][m6(k2, j)] - Qx[m6(k2, j)] * Db[k][m6(k1, j)]);
+        }
     }
     terms[1] = ed;
 }

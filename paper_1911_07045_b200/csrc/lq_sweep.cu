@@ -318,7 +318,7 @@ int lq_sweep_run(LqSweepPlan **planp, bool stored_F, const LqGeom &g, const LqPh
                  cudaStream_t st, long *launches, long *sweeps, LqFireScalars *h, std::string &err) {
     using C1 = Cfg<32, 16>;   // one-constant: 512 threads, <= 128 registers
     using C3 = Cfg<32, 16>;   // three-constant: same tile (ptxas fits the 19-point fast path in 128 registers)
-    const bool three = ph.L2 != 0.0 || ph.L3 != 0.0;
+    const bool three = lq_three(ph);
     const bool masked = f.flags != nullptr;
     LqSweepPlan *pl = *planp;
     if (!pl) {

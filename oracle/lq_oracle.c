@@ -59,6 +59,7 @@ typedef struct {
     /* external fields, Eq. 13: uniform H and E; chi = mu0 Delta-chi, eps = eps0 Delta-eps */
     double H[3], chi, E[3], eps;
     double L4;               /* chiral distortion constant of Eq. 10 */
+    double L6;               /* cubic distortion constant of Eq. 10 */
 } lqo_problem;
 
 typedef struct { double dt0, dtmax, alpha0, finc, fdec, falpha; int Nmin; int integrator; } lqo_fire_params;
@@ -278,7 +279,7 @@ static void allowed_signs(const lqo_problem *p, int x, int y, int z, int nopt[3]
 /* Levi-Civita symbol */
 static inline double eps3(int i, int j, int k) { return (double)((i - j) * (j - k) * (k - i)) / 2.0; }
 
-/* Eq. 10 with L6 = 0 for one choice of difference tensors
+/* Eq. 10, all five terms, for one choice of difference tensors
  * D[k][i][j] ~ dQ_ij/dx_k and the site's own tensor Q (the chiral term
  * L4/2 eps_lik Q_lj dQ_ij/dx_k carries an undifferentiated Q); index loops
  * exactly as printed.  If gD != NULL it receives d f / d D[k][i][j] and gQ
@@ -288,6 +289,19 @@ static double f_distortion(const lqo_problem *p, const double Q[3][3], const dou
 {
     double f = 0.0;
     if (gD) { memset(gD, 0, 27 * sizeof(double)); memset(gQ, 0, 9 * sizeof(double)); }
+    if (p->L6 != 0.0)
+        for (int l = 0; l < 3; ++l)
+            for (int k = 0; k < 3; ++k)
+                for (int i = 0; i < 3; ++i)
+                    for (int j = 0; j < 3; ++j) {
+                        /* L6/2 Q_lk dQij/dxl dQij/dxk */
+                        f += 0.5 * p->L6 * Q[l][k] * D[l][i][j] * D[k][i][j];
+                        if (gD) {
+                            gD[l][i][j] += 0.5 * p->L6 * Q[l][k] * D[k][i][j];
+                            gD[k][i][j] += 0.5 * p->L6 * Q[l][k] * D[l][i][j];
+                            gQ[l][k] += 0.5 * p->L6 * D[l][i][j] * D[k][i][j];
+                        }
+                    }
     if (p->L4 != 0.0)
         for (int l = 0; l < 3; ++l)
             for (int i = 0; i < 3; ++i)
@@ -480,6 +494,28 @@ static double site_factorised(const lqo_problem *p, const double *q, int x, int 
                         gQ4[l][j] += 0.5 * p->L4 * e * Dbar[k][i][j];
                     }
                 }
+
+    /* cubic term L6/2 Q_lk D_l Q_ij D_k Q_ij: quadratic in the differences like the L1..L3 terms, so same-axis
+     * products (l == k) average to the mean of squares and different-axis products to products of Dbar */
+    if (p->L6 != 0.0)
+        for (int l = 0; l < 3; ++l)
+            for (int k = 0; k < 3; ++k)
+                for (int i = 0; i < 3; ++i)
+                    for (int j = 0; j < 3; ++j) {
+                        if (l == k) {
+                            for (int d = 0; d < 2; ++d)
+                                if (ok[k][d]) {
+                                    ed += 0.5 * p->L6 * Q[k][k] * Ds[k][d][i][j] * Ds[k][d][i][j] / cnt[k];
+                                    gDs[k][d][i][j] += p->L6 * Q[k][k] * Ds[k][d][i][j] / cnt[k];
+                                    gQ4[k][k] += 0.5 * p->L6 * Ds[k][d][i][j] * Ds[k][d][i][j] / cnt[k];
+                                }
+                        } else {
+                            ed += 0.5 * p->L6 * Q[l][k] * Dbar[l][i][j] * Dbar[k][i][j];
+                            gDbar[l][i][j] += 0.5 * p->L6 * Q[l][k] * Dbar[k][i][j];
+                            gDbar[k][i][j] += 0.5 * p->L6 * Q[l][k] * Dbar[l][i][j];
+                            gQ4[l][k] += 0.5 * p->L6 * Dbar[l][i][j] * Dbar[k][i][j];
+                        }
+                    }
 
     double eb = bulk_energy(p, Q) + field_energy(p, Q);      /* the "bulk" slot carries Eq. 13 too */
     double Ga[3][3];

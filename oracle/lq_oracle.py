@@ -40,7 +40,7 @@ class _Problem(C.Structure):
                 ("L1", C.c_double), ("L2", C.c_double), ("L3", C.c_double),
                 ("mask", C.c_void_p), ("kind", C.c_void_p), ("W", C.c_void_p), ("axis", C.c_void_p),
                 ("H", C.c_double * 3), ("chi", C.c_double), ("E", C.c_double * 3), ("eps", C.c_double),
-                ("L4", C.c_double)]
+                ("L4", C.c_double), ("L6", C.c_double)]
 
 
 class _FireParams(C.Structure):
@@ -110,7 +110,7 @@ class Oracle:
     """One lattice problem held as host numpy arrays; every method calls C."""
 
     def __init__(self, Lx, Ly, Lz, A, B, Cc, L1, L2=0.0, L3=0.0,
-                 mask=None, kind=None, W=None, axis=None, H=(0.0, 0.0, 0.0), chi=0.0, E=(0.0, 0.0, 0.0), eps=0.0, L4=0.0):
+                 mask=None, kind=None, W=None, axis=None, H=(0.0, 0.0, 0.0), chi=0.0, E=(0.0, 0.0, 0.0), eps=0.0, L4=0.0, L6=0.0):
         self.lib = _load()
         self.shape = (int(Lx), int(Ly), int(Lz))
         self.N = int(Lx) * int(Ly) * int(Lz)
@@ -124,7 +124,7 @@ class Oracle:
         self.p = _Problem(int(Lx), int(Ly), int(Lz), A, B, Cc, L1, L2, L3,
                           _ptr(self.mask), _ptr(self.kind), _ptr(self.W), _ptr(self.axis),
                           (C.c_double * 3)(*[float(h) for h in H]), float(chi),
-                          (C.c_double * 3)(*[float(e) for e in E]), float(eps), float(L4))
+                          (C.c_double * 3)(*[float(e) for e in E]), float(eps), float(L4), float(L6))
 
     def _q(self, q):
         q = np.ascontiguousarray(q, dtype=np.float64)

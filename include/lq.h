@@ -154,6 +154,12 @@ int lq_set_field(lq_ctx *ctx, const double *H, double chi, const double *E, doub
  * L4 = 0 switches the term off.  Errors: LQ_ERR_ARG on a non-finite value. */
 int lq_set_chiral(lq_ctx *ctx, double L4);
 
+/* Cubic distortion constant L6 of Eq. 10: adds L6/2 Q_lk dQ_ij/dx_l dQ_ij/dx_k (in the uniaxial
+ * limit L6 = (4 / 27 S^3)(K3 - K1): it separates bend from splay).  Discretised like L1..L3: same-axis
+ * products average to the mean of the squared one-sided differences, different-axis products to products of the
+ * mean differences; the weight Q_lk is the site's own tensor.  Same routing and errors as lq_set_chiral. */
+int lq_set_cubic(lq_ctx *ctx, double L6);
+
 /* Other first-order minimisers on the same force.  The paper compares FIRE with gradient
  * descent and offers Nesterov's accelerated gradient as its second minimiser
  * without printing either update; the fixed-step textbook forms are used

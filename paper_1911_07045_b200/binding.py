@@ -23,7 +23,7 @@ _lib = None
 
 # every symbol include/lq.h declares (checked by tests/test_abi.py against the header)
 SYMBOLS = ["lq_create", "lq_destroy", "lq_set_stream", "lq_set_sites", "lq_get_flags", "lq_set_Q", "lq_get_Q",
-           "lq_get_velocity", "lq_set_field", "lq_set_chiral", "lq_analyze", "lq_energy", "lq_energy_terms", "lq_forces", "lq_fire_minimize", "lq_descent_minimize", "lq_get_S0",
+           "lq_get_velocity", "lq_set_field", "lq_set_chiral", "lq_set_cubic", "lq_analyze", "lq_energy", "lq_energy_terms", "lq_forces", "lq_fire_minimize", "lq_descent_minimize", "lq_get_S0",
            "lq_set_option", "lq_get_info", "lq_last_error", "lq_version"]
 
 
@@ -81,6 +81,7 @@ def load():
     L.lq_fire_minimize.argtypes = [vp, C.c_long, C.c_double, C.POINTER(lq_fire_params), C.POINTER(lq_fire_report)]
     L.lq_analyze.argtypes = [vp, C.c_double, vp, vp, vp, C.POINTER(C.c_long), ip]
     L.lq_set_chiral.argtypes = [vp, C.c_double]
+    L.lq_set_cubic.argtypes = [vp, C.c_double]
     L.lq_set_field.argtypes = [vp, dp, C.c_double, dp, C.c_double]
     L.lq_descent_minimize.argtypes = [vp, ip, C.c_long, C.c_double, C.POINTER(lq_descent_params), C.POINTER(lq_fire_report)]
     L.lq_get_S0.argtypes = [vp, dp]
@@ -270,6 +271,11 @@ def lq_analyze_device(ctx, threshold, S=None, director=None, defect=None) -> int
 def lq_set_chiral(ctx, L4: float) -> None:
     """chiral distortion constant L4 of Eq. 10 (0 = off)"""
     _check(ctx.handle, load().lq_set_chiral(ctx.handle, float(L4)))
+
+
+def lq_set_cubic(ctx, L6: float) -> None:
+    """cubic distortion constant L6 of Eq. 10 (0 = off)"""
+    _check(ctx.handle, load().lq_set_cubic(ctx.handle, float(L6)))
 
 
 def lq_set_field(ctx, H=None, chi=0.0, E=None, eps=0.0) -> None:

@@ -359,7 +359,7 @@ int lq_fire_minimize(lq_ctx *c, long max_steps, double force_tol, const lq_fire_
     if ((rc = ensure_field(c, &c->v[c->cur])) != LQ_OK) return rc;
     if ((rc = ensure_field(c, &c->F[c->cur])) != LQ_OK) return rc;
     // the fused sweeps' constant-weight stencils do not carry the chiral term: L4 != 0 runs the general kernels
-    const bool fused = c->fire_path != 1 && c->ph.L4 == 0.0;
+    const bool fused = c->fire_path != 1 && !lq_general_only(c->ph);
     const bool three = lq_three(c->ph);
     const bool stored_F = three || c->fire_path == 2;   // recompute-F sweep: one-constant only
     if (fused) {
@@ -476,6 +476,13 @@ int lq_set_chiral(lq_ctx *c, double L4) {
     return LQ_OK;
 }
 
+int lq_set_cubic(lq_ctx *c, double L6) {
+    if (!c) return LQ_ERR_ARG;
+    if (!std::isfinite(L6)) return fail(c, LQ_ERR_ARG, "lq_set_cubic: non-finite L6");
+    c->ph.L6 = L6;
+    return LQ_OK;
+}
+
 int lq_set_field(lq_ctx *c, const double *H, double chi, const double *E, double eps) {
     if (!c) return LQ_ERR_ARG;
     double h[3] = {0.0, 0.0, 0.0}, e[3] = {0.0, 0.0, 0.0};
@@ -520,7 +527,7 @@ int lq_descent_minimize(lq_ctx *c, int method, long max_steps, double force_tol,
     LQ_CUDA(c, cudaEventRecord(ev0, st));
     long launches = 0, sweeps = 0;
     int fin = 0;
-    rc = lq_descent_run(&c->descent, method, (c->fire_path == 1 || c->ph.L4 != 0.0) ? 1 : 0, g, c->ph, fields_of(c), buf, nbuf, &fin, c->dsc,
+    rc = lq_descent_run(&c->descent, method, (c->fire_path == 1 || lq_general_only(c->ph)) ? 1 : 0, g, c->ph, fields_of(c), buf, nbuf, &fin, c->dsc,
                         dp->eta, dp->mu, force_tol, max_steps, st, &launches, &sweeps, &h, c->err);
     if (rc == LQ_OK) {
         cudaEventRecord(ev1, st);

@@ -131,6 +131,11 @@ __device__ __forceinline__ double anchoring(const LqPhys &ph, int kind, double W
     return e;
 }
 
+// Frobenius product of two symmetric tensors stored as (xx, xy, xz, yy, yz, zz)
+__device__ __forceinline__ double frodot(const double a[6], const double b[6]) {
+    return a[0] * b[0] + a[3] * b[3] + a[5] * b[5] + 2.0 * (a[1] * b[1] + a[2] * b[2] + a[4] * b[4]);
+}
+
 __device__ __forceinline__ void G_to_F(const double G[3][3], double F[5]) {
     F[0] = -(G[0][0] - G[2][2]);
     F[1] = -(G[0][1] + G[1][0]);
@@ -159,16 +164,26 @@ __device__ __forceinline__ void site_force(const LqPhys &ph, const Acc &acc, uns
             int dx, dy, dz;
             off3(k, s, dx, dy, dz);
             const unsigned fn = acc.flag(dx, dy, dz);
-            const double coef = wx + w_axis(fn, k);
+            const double wn = w_axis(fn, k);
+            const double coef = wx + wn;
             double Qn[6];
             acc.Q(dx, dy, dz, Qn);
+            // cubic term, same-axis part: the bond weight of L1 with Q_kk w_k of the bond's two ends (Eq. 10, L6)
+            const double c6 = THREE ? ph.L6 * (wx * Qx[m6(k, k)] + wn * Qn[m6(k, k)]) : 0.0;
 #pragma unroll
             for (int a = 0; a < 3; ++a)
 #pragma unroll
                 for (int b = 0; b < 3; ++b) {
                     const double cab = ph.L1 + ((THREE && b == k) ? L23 : 0.0);
-                    G[a][b] -= cab * coef * (Qn[m6(a, b)] - Qx[m6(a, b)]);
+                    G[a][b] -= (cab * coef + c6) * (Qn[m6(a, b)] - Qx[m6(a, b)]);
                 }
+            if (THREE && ph.L6 != 0.0) {
+                // ... and its undifferentiated factor Q_kk(x): d/dQ_kk(x) = L6/2 w_k(x) |D^s_k Q(x)|^2
+                double D[6];
+#pragma unroll
+                for (int i = 0; i < 6; ++i) D[i] = Qn[i] - Qx[i];
+                G[k][k] += 0.5 * ph.L6 * wx * frodot(D, D);
+            }
         }
     }
     if (THREE) {
@@ -209,9 +224,17 @@ __device__ __forceinline__ void site_force(const LqPhys &ph, const Acc &acc, uns
                     G[m2][b] += coef * 0.5 * ph.L4 * Qy[m6(m1, b)];
                     G[m1][b] -= coef * 0.5 * ph.L4 * Qy[m6(m2, b)];
                 }
+                // cubic term, mixed part: H^(c)_ab(y) = L6 sum_{l != c} Q_lc(y) Dbar_l Q_ab(y)
+                if (ph.L6 != 0.0) {
+                    const double h1 = coef * ph.L6 * Qy[m6(m1, c)], h2 = coef * ph.L6 * Qy[m6(m2, c)];
+#pragma unroll
+                    for (int a = 0; a < 3; ++a)
+#pragma unroll
+                        for (int b = 0; b < 3; ++b) G[a][b] += h1 * D1[m6(a, b)] + h2 * D2[m6(a, b)];
+                }
             }
         }
-        if (ph.L4 != 0.0) {
+        if (ph.L4 != 0.0 || ph.L6 != 0.0) {
             // ... and its undifferentiated factor: d f4(x) / dQ_ab(x) = L4/2 eps_aik Dbar_k Q_ib(x)
             double Dk[3][6];
 #pragma unroll
@@ -221,6 +244,9 @@ __device__ __forceinline__ void site_force(const LqPhys &ph, const Acc &acc, uns
                 const int a1 = (a + 1) % 3, a2 = (a + 2) % 3;
 #pragma unroll
                 for (int b = 0; b < 3; ++b) G[a][b] += 0.5 * ph.L4 * (Dk[a2][m6(a1, b)] - Dk[a1][m6(a2, b)]);
+                // cubic term, undifferentiated off-diagonal factor: d/dQ_ab(x) = L6/2 Dbar_a Q : Dbar_b Q  (a != b)
+                G[a][a1] += 0.5 * ph.L6 * frodot(Dk[a], Dk[a1]);
+                G[a][a2] += 0.5 * ph.L6 * frodot(Dk[a], Dk[a2]);
             }
         }
     }
@@ -261,6 +287,7 @@ __device__ __forceinline__ void site_energy(const LqPhys &ph, const Acc &acc, un
             if (THREE) {
                 const double col = D[m6(0, k)] * D[m6(0, k)] + D[m6(1, k)] * D[m6(1, k)] + D[m6(2, k)] * D[m6(2, k)];
                 ed += 0.5 * L23 * w * col;
+                ed += 0.5 * ph.L6 * Qx[m6(k, k)] * w * fro;          // cubic term, same-axis part
             }
         }
     }
@@ -274,6 +301,11 @@ __device__ __forceinline__ void site_energy(const LqPhys &ph, const Acc &acc, un
                     ed += ph.L2 * Db[j][m6(i, j)] * Db[k][m6(i, k)];
                     ed += ph.L3 * Db[j][m6(i, k)] * Db[k][m6(i, j)];
                 }
+        // cubic term, mixed part: L6/2 sum_{l != k} Q_lk Dbar_l Q : Dbar_k Q
+#pragma unroll
+        for (int j = 0; j < 3; ++j)
+#pragma unroll
+            for (int k = j + 1; k < 3; ++k) ed += ph.L6 * Qx[m6(j, k)] * frodot(Db[j], Db[k]);
         // chiral term L4/2 eps_lik Q_lj Dbar_k Q_ij: for axis k the pairs (l, i) = (k+1, k+2) [+1] and (k+2, k+1) [-1]
 #pragma unroll
         for (int k = 0; k < 3; ++k) {

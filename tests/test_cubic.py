@@ -68,3 +68,58 @@ def test_uniform_field_feels_nothing(oracle_mod):
     ob = oracle_mod.Oracle(6, 5, 4, A, B, Cc, L1, mask=c["mask"], L6=0.9)
     assert abs(oa.energy(q, 0) - ob.energy(q, 0)) < 1e-13
     assert np.abs(oa.forces(q, 1) - ob.forces(q, 1)).max() < 1e-14
+
+
+# ------------------------------------------------------------------ GPU parity
+
+@pytest.fixture(scope="module")
+def lq():
+    import torch
+    assert torch.cuda.is_available(), "gpu tests need a CUDA device"
+    from paper_1911_07045_b200 import binding, build
+    build.build()
+    binding.load()
+    return binding
+
+
+GPU_CASES = {
+    "masked_37x21x11": lambda: wl.random_masked_problem(103, 37, 21, 11, obj_frac=0.15),
+    "masked_70x35x9_L1only": lambda: wl.random_masked_problem(104, 70, 35, 9, obj_frac=0.1, L2=0.0, L3=0.0),
+    "replica3": lambda: wl.make_replica("3"),
+    "replica4": lambda: wl.make_replica("4"),
+    "replica5p": lambda: wl.make_replica("5p"),
+}
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("name", sorted(GPU_CASES))
+@pytest.mark.parametrize("L4,L6", [(0.0, 0.7), (-0.45, -0.5)])
+def test_gpu_parity_with_cubic_term(lq, oracle_mod, name, L4, L6):
+    """all of Eq. 10 on: forces rel 1e-10, energy and its three terms rel 1e-9, Q after 40 FIRE / GD / Nesterov
+    steps max-abs 1e-8; L6 = L4 = 0 restores the force bit for bit"""
+    c = GPU_CASES[name]()
+    o = oracle_mod.Oracle(c["Lx"], c["Ly"], c["Lz"], c["A"], c["B"], c["C"], c["L1"], c["L2"], c["L3"], mask=c["mask"],
+                          kind=c["kind"], W=c["W"], axis=c["axis"], L4=L4, L6=L6)
+    ctx = lq.create_from_config(c)
+    F0 = lq.lq_forces(ctx)
+    lq.lq_set_chiral(ctx, L4)
+    lq.lq_set_cubic(ctx, L6)
+    Fref = o.forces(c["q"], 1)
+    assert np.abs(lq.lq_forces(ctx) - Fref).max() <= 1e-10 * np.abs(Fref).max()
+    eref, tref = o.energy(c["q"], 1, terms=True)
+    assert abs(lq.lq_energy(ctx) - eref) <= 1e-9 * abs(eref)
+    assert np.abs(lq.lq_energy_terms(ctx) - tref).max() <= 1e-9 * np.abs(tref).max()
+    rep = lq.lq_fire_minimize(ctx, 40, 0.0, c["fire"], report_energy=True)
+    qref, rref = o.fire(c["q"], 40, 0.0, c["fire"], variant=1)
+    assert np.abs(lq.lq_get_Q(ctx) - qref).max() <= 1e-8
+    assert abs(rep["energy"] - rref["energy"]) <= 1e-9 * abs(rref["energy"])
+    for method in (0, 1):
+        lq.lq_set_Q(ctx, np.ascontiguousarray(c["q"]))
+        lq.lq_descent_minimize(ctx, method, 40, 0.0, 0.003, 0.8)
+        qd, _ = o.descent(c["q"], method, 40, 0.0, 0.003, 0.8)
+        assert np.abs(lq.lq_get_Q(ctx) - qd).max() <= 1e-8
+    lq.lq_set_Q(ctx, np.ascontiguousarray(c["q"]))
+    lq.lq_set_chiral(ctx, 0.0)
+    lq.lq_set_cubic(ctx, 0.0)
+    assert np.array_equal(lq.lq_forces(ctx), F0)
+    lq.lq_destroy(ctx)

@@ -33,8 +33,20 @@
  * the total energy on tiny masked lattices, plane-wave/checkerboard response,
  * L2 == L3 on periodic object-free lattices, anchoring closed forms
  * (W_RP = 9 S0^2 W), translation / rotation invariance, FIRE
- * schedule hand trace, classification counts.  Parity UNPINNED: the FIRE
- * trajectory on the full-size configs 3 and 5 (no published numbers).
+ * schedule hand trace, classification counts.  Later additions and their pins:
+ * gradient descent / Nesterov (lqo_descent; tests/test_oracle_descent.py: Eq. 6
+ * scalar recurrence, plane-wave linear recurrences, descent lemma); the external
+ * field term of Eq. 13 (tests/test_field.py: the uniaxial limit printed under
+ * Eq. 13, constant force by hand, finite differences, alignment with H); the
+ * chiral L4 term (tests/test_chiral.py: hand-derived helix energy, the printed
+ * L4 <-> q0 K2 map, preferred pitch) and the cubic L6 term (tests/test_cubic.py:
+ * the printed L <-> K map on twist / splay / bend fields) of Eq. 10; the
+ * director / S / defect analysis lives in lq_oracle.py (numpy.linalg.eigh;
+ * tests/test_analyze.py: Eq. 2 and Eq. 3 round trips).
+ * Parity UNPINNED: the FIRE / GD / Nesterov trajectories on the full-size
+ * configs 3 and 5 (no published numbers) -- GPU-vs-oracle only; the L2-vs-L3
+ * split of the ENERGY next to objects (only L2 + L3 is fixed by the continuum
+ * pin; its gradient is pinned by finite differences).
  *
  * Layout: fields are SoA, q[c*N + s], c in (xx,xy,xz,yy,yz),
  * s = x + Lx*(y + Ly*z); Qzz = -Qxx-Qyy.  Index arithmetic is periodic in all

@@ -402,7 +402,7 @@ int lq_descent_run(LqDescentPlan **planp, int method, int path, const LqGeom &g,
             }
         const int ntx = (g.Lx + 31) / 32, nty = (g.Ly + 15) / 16;
         long long best = -1;
-        for (int nzc = 1; nzc <= (g.Lz + 7) / 8; ++nzc) {          // equal chunks, modelled makespan on 148 SMs
+        for (int nzc = 1; nzc <= (g.Lz + 3) / 4; ++nzc) {          // equal chunks, modelled makespan on 148 SMs
             const int c = (g.Lz + nzc - 1) / nzc;
             const long long ncta = (long long)ntx * nty * ((g.Lz + c - 1) / c);
             const long long cost = ((ncta + 147) / 148) * (c + (three ? 5 : 4));

@@ -345,13 +345,13 @@ int lq_sweep_run(LqSweepPlan **planp, bool stored_F, const LqGeom &g, const LqPh
         pl->three = three;
         pl->stored = stored_F;
         const int ntx = (g.Lx + TX - 1) / TX, nty = (g.Ly + TY - 1) / TY;
-        // z-chunk: aim for >= 4 CTAs per SM worth of work items, chunk >= 8 planes, <= 64
+        // z-chunk: >= 4 planes (small lattices want many short chunks: the machine is otherwise empty), <= 64
         // z-chunking: equal chunks; pick the chunk count that minimises the modelled makespan
         //   waves(ntiles * nzc / 148 SMs, 1 CTA/SM) * (planes per chunk + halo planes + pipeline fill)
         const int halo_planes = stored_F ? 2 : 4;
         long long best = -1;
         int zc = g.Lz;
-        for (int nzc = 1; nzc <= (g.Lz + 7) / 8; ++nzc) {
+        for (int nzc = 1; nzc <= (g.Lz + 3) / 4; ++nzc) {
             const int c = (g.Lz + nzc - 1) / nzc;
             if (c > 64 && nzc < (g.Lz + 63) / 64) continue;
             const long long ncta = (long long)ntx * nty * ((g.Lz + c - 1) / c);

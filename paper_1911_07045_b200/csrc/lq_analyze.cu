@@ -5,8 +5,8 @@
 // the director (24 B) and the defect byte; HBM-bound.
 //
 // Largest eigenvalue of the symmetric traceless 3x3 tensor in closed form (trigonometric solution of the
-// depressed cubic lambda^3 - (p2/2) lambda - det = 0, p2 = tr Q^2), polished by Newton steps on the characteristic
-// polynomial; eigenvector = the largest cross product of two rows of Q - lambda I (rows of a rank-2 matrix span the
+// depressed cubic lambda^3 - (p2/2) lambda - det = 0, p2 = tr Q^2; seeded in fp32), polished to fp64 by Newton steps
+// on the characteristic polynomial; eigenvector = the largest cross product of two rows of Q - lambda I (rows of a rank-2 matrix span the
 // plane normal to its null vector).  Sign convention: the component of largest magnitude is positive (first one
 // on ties), the director being a headless vector.
 #include "lq_internal.cuh"
@@ -28,14 +28,15 @@ __device__ __forceinline__ void top_eigenpair(double xx, double xy, double xz, d
     const double p2 = xx * xx + yy * yy + zz * zz + 2.0 * (xy * xy + xz * xz + yz * yz);       // tr Q^2
     const double det = xx * (yy * zz - yz * yz) - xy * (xy * zz - yz * xz) + xz * (xy * yz - yy * xz);
     if (!(p2 > 0.0)) { lam = 0.0; n[0] = 0.0; n[1] = 0.0; n[2] = 1.0; return; }              // Q == 0: isotropic
-    // lambda = 2 sqrt(p2/6) cos(phi/3), cos(phi) = det / (2 (p2/6)^{3/2}); the root with phi/3 in [0, pi/3] is the largest
+    // lambda = 2 sqrt(p2/6) cos(phi/3), cos(phi) = det / (2 (p2/6)^{3/2}); the root with phi/3 in [0, pi/3] is the
+    // largest.  The trigonometric part only seeds the iteration, so it runs in fp32 (relative error ~1e-6, nudged up
+    // so that the seed sits on the convex side of the root); three fp64 Newton steps on
+    // f(l) = l^3 - (p2/2) l - det then square the error each time (1e-6 -> 1e-12 -> rounding).
     const double s = sqrt(p2 / 6.0);
-    double r = det / (2.0 * s * s * s);
-    r = fmin(1.0, fmax(-1.0, r));
-    lam = 2.0 * s * cos(acos(r) / 3.0);
-    // Newton on f(l) = l^3 - (p2/2) l - det from above (f is convex right of the largest root): 2 steps
+    const float rf = fminf(1.0f, fmaxf(-1.0f, (float)(det / (2.0 * s * s * s))));
+    lam = 2.0 * s * (double)(__cosf(acosf(rf) * (1.0f / 3.0f)) * (1.0f + 3e-6f));
 #pragma unroll
-    for (int it = 0; it < 2; ++it) {
+    for (int it = 0; it < 3; ++it) {
         const double f = (lam * lam - 0.5 * p2) * lam - det, fp = 3.0 * lam * lam - 0.5 * p2;
         if (fp > 0.0) lam -= f / fp;
     }
@@ -52,7 +53,7 @@ __device__ __forceinline__ void top_eigenpair(double xx, double xy, double xz, d
         n[0] = 0.0; n[1] = 0.0; n[2] = 1.0;
         return;
     }
-    const double inv = 1.0 / sqrt(d);
+    const double inv = rsqrt(d);
     n[0] = c[0] * inv; n[1] = c[1] * inv; n[2] = c[2] * inv;
     const double a0 = fabs(n[0]), a1 = fabs(n[1]), a2 = fabs(n[2]);
     const double lead = (a0 >= a1 && a0 >= a2) ? n[0] : (a1 >= a2 ? n[1] : n[2]);

@@ -149,15 +149,17 @@ int lq_set_field(lq_ctx *ctx, const double *H, double chi, const double *E, doub
  *     L4/2 eps_lik Q_lj dQ_ij/dx_k      (in the uniaxial limit L4 = -(8 / 9 S^2) q0 K2)
  * to the distortion energy of every simulated site, with the same averaged one-sided differences as the other terms
  * (the term is linear in the derivative, so the average over the allowed sign combinations is the expression on the
- * mean differences).  With L4 != 0 every minimiser runs the general one-thread-per-site kernels (the fused sweeps'
- * constant-weight stencils do not carry the term yet).
+ * mean differences).  L4 != 0 routes every minimiser through the 19-point sweeps (like L2, L3 != 0), whose
+ * constant-weight stencil gains L4 eps_aik C_k Q_ib (C_k = centred difference).
  * L4 = 0 switches the term off.  Errors: LQ_ERR_ARG on a non-finite value. */
 int lq_set_chiral(lq_ctx *ctx, double L4);
 
 /* Cubic distortion constant L6 of Eq. 10: adds L6/2 Q_lk dQ_ij/dx_l dQ_ij/dx_k (in the uniaxial
  * limit L6 = (4 / 27 S^3)(K3 - K1): it separates bend from splay).  Discretised like L1..L3: same-axis
  * products average to the mean of the squared one-sided differences, different-axis products to products of the
- * mean differences; the weight Q_lk is the site's own tensor.  Same routing and errors as lq_set_chiral. */
+ * mean differences; the weight Q_lk is the site's own tensor.  With L6 != 0 every minimiser runs the general
+ * one-thread-per-site kernels (the fused sweeps' constant-weight stencils do not carry the term yet).  Errors as
+ * lq_set_chiral. */
 int lq_set_cubic(lq_ctx *ctx, double L6);
 
 /* Other first-order minimisers on the same force.  The paper compares FIRE with gradient

@@ -217,7 +217,7 @@ struct DS {
 
 // THREE: L2/L3 != 0 -- the 19-point constant-weight stencil (lqs::bulk_force_threeconst) reads planes k-1, k, k+1
 // from the ring (three live slots instead of two).
-template <bool NEST, bool MASKED, bool THREE, int NS>
+template <bool NEST, bool MASKED, bool THREE, bool CHIRAL, int NS>
 __global__ void __launch_bounds__(512, 1)
 k_descent_sweep(const __grid_constant__ CUtensorMap tq, const __grid_constant__ CUtensorMap tp, const DescArgs a,
                 const uint8_t *__restrict__ plain, int zc) {
@@ -289,7 +289,7 @@ k_descent_sweep(const __grid_constant__ CUtensorMap tq, const __grid_constant__ 
                         if (dz != 0 && dx == 0 && dy == 0) return dz < 0 ? ym[c] : yn[c];
                         return Y(dz < 0 ? sa : (dz > 0 ? sj : sb), c, dy * C::SW + dx);
                     };
-                    lqs::bulk_force_threeconst(a.ph, get, yc, F);
+                    lqs::bulk_force_threeconst<CHIRAL>(a.ph, get, yc, F);
                 }
 #pragma unroll
                 for (int c = 0; c < 5; ++c) {
@@ -332,7 +332,7 @@ struct LqDescentPlan {
     int n_list = 0;
     const uint8_t *flags_seen = nullptr;
     bool sites_dirty = true;
-    bool attr_set[8] = {false, false, false, false, false, false, false, false};
+    bool attr_set[16] = {};
 };
 
 void lq_descent_destroy(LqDescentPlan *p) {
@@ -351,24 +351,25 @@ void lq_descent_invalidate(LqDescentPlan *p) {
 namespace {
 constexpr int NS_GD = 6, NS_NEST = 4;   // ring depth: 6 x 25.4 KB (GD), 4 x 50.8 KB (Nesterov)
 
-template <bool NEST, bool MASKED, bool THREE>
+template <bool NEST, bool MASKED, bool THREE, bool CHIRAL = false>
 cudaError_t launch_sweep_t(LqDescentPlan *pl, dim3 grid, const CUtensorMap &mq, const CUtensorMap &mp, const DescArgs &a,
                            int zc, cudaStream_t st) {
     constexpr int NS = NEST ? NS_NEST : NS_GD;
     using C = DS<NEST, NS>;
-    const int v = (THREE ? 4 : 0) + (NEST ? 2 : 0) + (MASKED ? 1 : 0);
+    const int v = (CHIRAL ? 8 : 0) + (THREE ? 4 : 0) + (NEST ? 2 : 0) + (MASKED ? 1 : 0);
     if (!pl->attr_set[v]) {
-        cudaError_t e = cudaFuncSetAttribute(k_descent_sweep<NEST, MASKED, THREE, NS>,
+        cudaError_t e = cudaFuncSetAttribute(k_descent_sweep<NEST, MASKED, THREE, CHIRAL, NS>,
                                              cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES);
         if (e != cudaSuccess) return e;
         pl->attr_set[v] = true;
     }
-    k_descent_sweep<NEST, MASKED, THREE, NS><<<grid, C::NT, C::SMEM_BYTES, st>>>(mq, mp, a, pl->plain, zc);
+    k_descent_sweep<NEST, MASKED, THREE, CHIRAL, NS><<<grid, C::NT, C::SMEM_BYTES, st>>>(mq, mp, a, pl->plain, zc);
     return cudaGetLastError();
 }
 template <bool NEST, bool MASKED>
 cudaError_t launch_sweep(bool three, LqDescentPlan *pl, dim3 grid, const CUtensorMap &mq, const CUtensorMap &mp,
                          const DescArgs &a, int zc, cudaStream_t st) {
+    if (three && a.ph.L4 != 0.0) return launch_sweep_t<NEST, MASKED, true, true>(pl, grid, mq, mp, a, zc, st);
     return three ? launch_sweep_t<NEST, MASKED, true>(pl, grid, mq, mp, a, zc, st)
                  : launch_sweep_t<NEST, MASKED, false>(pl, grid, mq, mp, a, zc, st);
 }

@@ -342,7 +342,10 @@ __device__ __forceinline__ void bulk_force_oneconst(const LqPhys &ph, const doub
 //   F1 = 2 L1 lap xy + L23[d2x xy + d2y xy + Xxy xx + Xxy yy + Xyz xz + Xxz yz]
 //   F2 = 2 L1 lap xz + L23[d2x xz + d2z xz + Xyz xy + Xxy yz - Xxz yy]
 //   F4 = 2 L1 lap yz + L23[d2y yz + d2z yz + Xxz xy + Xxy xz - Xyz xx]
-template <class Get>
+// CHIRAL: also the L4 term on constant weights, G_ab += L4 eps_aik C_k Q_ib with centred differences C_k (the
+// gather form of lqs::site_force at a site whose weights are all 1/2) -- a template flag so
+// that the achiral instantiations keep their register budget.
+template <bool CHIRAL = false, class Get>
 __device__ __forceinline__ void bulk_force_threeconst(const LqPhys &ph, const Get &g, const double qc[5], double F[5]) {
     const double L1 = ph.L1, L23 = ph.L2 + ph.L3;
     auto d2 = [&](int c, int ax) -> double {
@@ -394,6 +397,25 @@ __device__ __forceinline__ void bulk_force_threeconst(const LqPhys &ph, const Ge
         F[2] += L23 * X(4, 0, 1);
         F[1] += L23 * X(4, 0, 2);
         F[0] -= L23 * X(4, 1, 2);
+    }
+    if (CHIRAL) {
+        double Cd[3][6];                 // C_k of (xx, xy, xz, yy, yz, zz)
+#pragma unroll
+        for (int k = 0; k < 3; ++k) {
+#pragma unroll
+            for (int c = 0; c < 5; ++c)
+                Cd[k][c] = 0.5 * (g(c, k == 0, k == 1, k == 2) - g(c, -(k == 0), -(k == 1), -(k == 2)));
+            Cd[k][5] = -Cd[k][0] - Cd[k][3];
+        }
+        double G4[3][3];
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+            const int a1 = (a + 1) % 3, a2 = (a + 2) % 3;
+#pragma unroll
+            for (int b = 0; b < 3; ++b) G4[a][b] = ph.L4 * (Cd[a2][m6(a1, b)] - Cd[a1][m6(a2, b)]);
+        }
+        F[0] -= G4[0][0] - G4[2][2]; F[1] -= G4[0][1] + G4[1][0]; F[2] -= G4[0][2] + G4[2][0];
+        F[3] -= G4[1][1] - G4[2][2]; F[4] -= G4[1][2] + G4[2][1];
     }
 }
 

@@ -54,7 +54,7 @@ struct Cfg {
     static constexpr int NHALO = 2 * BXW + 2 * (BYH - 2);
 };
 
-template <class C, bool THREE, bool MASKED>
+template <class C, bool THREE, bool MASKED, bool CHIRAL>
 __global__ void __launch_bounds__(C::NT, 1)
 k_sweep(const __grid_constant__ CUtensorMap tq, const __grid_constant__ CUtensorMap tv,
         const __grid_constant__ CUtensorMap tF, const SweepArgs a) {
@@ -175,7 +175,7 @@ k_sweep(const __grid_constant__ CUtensorMap tq, const __grid_constant__ CUtensor
                             if (dx == 0 && dy == 0) return dz < 0 ? qm[c] : qp[c];
                             return (dz < 0 ? rkm : rn)[c * C::PLANE + idx + dy * C::BXW + dx];
                         };
-                        lqs::bulk_force_threeconst(a.ph, get, qc, Fn);
+                        lqs::bulk_force_threeconst<CHIRAL>(a.ph, get, qc, Fn);
                     }
 #pragma unroll
                     for (int c = 0; c < 5; ++c) {
@@ -283,7 +283,7 @@ struct LqSweepPlan {
     bool sites_dirty = true;
     dim3 grid;
     int zc = 0;
-    bool attr_set[4] = {false, false, false, false};
+    bool attr_set[6] = {false, false, false, false, false, false};
 };
 
 void lq_sweep_destroy(LqSweepPlan *p) {
@@ -301,15 +301,15 @@ void lq_sweep_invalidate(LqSweepPlan *p) {
     if (p) p->sites_dirty = true;
 }
 
-template <class C, bool THREE, bool MASKED>
+template <class C, bool THREE, bool MASKED, bool CHIRAL = false>
 static cudaError_t launch(LqSweepPlan *pl, int in, const SweepArgs &a, int variant, cudaStream_t st) {
     if (!pl->attr_set[variant]) {
-        cudaError_t e = cudaFuncSetAttribute(k_sweep<C, THREE, MASKED>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+        cudaError_t e = cudaFuncSetAttribute(k_sweep<C, THREE, MASKED, CHIRAL>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                              C::SMEM_BYTES);
         if (e != cudaSuccess) return e;
         pl->attr_set[variant] = true;
     }
-    k_sweep<C, THREE, MASKED><<<pl->grid, C::NT, C::SMEM_BYTES, st>>>(pl->mq[in], pl->mv[in], pl->mF[in], a);
+    k_sweep<C, THREE, MASKED, CHIRAL><<<pl->grid, C::NT, C::SMEM_BYTES, st>>>(pl->mq[in], pl->mv[in], pl->mF[in], a);
     return cudaGetLastError();
 }
 
@@ -410,6 +410,8 @@ int lq_sweep_run(LqSweepPlan **planp, bool stored_F, const LqGeom &g, const LqPh
             const int in = (int)((cur0 + done + i) & 1), out = in ^ 1;
             a.qo = q[out]; a.vo = v[out]; a.Fo = F[out]; a.Fi = F[in];
             if (!stored_F) e = lq_launch_sweep_rc(masked, pl->grid, pl->mq[in], pl->mv[in], a, st);
+            else if (three && ph.L4 != 0.0)
+                e = masked ? launch<C3, true, true, true>(pl, in, a, 5, st) : launch<C3, true, false, true>(pl, in, a, 4, st);
             else if (three) e = masked ? launch<C3, true, true>(pl, in, a, 3, st) : launch<C3, true, false>(pl, in, a, 2, st);
             else e = masked ? launch<C1, false, true>(pl, in, a, 1, st) : launch<C1, false, false>(pl, in, a, 0, st);
             if (e == cudaSuccess && masked)

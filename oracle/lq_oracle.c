@@ -725,7 +725,60 @@ int lqo_fire(const lqo_problem *p, double *q, double *v_out, long max_steps, dou
     reduce4(p, F, v, N, &P, &FF, &vv, &Fmax);
     if (Fmax < force_tol) converged = 1;
 
-    while (!converged && step < max_steps) {
+    /* integrator 1 (R30): FIRE on the plain semi-implicit Euler step,
+     *     v += dt F(q);  P, |F|^2, |v|^2;  mix;  schedule;  q += dt v  (the step's dt, the mixed / reset v),
+     * then the new force and the stop test; one force evaluation per step. */
+    while (fp->integrator == 1 && !converged && step < max_steps) {
+        ++step;
+#pragma omp parallel for schedule(static)
+        for (long i = 0; i < 5 * N; ++i) {
+            if (!is_sim(p, i % N)) continue;
+            v[i] += dt * F[i];
+        }
+        double Fm0;
+        reduce4(p, F, v, N, &P, &FF, &vv, &Fm0);
+        double dt_next = dt;
+        if (FF > 0.0) {
+            const double sc = alpha * sqrt(vv / FF);
+#pragma omp parallel for schedule(static)
+            for (long i = 0; i < 5 * N; ++i) {
+                if (!is_sim(p, i % N)) continue;
+                v[i] = (1.0 - alpha) * v[i] + sc * F[i];
+            }
+        }
+        if (P > 0.0) {
+            npos += 1;
+            if (npos > fp->Nmin) {
+                dt_next = fmin(dt * fp->finc, fp->dtmax);
+                alpha *= fp->falpha;
+            }
+        } else {
+            npos = 0;
+            dt_next = dt * fp->fdec;
+            alpha = fp->alpha0;
+            memset(v, 0, 5 * N * sizeof(double));
+        }
+#pragma omp parallel for schedule(static)
+        for (long i = 0; i < 5 * N; ++i) {
+            if (!is_sim(p, i % N)) continue;
+            q[i] += dt * v[i];
+        }
+        dt = dt_next;
+        lqo_forces(p, q, F, variant);
+        {
+            double P1, FF1, vv1;
+            reduce4(p, F, v, N, &P1, &FF1, &vv1, &Fmax);
+            FF = FF1;                    /* reported Frms: of the force at the final q */
+        }
+        if (Fmax < force_tol) converged = 1;
+        if (trace) {
+            double *t = trace + 8 * (step - 1);
+            t[0] = dt; t[1] = alpha; t[2] = (double)npos; t[3] = P; t[4] = FF; t[5] = vv; t[6] = Fmax;
+            t[7] = trace_energy ? lqo_energy(p, q, variant, NULL) : 0.0;
+        }
+    }
+
+    while (fp->integrator == 0 && !converged && step < max_steps) {
         ++step;
         /* velocity Verlet: half kick, drift, new force, half kick */
 #pragma omp parallel for schedule(static)

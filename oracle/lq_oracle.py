@@ -165,7 +165,7 @@ class Oracle:
         """Run FIRE from q (not modified).  Returns (q_final, report dict[, v][, trace])."""
         q = self._q(q).copy()
         fp = _FireParams(params["dt0"], params["dtmax"], params["alpha0"], params["finc"],
-                         params["fdec"], params["falpha"], int(params["Nmin"]), 0)
+                         params["fdec"], params["falpha"], int(params["Nmin"]), int(params.get("integrator", 0)))
         rep = _FireReport()
         v = np.zeros((5, self.N), dtype=np.float64) if return_v else None
         tr = np.zeros((max(int(max_steps), 1), 8), dtype=np.float64) if trace else None

@@ -101,8 +101,10 @@ int lq_energy_terms(lq_ctx *ctx, double *terms);
  * object sites. */
 int lq_forces(lq_ctx *ctx, double *F, int where);
 
-/* FIRE parameters (Algorithm 1).  integrator must be 0 (velocity Verlet,
- * kick-drift-kick; R4).  report_energy != 0 fills lq_fire_report.energy (one extra pass). */
+/* FIRE parameters (Algorithm 1).  integrator 0 = velocity Verlet as kick-drift-kick
+ * (R4; the fused sweeps), 1 = plain semi-implicit Euler (R30): per step
+ * v += dt F(q); P, |F|^2, |v|^2; mix; schedule; q += dt v (the step's dt, the mixed or reset v); then the new force
+ * and the stop test -- one force evaluation per step, run on the general four-launch path.  report_energy != 0 fills lq_fire_report.energy (one extra pass). */
 typedef struct {
     double dt0, dtmax, alpha0, finc, fdec, falpha;
     int Nmin;
@@ -132,7 +134,7 @@ typedef struct {
  * The whole loop runs on the device; the host only polls a flag.  force_tol = 0 runs exactly
  * max_steps steps.  Errors: LQ_ERR_STATE before lq_set_Q; LQ_ERR_ARG on bad parameters
  * (dt0 <= 0, dtmax < dt0, alpha0 outside [0,1], finc < 1, fdec or falpha outside (0,1], Nmin < 0,
- * integrator != 0, max_steps < 0, NULL pointers). */
+ * integrator not 0 or 1, max_steps < 0, NULL pointers). */
 int lq_fire_minimize(lq_ctx *ctx, long max_steps, double force_tol,
                      const lq_fire_params *params, lq_fire_report *out);
 

@@ -350,7 +350,7 @@ int lq_fire_minimize(lq_ctx *c, long max_steps, double force_tol, const lq_fire_
     if (!c->has_Q) return fail(c, LQ_ERR_STATE, "lq_fire_minimize: no Q has been set");
     if (!(fp->dt0 > 0.0) || !(fp->dtmax >= fp->dt0) || !(fp->alpha0 >= 0.0 && fp->alpha0 <= 1.0) ||
         !(fp->finc >= 1.0) || !(fp->fdec > 0.0 && fp->fdec <= 1.0) || !(fp->falpha > 0.0 && fp->falpha <= 1.0) ||
-        fp->Nmin < 0 || fp->integrator != 0 || max_steps < 0 || !(force_tol >= 0.0))
+        fp->Nmin < 0 || (fp->integrator != 0 && fp->integrator != 1) || max_steps < 0 || !(force_tol >= 0.0))
         return fail(c, LQ_ERR_ARG, "lq_fire_minimize: bad FIRE parameter");
     memset(out, 0, sizeof(*out));
     const LqGeom &g = c->g;
@@ -359,7 +359,9 @@ int lq_fire_minimize(lq_ctx *c, long max_steps, double force_tol, const lq_fire_
     if ((rc = ensure_field(c, &c->v[c->cur])) != LQ_OK) return rc;
     if ((rc = ensure_field(c, &c->F[c->cur])) != LQ_OK) return rc;
     // the fused sweeps' constant-weight stencils do not carry the chiral term: L4 != 0 runs the general kernels
-    const bool fused = c->fire_path != 1 && !lq_general_only(c->ph);
+    // ... and so does the semi-implicit Euler variant (integrator = 1)
+    const bool euler = fp->integrator == 1;
+    const bool fused = c->fire_path != 1 && !lq_general_only(c->ph) && !euler;
     const bool three = lq_three(c->ph);
     const bool stored_F = three || c->fire_path == 2;   // recompute-F sweep: one-constant only
     if (fused) {
@@ -373,7 +375,7 @@ int lq_fire_minimize(lq_ctx *c, long max_steps, double force_tol, const lq_fire_
     LqFireConsts fc{fp->dt0, fp->dtmax, fp->alpha0, fp->finc, fp->fdec, fp->falpha, force_tol, fp->Nmin, (long long)max_steps};
     LqFireScalars h;
     memset(&h, 0, sizeof(h));
-    h.dt = 0.0; h.alpha = fp->alpha0; h.mix_a = 1.0; h.mix_b = 0.0;
+    h.dt = euler ? fp->dt0 : 0.0; h.alpha = fp->alpha0; h.mix_a = 1.0; h.mix_b = 0.0;
     LQ_CUDA(c, cudaMemcpyAsync(&c->dsc[0], &h, sizeof(h), cudaMemcpyHostToDevice, st));
     LQ_CUDA(c, cudaMemsetAsync(c->v[c->cur], 0, (size_t)5 * g.NP * sizeof(double), st));
     const LqFields f = fields_of(c);
@@ -385,8 +387,10 @@ int lq_fire_minimize(lq_ctx *c, long max_steps, double force_tol, const lq_fire_
     LQ_CUDA(c, cudaEventRecord(ev0, st));
 
     // step 0: F = force(q), convergence test on the initial state (dt = 0: no kick)
-    lq_launch_fire1_force(g, c->ph, f, c->q[c->cur], c->v[c->cur], c->F[c->cur], &c->dsc[0], c->partials, st);
-    lq_launch_fire_update(c->partials, nb1, &c->dsc[0], fc, 1, st);
+    // (Euler variant: the same launch is the first step's full kick v += dt0 F and its reductions)
+    const long long emax = euler ? (long long)max_steps : -1;
+    lq_launch_fire1_force(g, c->ph, f, c->q[c->cur], c->v[c->cur], c->F[c->cur], &c->dsc[0], c->partials, st, emax);
+    lq_launch_fire_update(c->partials, nb1, &c->dsc[0], fc, euler ? 2 : 1, st);
     launches += 2;
 
     long done = 0;
@@ -399,10 +403,10 @@ int lq_fire_minimize(lq_ctx *c, long max_steps, double force_tol, const lq_fire_
         while (done < max_steps) {
             const long n = (max_steps - done) < chunk ? (max_steps - done) : chunk;
             for (long i = 0; i < n; ++i) {
-                lq_launch_fire1_drift(g, f, c->q[c->cur], c->v[c->cur], c->F[c->cur], &c->dsc[0], st);
+                lq_launch_fire1_drift(g, f, c->q[c->cur], c->v[c->cur], c->F[c->cur], &c->dsc[0], st, euler ? 1 : 0);
                 lq_launch_fill_ghosts_f64(g, c->q[c->cur], 5, st);
-                lq_launch_fire1_force(g, c->ph, f, c->q[c->cur], c->v[c->cur], c->F[c->cur], &c->dsc[0], c->partials, st);
-                lq_launch_fire_update(c->partials, nb1, &c->dsc[0], fc, 0, st);
+                lq_launch_fire1_force(g, c->ph, f, c->q[c->cur], c->v[c->cur], c->F[c->cur], &c->dsc[0], c->partials, st, emax);
+                lq_launch_fire_update(c->partials, nb1, &c->dsc[0], fc, euler ? 2 : 0, st);
             }
             launches += 4 * n;
             done += n;

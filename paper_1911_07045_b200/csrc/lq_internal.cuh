@@ -50,6 +50,7 @@ struct LqFireScalars {
     long long step;  // steps completed
     int npos;
     int converged;
+    double dt_prev;  // semi-implicit Euler variant: the dt of the step just scheduled (its drift uses it)
 };
 
 struct LqFireConsts {
@@ -79,6 +80,26 @@ __host__ __device__ inline void lq_fire_advance(LqFireScalars &t, const LqFireCo
     }
 }
 
+// Same for FIRE on the semi-implicit Euler step (integrator = 1, R30).  tot are the reductions
+// of (F(q_k), v after the full kick v += dt F).  The stop test reads F(q_k); a step is scheduled only while the
+// budget lasts; the drift kernel then applies v <- mix_a v + mix_b F, q += dt_prev v.
+__host__ __device__ inline void lq_fire_advance_euler(LqFireScalars &t, const LqFireConsts &fc, const double tot[4]) {
+    t.FF = tot[1]; t.Fmax = tot[3];
+    if (t.Fmax < fc.force_tol) { t.converged = 1; return; }
+    if (t.step >= fc.max_steps) { t.mix_a = 1.0; t.mix_b = 0.0; t.dt_prev = 0.0; return; }
+    t.step += 1;
+    t.P = tot[0]; t.vv = tot[2];
+    if (t.FF > 0.0) { t.mix_a = 1.0 - t.alpha; t.mix_b = t.alpha * sqrt(t.vv / t.FF); }
+    else { t.mix_a = 1.0; t.mix_b = 0.0; }
+    t.dt_prev = t.dt;
+    if (t.P > 0.0) {
+        t.npos += 1;
+        if (t.npos > fc.Nmin) { t.dt = fmin(t.dt * fc.finc, fc.dtmax); t.alpha *= fc.falpha; }
+    } else {
+        t.npos = 0; t.dt *= fc.fdec; t.alpha = fc.alpha0; t.mix_a = 0.0; t.mix_b = 0.0;
+    }
+}
+
 struct LqFields {
     // padded device arrays; any of flags/kind/W/axis may be null (no objects / no anchoring)
     const uint8_t *flags;
@@ -101,10 +122,13 @@ void lq_launch_energy(const LqGeom &g, const LqPhys &ph, const LqFields &f, cons
 
 // unfused FIRE path (fire_path = 1): 4 launches per step
 int lq_fire1_num_blocks(const LqGeom &g);
+// euler != 0 / euler_max >= 0: the semi-implicit Euler variant (full kick while sc->step < euler_max; drift with
+// dt_prev and no half kick; first == 2 in lq_launch_fire_update)
 void lq_launch_fire1_drift(const LqGeom &g, const LqFields &f, double *q, double *v, const double *F,
-                           const LqFireScalars *sc, cudaStream_t st);
+                           const LqFireScalars *sc, cudaStream_t st, int euler = 0);
 void lq_launch_fire1_force(const LqGeom &g, const LqPhys &ph, const LqFields &f, const double *q, double *v,
-                           double *F, const LqFireScalars *sc, double *partials, cudaStream_t st);
+                           double *F, const LqFireScalars *sc, double *partials, cudaStream_t st,
+                           long long euler_max = -1);
 void lq_launch_fire_update(const double *partials, int nblocks, LqFireScalars *sc_in_out, LqFireConsts fc,
                            int first, cudaStream_t st);
 void lq_launch_zero_object_sites(const LqGeom &g, const uint8_t *flags, double *field, cudaStream_t st);

@@ -179,7 +179,7 @@ __global__ void __launch_bounds__(256) k_final_sum(const double *__restrict__ pa
 //        v += dt/2 F; q += dt v          (simulated sites only)
 __global__ void __launch_bounds__(BX * BY) k_fire1_drift(LqGeom g, LqFields f, double *__restrict__ q,
                                                          double *__restrict__ v, const double *__restrict__ F,
-                                                         const LqFireScalars *__restrict__ sc) {
+                                                         const LqFireScalars *__restrict__ sc, int euler) {
     if (sc->converged) return;
     const int x = blockIdx.x * BX + threadIdx.x;
     const int y = blockIdx.y * BY + threadIdx.y;
@@ -193,9 +193,9 @@ __global__ void __launch_bounds__(BX * BY) k_fire1_drift(LqGeom g, LqFields f, d
             const long long i = c * g.NP + p;
             const double Fc = F[i];
             double vc = ma * v[i] + mb * Fc;
-            vc += 0.5 * dt * Fc;
+            if (!euler) vc += 0.5 * dt * Fc;
             v[i] = vc;
-            q[i] += dt * vc;
+            q[i] += (euler ? sc->dt_prev : dt) * vc;
         }
     }
 }
@@ -205,11 +205,12 @@ template <bool THREE>
 __global__ void __launch_bounds__(BX * BY) k_fire1_force(LqGeom g, LqPhys ph, LqFields f,
                                                          const double *__restrict__ q, double *__restrict__ v,
                                                          double *__restrict__ F, const LqFireScalars *__restrict__ sc,
-                                                         double *__restrict__ partials) {
+                                                         double *__restrict__ partials, long long euler_max) {
     if (sc->converged) return;
     const int x = blockIdx.x * BX + threadIdx.x;
     const int y = blockIdx.y * BY + threadIdx.y;
-    const double hdt = 0.5 * sc->dt;
+    // velocity Verlet: second half kick; Euler variant: the full kick of the next step, none once the budget is spent
+    const double hdt = euler_max < 0 ? 0.5 * sc->dt : (sc->step < euler_max ? sc->dt : 0.0);
     double r[4] = {0, 0, 0, 0};
     if (x < g.Lx && y < g.Ly) {
         for (int z = blockIdx.z * ZPER; z < min(g.Lz, (int)(blockIdx.z + 1) * ZPER); ++z) {
@@ -254,7 +255,8 @@ __global__ void __launch_bounds__(256) k_fire_update(const double *__restrict__ 
     __syncthreads();
     if (threadIdx.x != 0) return;
     LqFireScalars t = *sc;
-    lq_fire_advance(t, fc, tot, first);
+    if (first == 2) lq_fire_advance_euler(t, fc, tot);
+    else lq_fire_advance(t, fc, tot, first);
     *sc = t;
 }
 
@@ -336,15 +338,16 @@ void lq_launch_energy(const LqGeom &g, const LqPhys &ph, const LqFields &f, cons
 }
 int lq_fire1_num_blocks(const LqGeom &g) { return lq_energy_num_blocks(g); }
 void lq_launch_fire1_drift(const LqGeom &g, const LqFields &f, double *q, double *v, const double *F,
-                           const LqFireScalars *sc, cudaStream_t st) {
-    k_fire1_drift<<<site_grid(g), dim3(BX, BY), 0, st>>>(g, f, q, v, F, sc);
+                           const LqFireScalars *sc, cudaStream_t st, int euler) {
+    k_fire1_drift<<<site_grid(g), dim3(BX, BY), 0, st>>>(g, f, q, v, F, sc, euler);
 }
 void lq_launch_fire1_force(const LqGeom &g, const LqPhys &ph, const LqFields &f, const double *q, double *v,
-                           double *F, const LqFireScalars *sc, double *partials, cudaStream_t st) {
+                           double *F, const LqFireScalars *sc, double *partials, cudaStream_t st,
+                           long long euler_max) {
     if (lq_three(ph))
-        k_fire1_force<true><<<site_grid(g), dim3(BX, BY), 0, st>>>(g, ph, f, q, v, F, sc, partials);
+        k_fire1_force<true><<<site_grid(g), dim3(BX, BY), 0, st>>>(g, ph, f, q, v, F, sc, partials, euler_max);
     else
-        k_fire1_force<false><<<site_grid(g), dim3(BX, BY), 0, st>>>(g, ph, f, q, v, F, sc, partials);
+        k_fire1_force<false><<<site_grid(g), dim3(BX, BY), 0, st>>>(g, ph, f, q, v, F, sc, partials, euler_max);
 }
 void lq_launch_fire_update(const double *partials, int nblocks, LqFireScalars *sc, LqFireConsts fc, int first,
                            cudaStream_t st) {

@@ -83,3 +83,64 @@ def test_converges_to_uniform_ground_state_and_lowers_energy(oracle_mod):
     assert rep["converged"] == 1
     assert abs(rep["energy"] - N * f0) < 1e-10 * abs(N * f0)
     assert rep["energy"] < o.energy(q, 1)
+
+
+# ------------------------------------------------------------------ GPU parity
+import pytest
+
+
+@pytest.fixture(scope="module")
+def lq():
+    import torch
+    assert torch.cuda.is_available(), "gpu tests need a CUDA device"
+    from paper_1911_07045_b200 import binding, build
+    build.build()
+    binding.load()
+    return binding
+
+
+GPU_CASES = {
+    "masked_37x21x11": lambda: wl.random_masked_problem(103, 37, 21, 11, obj_frac=0.15),
+    "masked_70x35x9_L1only": lambda: wl.random_masked_problem(104, 70, 35, 9, obj_frac=0.1, L2=0.0, L3=0.0),
+    "replica3": lambda: wl.make_replica("3"),
+    "replica4": lambda: wl.make_replica("4"),
+    "replica5p": lambda: wl.make_replica("5p"),
+}
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("name", sorted(GPU_CASES))
+def test_gpu_euler_fire_matches_oracle(lq, oracle_mod, name):
+    """Q after exactly 100 steps max-abs 1e-8; dt, alpha, steps exact; Fmax / Frms / P / energy rel 1e-9"""
+    c = GPU_CASES[name]()
+    o = oracle_mod.Oracle(c["Lx"], c["Ly"], c["Lz"], c["A"], c["B"], c["C"], c["L1"], c["L2"], c["L3"], mask=c["mask"],
+                          kind=c["kind"], W=c["W"], axis=c["axis"])
+    fp = dict(c["fire"], integrator=1)
+    ctx = lq.create_from_config(c)
+    for K in (1, 100):
+        lq.lq_set_Q(ctx, np.ascontiguousarray(c["q"]))
+        rep = lq.lq_fire_minimize(ctx, K, 0.0, fp, report_energy=True)
+        qref, rref = o.fire(c["q"], K, 0.0, fp, variant=1)
+        assert rep["steps"] == K and rep["converged"] == 0
+        assert np.abs(lq.lq_get_Q(ctx) - qref).max() <= 1e-8
+        assert rep["dt"] == rref["dt"] and abs(rep["alpha"] - rref["alpha"]) <= 1e-15
+        for key in ("Fmax", "Frms", "P", "energy"):
+            assert abs(rep[key] - rref[key]) <= 1e-9 * abs(rref[key]), key
+    lq.lq_destroy(ctx)
+
+
+@pytest.mark.gpu
+def test_gpu_euler_fire_stop_rule_and_convergence(lq, oracle_mod):
+    c = wl.bulk_quench(12, 5)
+    fp = dict(c["fire"], integrator=1)
+    o = oracle_mod.Oracle(c["Lx"], c["Ly"], c["Lz"], c["A"], c["B"], c["C"], c["L1"])
+    ctx = lq.create_from_config(c)
+    rep = lq.lq_fire_minimize(ctx, 50, 1e9, fp)
+    assert rep["steps"] == 0 and rep["converged"] == 1
+    assert np.array_equal(lq.lq_get_Q(ctx), np.asarray(c["q"]).reshape(lq.lq_get_Q(ctx).shape))
+    rep = lq.lq_fire_minimize(ctx, 20000, 1e-9, fp, report_energy=True)
+    qref, rref = o.fire(c["q"], 20000, 1e-9, fp, variant=1)
+    assert rep["converged"] == 1 and rref["converged"] == 1
+    assert abs(rep["steps"] - rref["steps"]) <= 2
+    assert abs(rep["energy"] - rref["energy"]) <= 1e-6 * abs(rref["energy"])
+    lq.lq_destroy(ctx)

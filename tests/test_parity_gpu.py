@@ -184,7 +184,7 @@ def test_edge_cases(lq, oracle_mod):
     rep = lq.lq_fire_minimize(ctx, 10, 1e-9, fire)
     assert rep["converged"] == 1 and rep["steps"] == 0 and np.array_equal(lq.lq_get_Q(ctx), qu)
     # bad parameters
-    for bad in (dict(fire, dt0=0.0), dict(fire, dtmax=0.001), dict(fire, falpha=1.5), dict(fire, integrator=1)):
+    for bad in (dict(fire, dt0=0.0), dict(fire, dtmax=0.001), dict(fire, falpha=1.5), dict(fire, integrator=2)):
         with pytest.raises(lq.LqError) as ei:
             lq.lq_fire_minimize(ctx, 1, 0.0, bad)
         assert ei.value.code == lq.LQ_ERR_ARG

@@ -16,7 +16,7 @@ struct SweepArgs {
     double *partials;
     unsigned int *counter;
     int zc;
-    int store_cs;
+    int store_cs;           // stored-force sweep: 1 = streaming (evict-first) stores of the outputs (LQ_STORE_CS; measured neutral)
     const uint8_t *plain;   // per-site 'constant stencil weights' byte (masked lattices)
     const uint8_t *tsum;    // per (plane, tile): tile + halo all plain
     const double *Fi;       // masked recompute sweep: stored force of the NON-plain sites (input buffer)

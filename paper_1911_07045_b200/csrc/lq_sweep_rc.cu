@@ -160,7 +160,7 @@ k_sweep_rc(const __grid_constant__ CUtensorMap tq, const __grid_constant__ CUten
 #pragma unroll
             for (int c = 0; c < 5; ++c) rn[c * RC::PLANE + idx] = qp[c];
         }
-        if (hx >= 0 && !(a.store_cs & 1)) {
+        if (hx >= 0) {
             double vk[5], qn[5];
             first(hx, hy, pbh, vk, qn);
             const int idx = hy * RC::BXW + hx;

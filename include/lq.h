@@ -174,6 +174,7 @@ int lq_set_cubic(lq_ctx *ctx, double L6);
  * One kernel launch per step.  The stop test max|F_a(y_k)| < force_tol uses the force the step evaluates and
  * the step's update is still applied, so steps = updates applied (force_tol = 0: exactly max_steps).
  * The report reuses lq_fire_report: Fmax, Frms of F(y_k) of the last step; P = 0; dt = eta; alpha = mu.
+ * lq_get_velocity returns zeros afterwards (these minimisers carry no velocity).
  * Errors: LQ_ERR_STATE before lq_set_Q; LQ_ERR_ARG on eta <= 0, mu outside [0, 1), unknown method,
  * max_steps < 0, NULL pointers. */
 enum { LQ_MIN_GD = 0, LQ_MIN_NESTEROV = 1 };

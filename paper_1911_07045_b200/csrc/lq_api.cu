@@ -544,6 +544,9 @@ int lq_descent_minimize(lq_ctx *c, int method, long max_steps, double force_tol,
     // make the buffer that holds the last iterate the live one
     if (fin == 1) c->cur ^= 1;
     else if (fin == 2) { double *t = c->q[c->cur]; c->q[c->cur] = c->v[0]; c->v[0] = t; }
+    // these minimisers carry no velocity; the velocity storage may have served as their third buffer
+    for (int i = 0; i < 2; ++i)
+        if (c->v[i]) LQ_CUDA(c, cudaMemsetAsync(c->v[i], 0, (size_t)5 * g.NP * sizeof(double), st));
     const double nsim = (double)(c->flags_active ? c->n_class[0] + c->n_class[1] : (unsigned long long)g.N);
     out->steps = (long)h.step; out->converged = h.converged;
     out->Fmax = h.Fmax; out->Frms = nsim > 0 ? sqrt(h.FF / nsim) : 0.0;

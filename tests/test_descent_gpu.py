@@ -105,6 +105,7 @@ def test_stop_convention_and_chaining(lq, oracle_mod):
     ctx = lq.create_from_config(c)
     rep = lq.lq_descent_minimize(ctx, 1, 50, 1e9, ETA, MU)
     assert rep["steps"] == 1 and rep["converged"] == 1
+    assert not lq.lq_get_velocity(ctx).any()           # no velocity is carried (the storage served as a buffer)
     q1ref, _ = o.descent(c["q"], 1, 1, 0.0, ETA, MU)
     assert np.abs(lq.lq_get_Q(ctx) - q1ref).max() <= 1e-13
     lq.lq_set_Q(ctx, np.ascontiguousarray(c["q"]))

@@ -159,8 +159,8 @@ int lq_set_chiral(lq_ctx *ctx, double L4);
 /* Cubic distortion constant L6 of Eq. 10: adds L6/2 Q_lk dQ_ij/dx_l dQ_ij/dx_k (in the uniaxial
  * limit L6 = (4 / 27 S^3)(K3 - K1): it separates bend from splay).  Discretised like L1..L3: same-axis
  * products average to the mean of the squared one-sided differences, different-axis products to products of the
- * mean differences; the weight Q_lk is the site's own tensor.  With L6 != 0 every minimiser runs the general
- * one-thread-per-site kernels (the fused sweeps' constant-weight stencils do not carry the term yet).  Errors as
+ * mean differences; the weight Q_lk is the site's own tensor.  Routed like lq_set_chiral (19-point sweeps with the
+ * term compiled in; those instantiations spill registers, so expect about a third of the L6 = 0 rate).  Errors as
  * lq_set_chiral. */
 int lq_set_cubic(lq_ctx *ctx, double L6);
 

@@ -217,7 +217,8 @@ struct DS {
 
 // THREE: L2/L3 != 0 -- the 19-point constant-weight stencil (lqs::bulk_force_threeconst) reads planes k-1, k, k+1
 // from the ring (three live slots instead of two).
-template <bool NEST, bool MASKED, bool THREE, bool CHIRAL, int NS>
+// XT: extra distortion terms in the 19-point stencil (bit 0 chiral L4, bit 1 cubic L6)
+template <bool NEST, bool MASKED, bool THREE, int XT, int NS>
 __global__ void __launch_bounds__(512, 1)
 k_descent_sweep(const __grid_constant__ CUtensorMap tq, const __grid_constant__ CUtensorMap tp, const DescArgs a,
                 const uint8_t *__restrict__ plain, int zc) {
@@ -289,7 +290,7 @@ k_descent_sweep(const __grid_constant__ CUtensorMap tq, const __grid_constant__ 
                         if (dz != 0 && dx == 0 && dy == 0) return dz < 0 ? ym[c] : yn[c];
                         return Y(dz < 0 ? sa : (dz > 0 ? sj : sb), c, dy * C::SW + dx);
                     };
-                    lqs::bulk_force_threeconst<CHIRAL>(a.ph, get, yc, F);
+                    lqs::bulk_force_threeconst<(XT & 1) != 0, (XT & 2) != 0>(a.ph, get, yc, F);
                 }
 #pragma unroll
                 for (int c = 0; c < 5; ++c) {
@@ -332,7 +333,7 @@ struct LqDescentPlan {
     int n_list = 0;
     const uint8_t *flags_seen = nullptr;
     bool sites_dirty = true;
-    bool attr_set[16] = {};
+    bool attr_set[32] = {};
 };
 
 void lq_descent_destroy(LqDescentPlan *p) {
@@ -351,25 +352,28 @@ void lq_descent_invalidate(LqDescentPlan *p) {
 namespace {
 constexpr int NS_GD = 6, NS_NEST = 4;   // ring depth: 6 x 25.4 KB (GD), 4 x 50.8 KB (Nesterov)
 
-template <bool NEST, bool MASKED, bool THREE, bool CHIRAL = false>
+template <bool NEST, bool MASKED, bool THREE, int XT = 0>
 cudaError_t launch_sweep_t(LqDescentPlan *pl, dim3 grid, const CUtensorMap &mq, const CUtensorMap &mp, const DescArgs &a,
                            int zc, cudaStream_t st) {
     constexpr int NS = NEST ? NS_NEST : NS_GD;
     using C = DS<NEST, NS>;
-    const int v = (CHIRAL ? 8 : 0) + (THREE ? 4 : 0) + (NEST ? 2 : 0) + (MASKED ? 1 : 0);
+    const int v = 8 * XT + (THREE ? 4 : 0) + (NEST ? 2 : 0) + (MASKED ? 1 : 0);
     if (!pl->attr_set[v]) {
-        cudaError_t e = cudaFuncSetAttribute(k_descent_sweep<NEST, MASKED, THREE, CHIRAL, NS>,
+        cudaError_t e = cudaFuncSetAttribute(k_descent_sweep<NEST, MASKED, THREE, XT, NS>,
                                              cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES);
         if (e != cudaSuccess) return e;
         pl->attr_set[v] = true;
     }
-    k_descent_sweep<NEST, MASKED, THREE, CHIRAL, NS><<<grid, C::NT, C::SMEM_BYTES, st>>>(mq, mp, a, pl->plain, zc);
+    k_descent_sweep<NEST, MASKED, THREE, XT, NS><<<grid, C::NT, C::SMEM_BYTES, st>>>(mq, mp, a, pl->plain, zc);
     return cudaGetLastError();
 }
 template <bool NEST, bool MASKED>
 cudaError_t launch_sweep(bool three, LqDescentPlan *pl, dim3 grid, const CUtensorMap &mq, const CUtensorMap &mp,
                          const DescArgs &a, int zc, cudaStream_t st) {
-    if (three && a.ph.L4 != 0.0) return launch_sweep_t<NEST, MASKED, true, true>(pl, grid, mq, mp, a, zc, st);
+    const int xt = (a.ph.L4 != 0.0 ? 1 : 0) | (a.ph.L6 != 0.0 ? 2 : 0);
+    if (three && xt == 1) return launch_sweep_t<NEST, MASKED, true, 1>(pl, grid, mq, mp, a, zc, st);
+    if (three && xt == 2) return launch_sweep_t<NEST, MASKED, true, 2>(pl, grid, mq, mp, a, zc, st);
+    if (three && xt == 3) return launch_sweep_t<NEST, MASKED, true, 3>(pl, grid, mq, mp, a, zc, st);
     return three ? launch_sweep_t<NEST, MASKED, true>(pl, grid, mq, mp, a, zc, st)
                  : launch_sweep_t<NEST, MASKED, false>(pl, grid, mq, mp, a, zc, st);
 }

@@ -37,7 +37,7 @@ struct LqPhys {
 // the 19-point / general mixed-derivative code paths are needed as soon as any of L2, L3, L4 is non-zero
 __host__ __device__ inline bool lq_three(const LqPhys &ph) { return ph.L2 != 0.0 || ph.L3 != 0.0 || ph.L4 != 0.0 || ph.L6 != 0.0; }
 // terms the fused sweeps' constant-weight stencils do not carry: such runs use the general kernels
-__host__ __device__ inline bool lq_general_only(const LqPhys &ph) { return ph.L6 != 0.0; }
+__host__ __device__ inline bool lq_general_only(const LqPhys &) { return false; }
 
 // FIRE state that lives on the device (Algorithm 1).
 // mix_a, mix_b: the velocity rescale of the step just reduced, v <- mix_a*v + mix_b*F

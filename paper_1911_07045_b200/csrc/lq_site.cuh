@@ -345,7 +345,12 @@ __device__ __forceinline__ void bulk_force_oneconst(const LqPhys &ph, const doub
 // CHIRAL: also the L4 term on constant weights, G_ab += L4 eps_aik C_k Q_ib with centred differences C_k (the
 // gather form of lqs::site_force at a site whose weights are all 1/2) -- a template flag so
 // that the achiral instantiations keep their register budget.
-template <bool CHIRAL = false, class Get>
+// CUBIC: the L6 term on constant weights (all w = 1/2), from the same gather form:
+//   bonds      G_ab -= L6/2 [Q_kk(x) + Q_kk(x + s k)] (Q_ab(x + s k) - Q_ab(x))            for the six neighbours
+//   own factor G_kk += L6/4 sum_s |Q(x + s k) - Q(x)|^2 ;  G_ab += L6/2 C_a Q : C_b Q  (a != b)
+//   mixed      G_ab += sum_c 1/2 [H_c(x - c) - H_c(x + c)]_ab ,  H_c(y) = L6 sum_{l != c} Q_lc(y) C_l Q(y)
+// with C_l the centred difference; the edge neighbours x +- c +- l enter through C_l Q(x +- c).
+template <bool CHIRAL = false, bool CUBIC = false, class Get>
 __device__ __forceinline__ void bulk_force_threeconst(const LqPhys &ph, const Get &g, const double qc[5], double F[5]) {
     const double L1 = ph.L1, L23 = ph.L2 + ph.L3;
     auto d2 = [&](int c, int ax) -> double {
@@ -416,6 +421,63 @@ __device__ __forceinline__ void bulk_force_threeconst(const LqPhys &ph, const Ge
         }
         F[0] -= G4[0][0] - G4[2][2]; F[1] -= G4[0][1] + G4[1][0]; F[2] -= G4[0][2] + G4[2][0];
         F[3] -= G4[1][1] - G4[2][2]; F[4] -= G4[1][2] + G4[2][1];
+    }
+    if (CUBIC) {
+        auto T6 = [&](int dx, int dy, int dz, double o[6]) {     // full tensor at an offset
+#pragma unroll
+            for (int c = 0; c < 5; ++c) o[c] = g(c, dx, dy, dz);
+            o[5] = -o[0] - o[3];
+        };
+        const double Q0[6] = {qc[0], qc[1], qc[2], qc[3], qc[4], -qc[0] - qc[3]};
+        double G6[3][3] = {{0.0, 0.0, 0.0}, {0.0, 0.0, 0.0}, {0.0, 0.0, 0.0}};
+        double Cx[3][6];                                         // C_k Q at the site itself
+#pragma unroll
+        for (int k = 0; k < 3; ++k) {
+            const int ex = k == 0, ey = k == 1, ez = k == 2;
+            const int m1 = (k + 1) % 3, m2 = (k + 2) % 3;
+            double Qp[6], Qm[6];
+            T6(ex, ey, ez, Qp);
+            T6(-ex, -ey, -ez, Qm);
+            double dp[6], dm[6];
+#pragma unroll
+            for (int i = 0; i < 6; ++i) { dp[i] = Qp[i] - Q0[i]; dm[i] = Qm[i] - Q0[i]; Cx[k][i] = 0.5 * (Qp[i] - Qm[i]); }
+            const double wp = 0.5 * ph.L6 * (Q0[m6(k, k)] + Qp[m6(k, k)]), wm = 0.5 * ph.L6 * (Q0[m6(k, k)] + Qm[m6(k, k)]);
+#pragma unroll
+            for (int a = 0; a < 3; ++a)
+#pragma unroll
+                for (int b = 0; b < 3; ++b) G6[a][b] -= wp * dp[m6(a, b)] + wm * dm[m6(a, b)];
+            G6[k][k] += 0.25 * ph.L6 * (frodot(dp, dp) + frodot(dm, dm));
+            // mixed part: y = x + s k, l in {m1, m2}
+#pragma unroll
+            for (int s = -1; s <= 1; s += 2) {
+                const double *Qy = s > 0 ? Qp : Qm;
+                double H[6] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
+#pragma unroll
+                for (int t = 0; t < 2; ++t) {
+                    const int l = t == 0 ? m1 : m2;
+                    const int lx = l == 0, ly = l == 1, lz = l == 2;
+                    double A[6], Bm[6];
+                    T6(s * ex + lx, s * ey + ly, s * ez + lz, A);
+                    T6(s * ex - lx, s * ey - ly, s * ez - lz, Bm);
+                    const double wl = ph.L6 * Qy[m6(l, k)] * 0.5;
+#pragma unroll
+                    for (int i = 0; i < 6; ++i) H[i] += wl * (A[i] - Bm[i]);
+                }
+                // 1/2 [H(x - k) - H(x + k)]
+#pragma unroll
+                for (int a = 0; a < 3; ++a)
+#pragma unroll
+                    for (int b = 0; b < 3; ++b) G6[a][b] += (s > 0 ? -0.5 : 0.5) * H[m6(a, b)];
+            }
+        }
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+            const int a1 = (a + 1) % 3, a2 = (a + 2) % 3;
+            G6[a][a1] += 0.5 * ph.L6 * frodot(Cx[a], Cx[a1]);
+            G6[a][a2] += 0.5 * ph.L6 * frodot(Cx[a], Cx[a2]);
+        }
+        F[0] -= G6[0][0] - G6[2][2]; F[1] -= G6[0][1] + G6[1][0]; F[2] -= G6[0][2] + G6[2][0];
+        F[3] -= G6[1][1] - G6[2][2]; F[4] -= G6[1][2] + G6[2][1];
     }
 }
 

@@ -54,7 +54,8 @@ struct Cfg {
     static constexpr int NHALO = 2 * BXW + 2 * (BYH - 2);
 };
 
-template <class C, bool THREE, bool MASKED, bool CHIRAL>
+// XT: extra distortion terms compiled into the 19-point stencil (bit 0 chiral L4, bit 1 cubic L6)
+template <class C, bool THREE, bool MASKED, int XT>
 __global__ void __launch_bounds__(C::NT, 1)
 k_sweep(const __grid_constant__ CUtensorMap tq, const __grid_constant__ CUtensorMap tv,
         const __grid_constant__ CUtensorMap tF, const SweepArgs a) {
@@ -175,7 +176,7 @@ k_sweep(const __grid_constant__ CUtensorMap tq, const __grid_constant__ CUtensor
                             if (dx == 0 && dy == 0) return dz < 0 ? qm[c] : qp[c];
                             return (dz < 0 ? rkm : rn)[c * C::PLANE + idx + dy * C::BXW + dx];
                         };
-                        lqs::bulk_force_threeconst<CHIRAL>(a.ph, get, qc, Fn);
+                        lqs::bulk_force_threeconst<(XT & 1) != 0, (XT & 2) != 0>(a.ph, get, qc, Fn);
                     }
 #pragma unroll
                     for (int c = 0; c < 5; ++c) {
@@ -283,7 +284,7 @@ struct LqSweepPlan {
     bool sites_dirty = true;
     dim3 grid;
     int zc = 0;
-    bool attr_set[6] = {false, false, false, false, false, false};
+    bool attr_set[12] = {};
 };
 
 void lq_sweep_destroy(LqSweepPlan *p) {
@@ -301,15 +302,15 @@ void lq_sweep_invalidate(LqSweepPlan *p) {
     if (p) p->sites_dirty = true;
 }
 
-template <class C, bool THREE, bool MASKED, bool CHIRAL = false>
+template <class C, bool THREE, bool MASKED, int XT = 0>
 static cudaError_t launch(LqSweepPlan *pl, int in, const SweepArgs &a, int variant, cudaStream_t st) {
     if (!pl->attr_set[variant]) {
-        cudaError_t e = cudaFuncSetAttribute(k_sweep<C, THREE, MASKED, CHIRAL>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+        cudaError_t e = cudaFuncSetAttribute(k_sweep<C, THREE, MASKED, XT>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                              C::SMEM_BYTES);
         if (e != cudaSuccess) return e;
         pl->attr_set[variant] = true;
     }
-    k_sweep<C, THREE, MASKED, CHIRAL><<<pl->grid, C::NT, C::SMEM_BYTES, st>>>(pl->mq[in], pl->mv[in], pl->mF[in], a);
+    k_sweep<C, THREE, MASKED, XT><<<pl->grid, C::NT, C::SMEM_BYTES, st>>>(pl->mq[in], pl->mv[in], pl->mF[in], a);
     return cudaGetLastError();
 }
 
@@ -410,8 +411,12 @@ int lq_sweep_run(LqSweepPlan **planp, bool stored_F, const LqGeom &g, const LqPh
             const int in = (int)((cur0 + done + i) & 1), out = in ^ 1;
             a.qo = q[out]; a.vo = v[out]; a.Fo = F[out]; a.Fi = F[in];
             if (!stored_F) e = lq_launch_sweep_rc(masked, pl->grid, pl->mq[in], pl->mv[in], a, st);
-            else if (three && ph.L4 != 0.0)
-                e = masked ? launch<C3, true, true, true>(pl, in, a, 5, st) : launch<C3, true, false, true>(pl, in, a, 4, st);
+            else if (three && (ph.L4 != 0.0 || ph.L6 != 0.0)) {
+                const int xt = (ph.L4 != 0.0 ? 1 : 0) | (ph.L6 != 0.0 ? 2 : 0);
+                if (xt == 1) e = masked ? launch<C3, true, true, 1>(pl, in, a, 5, st) : launch<C3, true, false, 1>(pl, in, a, 4, st);
+                else if (xt == 2) e = masked ? launch<C3, true, true, 2>(pl, in, a, 7, st) : launch<C3, true, false, 2>(pl, in, a, 6, st);
+                else e = masked ? launch<C3, true, true, 3>(pl, in, a, 9, st) : launch<C3, true, false, 3>(pl, in, a, 8, st);
+            }
             else if (three) e = masked ? launch<C3, true, true>(pl, in, a, 3, st) : launch<C3, true, false>(pl, in, a, 2, st);
             else e = masked ? launch<C1, false, true>(pl, in, a, 1, st) : launch<C1, false, false>(pl, in, a, 0, st);
             if (e == cudaSuccess && masked)

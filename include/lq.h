@@ -104,7 +104,7 @@ int lq_forces(lq_ctx *ctx, double *F, int where);
 /* FIRE parameters (Algorithm 1).  integrator 0 = velocity Verlet as kick-drift-kick
  * (R4; the fused sweeps), 1 = plain semi-implicit Euler (R30): per step
  * v += dt F(q); P, |F|^2, |v|^2; mix; schedule; q += dt v (the step's dt, the mixed or reset v); then the new force
- * and the stop test -- one force evaluation per step, run on the general four-launch path.  report_energy != 0 fills lq_fire_report.energy (one extra pass). */
+ * and the stop test.  Both run on the fused sweeps (the lazily applied part of a step only changes coefficients).  report_energy != 0 fills lq_fire_report.energy (one extra pass). */
 typedef struct {
     double dt0, dtmax, alpha0, finc, fdec, falpha;
     int Nmin;

@@ -361,7 +361,7 @@ int lq_fire_minimize(lq_ctx *c, long max_steps, double force_tol, const lq_fire_
     // the fused sweeps' constant-weight stencils do not carry the chiral term: L4 != 0 runs the general kernels
     // ... and so does the semi-implicit Euler variant (integrator = 1)
     const bool euler = fp->integrator == 1;
-    const bool fused = c->fire_path != 1 && !lq_general_only(c->ph) && !euler;
+    const bool fused = c->fire_path != 1 && !lq_general_only(c->ph);
     const bool three = lq_three(c->ph);
     const bool stored_F = three || c->fire_path == 2;   // recompute-F sweep: one-constant only
     if (fused) {
@@ -372,7 +372,8 @@ int lq_fire_minimize(lq_ctx *c, long max_steps, double force_tol, const lq_fire_
     const int nb1 = lq_fire1_num_blocks(g);
     if ((rc = ensure_partials(c, (size_t)4 * nb1)) != LQ_OK) return rc;
 
-    LqFireConsts fc{fp->dt0, fp->dtmax, fp->alpha0, fp->finc, fp->fdec, fp->falpha, force_tol, fp->Nmin, (long long)max_steps};
+    LqFireConsts fc{fp->dt0, fp->dtmax, fp->alpha0, fp->finc, fp->fdec, fp->falpha, force_tol, fp->Nmin, (long long)max_steps,
+                    fp->integrator == 1 ? 1 : 0};
     LqFireScalars h;
     memset(&h, 0, sizeof(h));
     h.dt = euler ? fp->dt0 : 0.0; h.alpha = fp->alpha0; h.mix_a = 1.0; h.mix_b = 0.0;

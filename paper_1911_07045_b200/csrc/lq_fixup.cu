@@ -45,7 +45,7 @@ __global__ void __launch_bounds__(FB, LQ_FIX_MINB) k_fixup(const FixArgs a) {
     if (sc.converged) return;
     const int i = blockIdx.x * FB + threadIdx.x;
     const long long NP = a.g.NP;
-    const double hdt = 0.5 * sc.dt;
+    const double hdt = lq_step_coef(sc, a.fc).kick;
     double r[4] = {0.0, 0.0, 0.0, 0.0};
     if (i < a.n) {
         const long long p = a.list[i];
@@ -128,7 +128,7 @@ __global__ void __launch_bounds__(FB, LQ_FIX_MINB) k_fixup(const FixArgs a) {
             for (int w = 1; w < NW; ++w) tot[k] = k < 3 ? tot[k] + red[k * NW + w] : fmax(tot[k], red[k * NW + w]);
         }
         LqFireScalars nx = sc;
-        lq_fire_advance(nx, a.fc, tot, 0);
+        lq_fire_advance_any(nx, a.fc, tot);
         *a.sc = nx;
         *a.counter = 0u;
     }

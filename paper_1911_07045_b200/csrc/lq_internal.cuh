@@ -57,6 +57,7 @@ struct LqFireConsts {
     double dt0, dtmax, alpha0, finc, fdec, falpha, force_tol;
     int Nmin;
     long long max_steps;
+    int euler;  // 1: FIRE on the semi-implicit Euler step (integrator = 1), 0: velocity Verlet
 };
 
 // Reductions of one step -> schedule of the next (Algorithm 1; readings
@@ -98,6 +99,23 @@ __host__ __device__ inline void lq_fire_advance_euler(LqFireScalars &t, const Lq
     } else {
         t.npos = 0; t.dt *= fc.fdec; t.alpha = fc.alpha0; t.mix_a = 0.0; t.mix_b = 0.0;
     }
+}
+
+// The three coefficients a fused step needs, for either integrator (the lazily applied part of the previous step
+// plus this step's kick):  v_k = ma vc + cF F ;  q' = q + dt v_k ;  vc' = v_k + kick F'.
+//   velocity Verlet: dt = sc.dt, cF = mix_b + dt/2, kick = dt/2
+//   Euler variant:   dt = sc.dt_prev (the scheduled step's own dt), cF = mix_b, kick = sc.dt while the budget lasts
+struct LqStepCoef { double dt, ma, cF, kick; };
+__host__ __device__ inline LqStepCoef lq_step_coef(const LqFireScalars &sc, const LqFireConsts &fc) {
+    LqStepCoef k;
+    k.ma = sc.mix_a;
+    if (fc.euler) { k.dt = sc.dt_prev; k.cF = sc.mix_b; k.kick = sc.step < fc.max_steps ? sc.dt : 0.0; }
+    else { k.dt = sc.dt; k.cF = sc.mix_b + 0.5 * sc.dt; k.kick = 0.5 * sc.dt; }
+    return k;
+}
+__host__ __device__ inline void lq_fire_advance_any(LqFireScalars &t, const LqFireConsts &fc, const double tot[4]) {
+    if (fc.euler) lq_fire_advance_euler(t, fc, tot);
+    else lq_fire_advance(t, fc, tot, 0);
 }
 
 struct LqFields {

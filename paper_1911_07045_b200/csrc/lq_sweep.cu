@@ -99,7 +99,8 @@ k_sweep(const __grid_constant__ CUtensorMap tq, const __grid_constant__ CUtensor
         if (nplanes > 1) issue(1);
     }
 
-    const double dt = sc.dt, ma = sc.mix_a, cF = sc.mix_b + 0.5 * sc.dt, hdt = 0.5 * sc.dt;
+    const LqStepCoef kc = lq_step_coef(sc, a.fc);
+    const double dt = kc.dt, ma = kc.ma, cF = kc.cF, hdt = kc.kick;
     double qm[5], qc[5], qp[5], vk0[5], vk1[5];
 #pragma unroll
     for (int c = 0; c < 5; ++c) qm[c] = qc[c] = qp[c] = vk0[c] = vk1[c] = 0.0;
@@ -393,6 +394,10 @@ int lq_sweep_run(LqSweepPlan **planp, bool stored_F, const LqGeom &g, const LqPh
     if (e != cudaSuccess) { err = cudaGetErrorString(e); return LQ_ERR_CUDA; }
     if (stored_F || masked) {   // F of the entry state was written by the generic kernel without its ghost shell
         lq_launch_fill_ghosts_f64(g, F[*cur], 5, st);
+        *launches += 1;
+    }
+    if (fc.euler) {             // Euler variant: the entry velocity already carries the first kick (interior only)
+        lq_launch_fill_ghosts_f64(g, v[*cur], 5, st);
         *launches += 1;
     }
 

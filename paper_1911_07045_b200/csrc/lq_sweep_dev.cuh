@@ -129,7 +129,7 @@ __device__ __forceinline__ void finish_step(const SweepArgs &a, const LqFireScal
             for (int w = 1; w < NW; ++w) tot[i] = i < 3 ? tot[i] + red[i * NW + w] : fmax(tot[i], red[i * NW + w]);
         }
         LqFireScalars nx = sc;
-        lq_fire_advance(nx, a.fc, tot, 0);
+        lq_fire_advance_any(nx, a.fc, tot);
         *a.sc = nx;
         *a.counter = 0u;
     }

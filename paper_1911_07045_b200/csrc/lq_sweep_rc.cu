@@ -79,7 +79,8 @@ k_sweep_rc(const __grid_constant__ CUtensorMap tq, const __grid_constant__ CUten
     if (tid == 0)
         for (int j = 0; j < 4 && j < nplanes; ++j) issue(j);
 
-    const double dt = sc.dt, ma = sc.mix_a, cF = sc.mix_b + 0.5 * sc.dt, hdt = 0.5 * sc.dt;
+    const LqStepCoef kc = lq_step_coef(sc, a.fc);
+    const double dt = kc.dt, ma = kc.ma, cF = kc.cF, hdt = kc.kick;
     double qm[5], qc[5], qp[5], vk0[5], vk1[5];
 #pragma unroll
     for (int c = 0; c < 5; ++c) qm[c] = qc[c] = qp[c] = vk0[c] = vk1[c] = 0.0;

@@ -109,15 +109,18 @@ GPU_CASES = {
 
 
 @pytest.mark.gpu
+@pytest.mark.parametrize("path", [0, 1, 2])
 @pytest.mark.parametrize("name", sorted(GPU_CASES))
-def test_gpu_euler_fire_matches_oracle(lq, oracle_mod, name):
-    """Q after exactly 100 steps max-abs 1e-8; dt, alpha, steps exact; Fmax / Frms / P / energy rel 1e-9"""
+def test_gpu_euler_fire_matches_oracle(lq, oracle_mod, name, path):
+    """Q after exactly 100 steps max-abs 1e-8; dt, alpha, steps exact; Fmax / Frms / P / energy rel 1e-9;
+    on the fused sweeps (path 0: default, 2: stored force) and on the four-launch general path (1)"""
     c = GPU_CASES[name]()
     o = oracle_mod.Oracle(c["Lx"], c["Ly"], c["Lz"], c["A"], c["B"], c["C"], c["L1"], c["L2"], c["L3"], mask=c["mask"],
                           kind=c["kind"], W=c["W"], axis=c["axis"])
     fp = dict(c["fire"], integrator=1)
     ctx = lq.create_from_config(c)
-    for K in (1, 100):
+    lq.lq_set_option(ctx, "fire_path", path)
+    for K in (1, 2, 100):
         lq.lq_set_Q(ctx, np.ascontiguousarray(c["q"]))
         rep = lq.lq_fire_minimize(ctx, K, 0.0, fp, report_energy=True)
         qref, rref = o.fire(c["q"], K, 0.0, fp, variant=1)

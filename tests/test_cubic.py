@@ -123,3 +123,36 @@ def test_gpu_parity_with_cubic_term(lq, oracle_mod, name, L4, L6):
     lq.lq_set_cubic(ctx, 0.0)
     assert np.array_equal(lq.lq_forces(ctx), F0)
     lq.lq_destroy(ctx)
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("name", ["masked_37x21x11", "replica3", "replica5p"])
+def test_gpu_everything_on(lq, oracle_mod, name):
+    """L1..L6, both external fields, anchoring and objects together; FIRE (both integrators), GD and Nesterov"""
+    c = GPU_CASES[name]()
+    Hf, chi, Ef, eps, L4, L6 = (0.3, -0.5, 0.8), 0.7, (0.6, 0.2, -0.4), -0.9, 0.35, -0.4
+    o = oracle_mod.Oracle(c["Lx"], c["Ly"], c["Lz"], c["A"], c["B"], c["C"], c["L1"], c["L2"], c["L3"], mask=c["mask"],
+                          kind=c["kind"], W=c["W"], axis=c["axis"], H=Hf, chi=chi, E=Ef, eps=eps, L4=L4, L6=L6)
+    ctx = lq.create_from_config(c)
+    lq.lq_set_field(ctx, Hf, chi, Ef, eps)
+    lq.lq_set_chiral(ctx, L4)
+    lq.lq_set_cubic(ctx, L6)
+    Fref = o.forces(c["q"], 1)
+    assert np.abs(lq.lq_forces(ctx) - Fref).max() <= 1e-10 * np.abs(Fref).max()
+    eref = o.energy(c["q"], 1)
+    assert abs(lq.lq_energy(ctx) - eref) <= 1e-9 * abs(eref)
+    for integ in (0, 1):
+        fp = dict(c["fire"], integrator=integ)
+        lq.lq_set_Q(ctx, np.ascontiguousarray(c["q"]))
+        lq.lq_fire_minimize(ctx, 30, 0.0, fp)
+        qref, _ = o.fire(c["q"], 30, 0.0, fp, variant=1)
+        assert np.abs(lq.lq_get_Q(ctx) - qref).max() <= 1e-8
+    for method in (0, 1):
+        lq.lq_set_Q(ctx, np.ascontiguousarray(c["q"]))
+        lq.lq_descent_minimize(ctx, method, 30, 0.0, 0.003, 0.8)
+        qd, _ = o.descent(c["q"], method, 30, 0.0, 0.003, 0.8)
+        assert np.abs(lq.lq_get_Q(ctx) - qd).max() <= 1e-8
+    a = lq.lq_analyze(ctx, 0.3)
+    Sref, _, _ = oracle_mod.analyze(lq.lq_get_Q(ctx), c["mask"], 0.3)
+    assert np.abs(a["S"] - Sref).max() <= 1e-10
+    lq.lq_destroy(ctx)

@@ -43,10 +43,11 @@
  * the printed L <-> K map on twist / splay / bend fields) of Eq. 10; the
  * director / S / defect analysis lives in lq_oracle.py (numpy.linalg.eigh;
  * tests/test_analyze.py: Eq. 2 and Eq. 3 round trips).
+ * The L2-vs-L3 split of Eq. 10 next to objects (tests/test_oracle_pins.py: hand-
+ * evaluated ramp fields where only L2 carries the cross product, and the wall
+ * surface sum that E(L2) - E(L3) reduces to by discrete summation by parts).
  * Parity UNPINNED: the FIRE / GD / Nesterov trajectories on the full-size
- * configs 3 and 5 (no published numbers) -- GPU-vs-oracle only; the L2-vs-L3
- * split of the ENERGY next to objects (only L2 + L3 is fixed by the continuum
- * pin; its gradient is pinned by finite differences).
+ * configs 3 and 5 (no published numbers) -- GPU-vs-oracle only.
  *
  * Layout: fields are SoA, q[c*N + s], c in (xx,xy,xz,yy,yz),
  * s = x + Lx*(y + Ly*z); Qzz = -Qxx-Qyy.  Index arithmetic is periodic in all
@@ -212,15 +213,16 @@ static void bulk_grad(const lqo_problem *p, const double Q[3][3], double G[3][3]
             G[a][b] = p->A * Q[b][a] + p->B * Q2[b][a] + p->C * tr2 * Q[b][a];
 }
 
-/* Anchoring energy of one boundary site (DESIGN.md R9: one term per boundary
- * site).  kind 1: Eq. 14, Q0 = (3/2) S0 (n n - I/3).
+/* Anchoring energy of one boundary site (DESIGN.md R9, SURVEY 8(c) O5: one term per boundary
+ * site, and only there: `boundary` = the site's class is boundary; kind set on a bulk site adds nothing).  kind 1: Eq. 14, Q0 = (3/2) S0 (n n - I/3).
  * kind 2: Eq. 15 with the garbled projection read as
  * Qt_perp = P Qt P (R2), Qt = Q + (S0/2) I, P = I - nu nu.
  * Returns the energy; if G != NULL also d/dQ_ab.                              */
-static double anchoring(const lqo_problem *p, long N, long s, const double Q[3][3], double G[3][3])
+static double anchoring(const lqo_problem *p, long N, long s, int boundary, const double Q[3][3], double G[3][3])
 {
     if (G) memset(G, 0, 9 * sizeof(double));
-    if (p->kind == NULL || p->kind[s] == 0) return 0.0;
+    /* SURVEY 8(c) O5 / DESIGN.md R9: a term only where class == boundary and kind != 0 */
+    if (!boundary || p->kind == NULL || p->kind[s] == 0) return 0.0;
     const double S0 = lqo_S0(p->A, p->B, p->C);
     const double W = p->W[s];
     const double n[3] = { p->axis[s], p->axis[N + s], p->axis[2 * N + s] };
@@ -273,6 +275,17 @@ static double anchoring(const lqo_problem *p, long N, long s, const double Q[3][
         }
     }
     return e;
+}
+
+/* boundary class (R8): a simulated site with at least one of its 6 face
+ * neighbours (periodic wrap) an object site */
+static int is_boundary_site(const lqo_problem *p, int x, int y, int z)
+{
+    if (!is_sim(p, site_of(p, x, y, z))) return 0;
+    for (int k = 0; k < 3; ++k)
+        for (int sg = +1; sg >= -1; sg -= 2)
+            if (!is_sim(p, nbr_of(p, x, y, z, k, sg))) return 1;
+    return 0;
 }
 
 /* allowed finite-difference signs per axis at a simulated site.
@@ -410,7 +423,7 @@ static double site_literal(const lqo_problem *p, const double *q, int x, int y, 
             }
 
     double Ga[3][3];
-    double ea = anchoring(p, N, s, Q, g ? Ga : NULL);
+    double ea = anchoring(p, N, s, is_boundary_site(p, x, y, z), Q, g ? Ga : NULL);
     if (g)
         for (int i = 0; i < 3; ++i)
             for (int j = 0; j < 3; ++j) G9[0][i][j] += Ga[i][j];
@@ -531,7 +544,7 @@ static double site_factorised(const lqo_problem *p, const double *q, int x, int 
 
     double eb = bulk_energy(p, Q) + field_energy(p, Q);      /* the "bulk" slot carries Eq. 13 too */
     double Ga[3][3];
-    double ea = anchoring(p, N, s, Q, g ? Ga : NULL);
+    double ea = anchoring(p, N, s, is_boundary_site(p, x, y, z), Q, g ? Ga : NULL);
 
     if (g) {
         double G9[7][3][3];

@@ -330,13 +330,129 @@ def test_anchoring_closed_forms(oracle_mod, variant):
             assert abs(terms[1]) < 1e-28             # uniform field
 
 
-def test_anchoring_ignored_off_boundary(oracle_mod):
-    """only boundary-class sites carry an anchoring term: kind on a bulk site still counts only
-    if the caller put it there -- the library's rule (DESIGN.md R9) is class==boundary && kind!=0;
-    the oracle takes kind as given, so workloads must only set kind on boundary sites."""
-    c = wl.make_replica("5")
-    f = make(oracle_mod, c).classify()
-    assert np.all((c["kind"] != 0) <= ((f & 3) == 1))
+@pytest.mark.parametrize("variant", [0, 1])
+def test_anchoring_only_on_boundary_class_sites(oracle_mod, variant):
+    """SURVEY 8(c) O5 / DESIGN.md R9: the anchoring term exists iff class == boundary and kind != 0.
+    kind / W / axis records on bulk and object sites must contribute nothing: energy (all three terms)
+    and forces are those of the same problem with the records stripped to the boundary sites, and the
+    anchoring energy equals the closed form of the boundary layer alone."""
+    S0 = oracle_mod.S0_of(A, B, Cc)
+    Lx, Ly, Lz = 5, 4, 6
+    N = Lx * Ly * Lz
+    mask = np.zeros((Lz, Ly, Lx), np.uint8)
+    mask[0] = 1                                        # wall: z = 1 and z = 5 are the boundary layers
+    rng = np.random.default_rng(17)
+    kind_all = rng.integers(1, 3, size=(Lz, Ly, Lx)).astype(np.uint8)       # 1 or 2 EVERYWHERE
+    W = rng.uniform(0.5, 2.0, N)
+    axis = rng.standard_normal((3, N))
+    axis /= np.linalg.norm(axis, axis=0)
+    q = 0.3 * rng.standard_normal((5, N))
+    bnd = np.zeros((Lz, Ly, Lx), bool)
+    bnd[1] = bnd[5] = True
+    kind_bnd = np.where(bnd, kind_all, 0).astype(np.uint8)
+    o_all = oracle_mod.Oracle(Lx, Ly, Lz, A, B, Cc, L1, 1.0, 0.5, mask=mask, kind=kind_all, W=W, axis=axis)
+    o_bnd = oracle_mod.Oracle(Lx, Ly, Lz, A, B, Cc, L1, 1.0, 0.5, mask=mask, kind=kind_bnd, W=W, axis=axis)
+    f = o_all.classify().reshape(Lz, Ly, Lx)
+    assert np.array_equal((f & 3) == 1, bnd)
+    e_all, t_all = o_all.energy(q, variant, terms=True)
+    e_bnd, t_bnd = o_bnd.energy(q, variant, terms=True)
+    assert e_all == e_bnd and np.array_equal(t_all, t_bnd)
+    assert np.array_equal(o_all.forces(q, variant), o_bnd.forces(q, variant))
+    # a bulk site and an object site with a record: no anchoring in the single-site energy
+    for (x, y, z) in ((2, 1, 3), (2, 1, 0)):
+        assert o_all.site_energy(q, x, y, z, variant)[1][2] == 0.0
+    # and the term that remains is the boundary layers' closed form (kind 1 everywhere there, uniform tilt)
+    theta = 0.7
+    n = np.array([np.sin(theta), 0.0, np.cos(theta)])
+    qu = wl.uniaxial_q(np.repeat(n[:, None], N, axis=1), 1.5 * S0)
+    ones = np.ones((Lz, Ly, Lx), np.uint8)
+    zax = np.repeat(np.array([0.0, 0.0, 1.0])[:, None], N, axis=1)
+    o1 = oracle_mod.Oracle(Lx, Ly, Lz, A, B, Cc, L1, mask=mask, kind=ones, W=np.full(N, 1.3), axis=zax)
+    assert abs(o1.energy(qu, variant, terms=True)[1][2] - 2 * Lx * Ly * 4.5 * S0 ** 2 * 1.3 * np.sin(theta) ** 2) < 1e-12
+
+
+# ------------------------------- P13: the L2-vs-L3 split of Eq. 10 next to objects
+
+def _ramp_site_problem(oracle_mod, L2, L3, L1v=0.0, wall=False):
+    """6^3 lattice, probe site (2,2,2); with wall=True the site (1,2,2) is an object, so the probe has
+    only a FORWARD x difference."""
+    mask = np.zeros((6, 6, 6), np.uint8)
+    if wall:
+        mask[2, 2, 1] = 1
+    return oracle_mod.Oracle(6, 6, 6, 0.0, 0.0, 1.0, L1v, L2, L3, mask=mask)
+
+
+@pytest.mark.parametrize("variant", [0, 1])
+@pytest.mark.parametrize("wall", [False, True])
+def test_L2_and_L3_terms_separately_on_hand_built_ramps(oracle_mod, variant, wall):
+    """Eq. 10:  f = L1/2 d_k Q_ij d_k Q_ij + L2/2 d_j Q_ij d_k Q_ik + L3/2 d_j Q_ik d_k Q_ij.
+    Field: around the probe site only  d_x Q_xx = a  (hence d_x Q_zz = -a, tracelessness) and
+    d_y Q_xy = d_y Q_yx = b  are non-zero.  By hand from the printed index patterns:
+      L2 term: (L2/2) sum_i (sum_j d_j Q_ij)^2; only i = x survives: d_x Q_xx + d_y Q_xy = a + b
+               -> (L2/2) (a^2 + 2 a b + b^2)
+      L3 term: (L3/2) sum_ijk d_j Q_ik d_k Q_ij; the surviving products are (j,i,k) = (x,x,x): a^2 and
+               (y,x,y): b^2 -- no product pairs d_x Q_xx with d_y Q_xy -> (L3/2) (a^2 + b^2)
+      L1 term: (L1/2) (2 a^2 + 2 b^2)  (entries xx, zz and xy, yx)
+    so the cross product 2ab tells the two index patterns apart.  Discretisation (DESIGN.md
+    R5/R7): forward and backward differences differ here (a+ != a-, b+ != b-); same-axis products average to
+    the mean of the allowed squares, different-axis products to the product of the mean differences.  With the
+    object at x-1 only the forward x difference is allowed."""
+    ap, am, bp, bm = 0.11, 0.05, -0.07, 0.13
+    base = np.array([0.2, -0.1, 0.3, 0.15, -0.25])
+    q = np.repeat(base[:, None], 216, axis=1).reshape(5, 6, 6, 6).copy()     # [c][z][y][x]
+    q[0, 2, 2, 3] += ap        # Q_xx(x+1) = Q_xx + a+
+    q[0, 2, 2, 1] -= am        # Q_xx(x-1) = Q_xx - a-   (an object site when wall=True: never read)
+    q[1, 2, 3, 2] += bp        # Q_xy(y+1) = Q_xy + b+
+    q[1, 2, 1, 2] -= bm        # Q_xy(y-1) = Q_xy - b-
+    q = q.reshape(5, -1)
+    a2 = ap ** 2 if wall else 0.5 * (ap ** 2 + am ** 2)
+    abar = ap if wall else 0.5 * (ap + am)
+    b2, bbar = 0.5 * (bp ** 2 + bm ** 2), 0.5 * (bp + bm)
+    e_L2 = _ramp_site_problem(oracle_mod, 1.0, 0.0, wall=wall).site_energy(q, 2, 2, 2, variant)[1][1]
+    e_L3 = _ramp_site_problem(oracle_mod, 0.0, 1.0, wall=wall).site_energy(q, 2, 2, 2, variant)[1][1]
+    e_L1 = _ramp_site_problem(oracle_mod, 0.0, 0.0, L1v=1.0, wall=wall).site_energy(q, 2, 2, 2, variant)[1][1]
+    assert abs(e_L2 - 0.5 * (a2 + 2 * abar * bbar + b2)) < 1e-16
+    assert abs(e_L3 - 0.5 * (a2 + b2)) < 1e-16
+    assert abs(e_L1 - (a2 + b2)) < 1e-16
+    assert abs(e_L2 - e_L3) > 1e-3                      # the pin separates them
+
+
+@pytest.mark.parametrize("variant", [0, 1])
+def test_L2_minus_L3_is_a_wall_surface_sum(oracle_mod, variant):
+    """E(L2 = a, L3 = 0) - E(L2 = 0, L3 = a) on a slab (object layers z = 0 and z = Lz-1, periodic x, y).
+    Per site the two terms differ by  (a/2) sum_i sum_{j != k} [Dbar_j Q_ij Dbar_k Q_ik - Dbar_j Q_ik Dbar_k Q_ij]
+    (Eq. 10; the j = k products are identical).  Pairs (x, y): both are centred differences on
+    periodic planes, which commute and are antisymmetric -> the plane sum vanishes by summation by parts.  Pairs
+    (m, z), m in {x, y}: with <f, g> the sum over a plane, <C_m f, g> = -<f, C_m g>, and Dbar_z = sum_z' d_zz' with
+    d centred in the interior, forward at z = 1, backward at z = n = Lz-2, the sum over planes collapses to
+    sum_zz' (d + d^T)_zz' <C_m Q_im (z), Q_iz (z')>; d + d^T vanishes except
+       (1,1) = -2, (1,2) = (2,1) = 1/2, (n,n) = +2, (n,n-1) = (n-1,n) = -1/2.
+    Hence the difference is a sum over the two planes next to each wall only:
+       dE = a sum_i sum_m [ -2 M(1,1) + (M(1,2) + M(2,1))/2 + 2 M(n,n) - (M(n,n-1) + M(n-1,n))/2 ],
+       M(z,z') = sum_{x,y} (C_m Q_im)(x,y,z) Q_iz(x,y,z').
+    A swap of the L2 and L3 index patterns flips the sign of dE."""
+    Lx, Ly, Lz = 6, 5, 7
+    a = 0.9
+    rng = np.random.default_rng(33)
+    q = 0.3 * rng.standard_normal((5, Lx * Ly * Lz))
+    mask = np.zeros((Lz, Ly, Lx), np.uint8)
+    mask[0] = mask[Lz - 1] = 1
+    o2 = oracle_mod.Oracle(Lx, Ly, Lz, A, B, Cc, L1, a, 0.0, mask=mask)
+    o3 = oracle_mod.Oracle(Lx, Ly, Lz, A, B, Cc, L1, 0.0, a, mask=mask)
+    dE = o2.energy(q, variant) - o3.energy(q, variant)
+    Q = full_tensor(q).reshape(Lz, Ly, Lx, 3, 3)                      # [z][y][x][i][j]
+    n = Lz - 2
+    expect = 0.0
+    for i in range(3):
+        for m, ax in ((0, 2), (1, 1)):                               # m = x (array axis 2), y (array axis 1)
+            Cm = 0.5 * (np.roll(Q[..., i, m], -1, axis=ax) - np.roll(Q[..., i, m], 1, axis=ax))   # [z][y][x]
+            Qiz = Q[..., i, 2]
+
+            def M(z, zp):
+                return float(np.sum(Cm[z] * Qiz[zp]))
+            expect += a * (-2 * M(1, 1) + 0.5 * (M(1, 2) + M(2, 1)) + 2 * M(n, n) - 0.5 * (M(n, n - 1) + M(n - 1, n)))
+    assert abs(dE) > 1e-3
+    assert abs(dE - expect) < 1e-12
 
 
 # ------------------------------------------------------- P11: classification

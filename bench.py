@@ -12,8 +12,9 @@ Prints ONE JSON line (rank 0).  Keys follow the driver's contract; see DESIGN.md
              on the library's stream, max over ranks)
   e2e        same metric through the C ABI with HOST buffers: lq_set_Q(pinned host) +
              lq_fire_minimize(K) + lq_get_Q(pinned host), all inside the timed region
-  roofline   algorithmic bytes (160 B per site-update, +1 flag byte with objects) per launch
-             / average launch duration, against MEASURED_PEAKS.json's HBM copy bandwidth
+  roofline   algorithmic bytes (160 B per site-update, +1 flag byte with objects) x simulated sites
+             per launch / average launch duration of the sweep (the library's CUDA events around its launch loop /
+             sweep launches), against MEASURED_PEAKS.json's HBM copy bandwidth
   cpu_baseline  the oracle (oracle/, OpenMP, as it stands) timed on this box's host cores on a bounded
              crop of the same workload
 Multi-GPU: the path is single-GPU by design (north_star); --gpus N runs N independent replicas
@@ -315,8 +316,9 @@ def main():
         t_max, units2 = aggregate(t_e2e, nsim * K, world, dist, torch.device("cuda", local))
         e2e = {"value": units2 / (t_max * 1e-3), "unit": UNIT, "h2d_bytes_per_step": 40.0 * N / K,
                "d2h_bytes_per_step": 40.0 * N / K, "ms_total": t_max,
-               "call": "lq_set_Q(pinned host) + %s(%d) + lq_get_Q(pinned host)" % (
-                   "lq_fire_minimize" if args.method == "fire" else "lq_descent_minimize", K)}
+               "call": "lq_set_Q(pinned host) + %s + lq_get_Q(pinned host)" % (
+                   {"fire": "lq_fire_minimize(%d)" % K, "analyze": "%d x lq_analyze" % K}.get(
+                       args.method, "lq_descent_minimize(%d)" % K))}
 
     if rank != 0:
         if dist is not None:
@@ -327,8 +329,13 @@ def main():
     flag_byte = 1.0 if lq.lq_get_info(ctx, "n_object") > 0 else 0.0
     # FIRE reads + writes q and v (+ flag byte).  GD: read q, write q; Nesterov: read q_k, q_{k-1}, write q_{k+1}
     alg_bytes_site = {"fire": 160.0, "gd": 80.0, "nesterov": 120.0, "analyze": 73.0}[args.method] + flag_byte
-    launch_ms = ms / max(rep["sweep_launches"], 1)           # average launch duration over the timed region
-    achieved = alg_bytes_site * N / (launch_ms * 1e-3) / 1e9
+    # average duration of one launch of the dominant kernel over the timed region: the library's own CUDA events
+    # around its launch loop (on the stream the kernels run on) / launches of that kernel.  Since Algorithm 1's
+    # initialisation rides on the first sweep there is nothing else inside those events (masked three-constant
+    # lattices: the sweep plus its fix-up launch).  Units per launch = simulated sites.
+    loop_ms = rep.get("gpu_ms") or ms
+    launch_ms = loop_ms / max(rep["sweep_launches"], 1)
+    achieved = alg_bytes_site * nsim / (launch_ms * 1e-3) / 1e9
     design_bytes_site = lq.lq_get_info(ctx, "sweep_bytes_per_site") if args.method == "fire" else alg_bytes_site
     three = c["L2"] != 0 or c["L3"] != 0
     if args.method == "analyze":
@@ -347,8 +354,8 @@ def main():
     roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                 "traffic": traffic, "peak_kind": peak_kind, "kernel": kernel_name,
                 "algorithmic_bytes_per_site": alg_bytes_site, "design_bytes_per_site": design_bytes_site,
-                "achieved_design_GBs": design_bytes_site * N / (launch_ms * 1e-3) / 1e9,
-                "launch_ms": launch_ms}
+                "achieved_design_GBs": design_bytes_site * nsim / (launch_ms * 1e-3) / 1e9,
+                "launch_ms": launch_ms, "launches_timed": rep["sweep_launches"], "sites_per_launch": nsim}
 
     cpu = None
     if not args.no_cpu_baseline:

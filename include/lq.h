@@ -81,13 +81,18 @@ int lq_set_sites(lq_ctx *ctx, const uint8_t *mask, const uint8_t *anch_kind,
 /* Copy the packed class/neighbour byte of every site into flags[N] (bit-exact parity gate). */
 int lq_get_flags(lq_ctx *ctx, uint8_t *flags, int where);
 
-/* Set / read the Q field, [5][N] fp64 SoA.  lq_set_Q also resets the FIRE velocities to 0.
+/* Set / read the Q field, [5][N] fp64 SoA.  After lq_set_Q the FIRE velocities read as 0.
  * Values at object sites are stored and returned unchanged and never enter any result
  * (R17).  lq_get_Q before lq_set_Q: LQ_ERR_STATE. */
 int lq_set_Q(lq_ctx *ctx, const double *q, int where);
 int lq_get_Q(lq_ctx *ctx, double *q, int where);
 
-/* FIRE velocities after the last lq_fire_minimize ([5][N]; zeros after lq_set_Q). */
+/* FIRE velocities after the last lq_fire_minimize ([5][N]): the v of Algorithm 1 at the end of
+ * the last step, i.e. after its rescale v <- (1-alpha) v + alpha |v| F/|F| (or v <- 0 when P <= 0); the state the
+ * stop test fired on keeps its un-rescaled v.  Zeros after lq_set_Q, after lq_descent_minimize and when no step
+ * was taken.  The fused sweeps apply the rescale lazily (inside the next step), so this call finishes it on a copy:
+ * one force pass + one streaming pass, only when asked.  With integrator = 1 a run stopped by force_tol returns the
+ * velocity already kicked with the final force. */
 int lq_get_velocity(lq_ctx *ctx, double *v, int where);
 
 /* Total free energy F = sum over simulated sites of f_bulk + f_distortion + f_anchoring
@@ -206,6 +211,8 @@ int lq_get_S0(lq_ctx *ctx, double *S0);
  *                      path, 2 = fused sweep with the force stored (any constants).
  *                      lq_descent_minimize: 0 = TMA sweep over the constant-weight sites + list kernel for the
  *                      rest, 1 = general kernel on every site
+ *   "rc_chunks" (set): recompute sweep: 0 = z-chunks per tile column chosen by the makespan model (default),
+ *                      n > 0 = n equal chunks per column (clamped to chunks of 4 .. 126 planes)
  *   "sweep_bytes_per_site" (get): algorithmic HBM bytes one sweep moves per site
  *   "n_simulated" (get), "n_boundary" (get), "n_object" (get)
  * Unknown key: LQ_ERR_ARG. */

@@ -32,6 +32,12 @@ struct lq_ctx {
     LqSweepPlan *sweep = nullptr;
     LqDescentPlan *descent = nullptr;
     int fire_path = 0;
+    int rc_chunks = 0;                   // "rc_chunks" option: 0 = chunk table chosen by the makespan model
+    bool v_valid = false;                // v[cur] holds the velocities of the last lq_fire_minimize (else: report zeros)
+    double v_mix_a = 1.0, v_mix_b = 0.0; // FIRE rescale of the last step, not yet applied to v[cur] (the sweeps apply it lazily)
+    cudaEvent_t ev0 = nullptr, ev1 = nullptr;   // timing of the minimisation loops (report.gpu_ms)
+    void *scratch = nullptr;             // lq_analyze(LQ_HOST): device staging of the outputs, grown on demand
+    size_t scratch_len = 0;
     std::string err;
 };
 
@@ -62,8 +68,9 @@ LqFields fields_of(const lq_ctx *c) {
 }
 
 // copy between a caller's dense [ncomp][Lz][Ly][Lx] array and a padded device array
-cudaError_t copy_box(const LqGeom &g, void *padded, const void *user, size_t elem, int ncomp, bool to_padded,
+cudaError_t copy_box(const LqGeom &g, const void *padded_c, const void *user, size_t elem, int ncomp, bool to_padded,
                      cudaStream_t st) {
+    void *padded = const_cast<void *>(padded_c);
     for (int c = 0; c < ncomp; ++c) {
         cudaMemcpy3DParms p;
         memset(&p, 0, sizeof(p));
@@ -97,6 +104,16 @@ int ensure_field(lq_ctx *c, double **p) {
 }
 
 bool bad_where(int w) { return w != LQ_HOST && w != LQ_DEVICE; }
+
+// every ABI entry runs on the context's device, whatever device the calling thread had current
+struct DeviceGuard {
+    int prev = -1;
+    explicit DeviceGuard(const lq_ctx *c) {
+        if (c && cudaGetDevice(&prev) == cudaSuccess && prev != c->device) cudaSetDevice(c->device);
+        else prev = -1;
+    }
+    ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
+};
 
 }  // namespace
 
@@ -142,8 +159,12 @@ int lq_create(int Lx, int Ly, int Lz, double A, double B, double C, double L1, d
         if (cudaMalloc(&c->dscal3, 3 * sizeof(double)) != cudaSuccess ||
             cudaMalloc(&c->dsc, 2 * sizeof(LqFireScalars)) != cudaSuccess ||
             cudaMalloc(&c->dcounts, 3 * sizeof(unsigned long long)) != cudaSuccess ||
-            cudaMalloc(&c->dbad, sizeof(int)) != cudaSuccess) {
+            cudaMalloc(&c->dbad, 2 * sizeof(int)) != cudaSuccess) {
             rc = fail(nullptr, LQ_ERR_NOMEM, "lq_create: cudaMalloc failed");
+            break;
+        }
+        if (cudaEventCreate(&c->ev0) != cudaSuccess || cudaEventCreate(&c->ev1) != cudaSuccess) {
+            rc = fail(nullptr, LQ_ERR_CUDA, "lq_create: cudaEventCreate failed");
             break;
         }
     } while (0);
@@ -154,6 +175,10 @@ int lq_create(int Lx, int Ly, int Lz, double A, double B, double C, double L1, d
 
 void lq_destroy(lq_ctx *c) {
     if (!c) return;
+    DeviceGuard dg(c);
+    if (c->ev0) cudaEventDestroy(c->ev0);
+    if (c->ev1) cudaEventDestroy(c->ev1);
+    cudaFree(c->scratch);
     for (int i = 0; i < 2; ++i) { cudaFree(c->q[i]); cudaFree(c->v[i]); cudaFree(c->F[i]); }
     cudaFree(c->maskp); cudaFree(c->flags); cudaFree(c->kind); cudaFree(c->W); cudaFree(c->axis);
     cudaFree(c->partials); cudaFree(c->dscal3); cudaFree(c->dsc); cudaFree(c->dcounts); cudaFree(c->dbad);
@@ -164,6 +189,7 @@ void lq_destroy(lq_ctx *c) {
 
 int lq_set_stream(lq_ctx *c, void *s) {
     if (!c) return LQ_ERR_ARG;
+    DeviceGuard dg(c);
     c->stream = (cudaStream_t)s;
     return LQ_OK;
 }
@@ -171,61 +197,64 @@ int lq_set_stream(lq_ctx *c, void *s) {
 int lq_set_sites(lq_ctx *c, const uint8_t *mask, const uint8_t *anch_kind, const double *W, const double *axis,
                  int where) {
     if (!c) return LQ_ERR_ARG;
+    DeviceGuard dg(c);
     if (bad_where(where)) return fail(c, LQ_ERR_ARG, "lq_set_sites: bad `where`");
     if (anch_kind && (!W || !axis)) return fail(c, LQ_ERR_ARG, "lq_set_sites: anch_kind given without W / axis");
     const LqGeom &g = c->g;
     cudaStream_t st = c->stream;
-    lq_sweep_invalidate(c->sweep);
-    lq_descent_invalidate(c->descent);
     if (!mask) {
+        lq_sweep_invalidate(c->sweep);
+        lq_descent_invalidate(c->descent);
         c->flags_active = false; c->anch_active = false;
         c->n_class[0] = (unsigned long long)g.N; c->n_class[1] = c->n_class[2] = 0;
         return LQ_OK;
     }
+    // 1. stage the inputs and validate them; the context's geometry state changes only after both checks passed
+    //    (the staging arrays themselves are scratch until then: on a bad input the sites are reset to "all bulk")
     if (!c->maskp) LQ_CUDA(c, cudaMalloc(&c->maskp, (size_t)g.NP));
     if (!c->flags) LQ_CUDA(c, cudaMalloc(&c->flags, (size_t)g.NP));
     LQ_CUDA(c, cudaMemsetAsync(c->maskp, 0, (size_t)g.NP, st));
-    LQ_CUDA(c, cudaMemsetAsync(c->flags, 0xFC, (size_t)g.NP, st));
     LQ_CUDA(c, copy_box(g, c->maskp, mask, 1, 1, true, st));
-    LQ_CUDA(c, cudaMemsetAsync(c->dbad, 0, sizeof(int), st));
+    LQ_CUDA(c, cudaMemsetAsync(c->dbad, 0, 2 * sizeof(int), st));
     lq_launch_check_u8_max(g, c->maskp, 1, c->dbad, st);
-    lq_launch_fill_ghosts_u8(g, c->maskp, st);
-    lq_launch_classify(g, c->maskp, c->flags, st);
-    lq_launch_fill_ghosts_u8(g, c->flags, st);
-    LQ_CUDA(c, cudaMemsetAsync(c->dcounts, 0, 3 * sizeof(unsigned long long), st));
-    lq_launch_count_classes(g, c->flags, c->dcounts, st);
-    int bad_kind = 0;
     if (anch_kind) {
         if (!c->kind) LQ_CUDA(c, cudaMalloc(&c->kind, (size_t)g.NP));
         if (!c->W) LQ_CUDA(c, cudaMalloc(&c->W, (size_t)g.NP * sizeof(double)));
         if (!c->axis) LQ_CUDA(c, cudaMalloc(&c->axis, (size_t)3 * g.NP * sizeof(double)));
         LQ_CUDA(c, cudaMemsetAsync(c->kind, 0, (size_t)g.NP, st));
+        LQ_CUDA(c, copy_box(g, c->kind, anch_kind, 1, 1, true, st));
+        lq_launch_check_u8_max(g, c->kind, 2, c->dbad + 1, st);
+    }
+    int bad[2] = {0, 0};
+    LQ_CUDA(c, cudaMemcpyAsync(bad, c->dbad, 2 * sizeof(int), cudaMemcpyDeviceToHost, st));
+    LQ_CUDA(c, cudaStreamSynchronize(st));
+    lq_sweep_invalidate(c->sweep);
+    lq_descent_invalidate(c->descent);
+    if (bad[0] || (anch_kind && bad[1])) {
+        c->flags_active = false; c->anch_active = false;
+        c->n_class[0] = (unsigned long long)g.N; c->n_class[1] = c->n_class[2] = 0;
+        return fail(c, LQ_ERR_ARG, bad[0] ? "lq_set_sites: mask value > 1 (sites reset to all bulk)"
+                                          : "lq_set_sites: anch_kind value > 2 (sites reset to all bulk)");
+    }
+    // 2. classify
+    LQ_CUDA(c, cudaMemsetAsync(c->flags, 0xFC, (size_t)g.NP, st));
+    lq_launch_fill_ghosts_u8(g, c->maskp, st);
+    lq_launch_classify(g, c->maskp, c->flags, st);
+    lq_launch_fill_ghosts_u8(g, c->flags, st);
+    LQ_CUDA(c, cudaMemsetAsync(c->dcounts, 0, 3 * sizeof(unsigned long long), st));
+    lq_launch_count_classes(g, c->flags, c->dcounts, st);
+    if (anch_kind) {
         LQ_CUDA(c, cudaMemsetAsync(c->W, 0, (size_t)g.NP * sizeof(double), st));
         LQ_CUDA(c, cudaMemsetAsync(c->axis, 0, (size_t)3 * g.NP * sizeof(double), st));
-        LQ_CUDA(c, copy_box(g, c->kind, anch_kind, 1, 1, true, st));
         LQ_CUDA(c, copy_box(g, c->W, W, sizeof(double), 1, true, st));
         LQ_CUDA(c, copy_box(g, c->axis, axis, sizeof(double), 3, true, st));
         lq_launch_fill_ghosts_u8(g, c->kind, st);     // the recompute sweep evaluates anchoring on halo sites
         lq_launch_fill_ghosts_f64(g, c->W, 1, st);
         lq_launch_fill_ghosts_f64(g, c->axis, 3, st);
-        int *dbad2 = c->dbad;  // reuse after reading the first result
-        int bad_mask = 0;
-        LQ_CUDA(c, cudaMemcpyAsync(&bad_mask, c->dbad, sizeof(int), cudaMemcpyDeviceToHost, st));
-        LQ_CUDA(c, cudaStreamSynchronize(st));
-        if (bad_mask) { c->flags_active = false; return fail(c, LQ_ERR_ARG, "lq_set_sites: mask value > 1"); }
-        LQ_CUDA(c, cudaMemsetAsync(dbad2, 0, sizeof(int), st));
-        lq_launch_check_u8_max(g, c->kind, 2, dbad2, st);
-        LQ_CUDA(c, cudaMemcpyAsync(&bad_kind, dbad2, sizeof(int), cudaMemcpyDeviceToHost, st));
-    } else {
-        int bad_mask = 0;
-        LQ_CUDA(c, cudaMemcpyAsync(&bad_mask, c->dbad, sizeof(int), cudaMemcpyDeviceToHost, st));
-        LQ_CUDA(c, cudaStreamSynchronize(st));
-        if (bad_mask) { c->flags_active = false; return fail(c, LQ_ERR_ARG, "lq_set_sites: mask value > 1"); }
     }
     LQ_CUDA(c, cudaMemcpyAsync(c->n_class, c->dcounts, 3 * sizeof(unsigned long long), cudaMemcpyDeviceToHost, st));
     LQ_CUDA(c, cudaStreamSynchronize(st));
     LQ_CUDA(c, cudaGetLastError());
-    if (bad_kind) { c->anch_active = false; return fail(c, LQ_ERR_ARG, "lq_set_sites: anch_kind value > 2"); }
     c->flags_active = c->n_class[2] > 0;
     c->anch_active = anch_kind != nullptr && c->n_class[1] > 0;
     return LQ_OK;
@@ -233,6 +262,7 @@ int lq_set_sites(lq_ctx *c, const uint8_t *mask, const uint8_t *anch_kind, const
 
 int lq_get_flags(lq_ctx *c, uint8_t *flags, int where) {
     if (!c) return LQ_ERR_ARG;
+    DeviceGuard dg(c);
     if (!flags || bad_where(where)) return fail(c, LQ_ERR_ARG, "lq_get_flags: bad argument");
     if (!c->flags_active) {
         if (where == LQ_HOST) memset(flags, 0xFC, (size_t)c->g.N);
@@ -246,18 +276,20 @@ int lq_get_flags(lq_ctx *c, uint8_t *flags, int where) {
 
 int lq_set_Q(lq_ctx *c, const double *q, int where) {
     if (!c) return LQ_ERR_ARG;
+    DeviceGuard dg(c);
     if (!q || bad_where(where)) return fail(c, LQ_ERR_ARG, "lq_set_Q: bad argument");
     LQ_CUDA(c, copy_box(c->g, c->q[c->cur], q, sizeof(double), 5, true, c->stream));
     lq_launch_fill_ghosts_f64(c->g, c->q[c->cur], 5, c->stream);
-    if (c->v[c->cur]) LQ_CUDA(c, cudaMemsetAsync(c->v[c->cur], 0, (size_t)5 * c->g.NP * sizeof(double), c->stream));
     LQ_CUDA(c, cudaStreamSynchronize(c->stream));
     LQ_CUDA(c, cudaGetLastError());
     c->has_Q = true;
+    c->v_valid = false;        // velocities read as zero until the next lq_fire_minimize (no 40 B/site memset here)
     return LQ_OK;
 }
 
 int lq_get_Q(lq_ctx *c, double *q, int where) {
     if (!c) return LQ_ERR_ARG;
+    DeviceGuard dg(c);
     if (!q || bad_where(where)) return fail(c, LQ_ERR_ARG, "lq_get_Q: bad argument");
     if (!c->has_Q) return fail(c, LQ_ERR_STATE, "lq_get_Q: no Q has been set");
     LQ_CUDA(c, copy_box(c->g, c->q[c->cur], q, sizeof(double), 5, false, c->stream));
@@ -267,17 +299,31 @@ int lq_get_Q(lq_ctx *c, double *q, int where) {
 
 int lq_get_velocity(lq_ctx *c, double *v, int where) {
     if (!c) return LQ_ERR_ARG;
+    DeviceGuard dg(c);
     if (!v || bad_where(where)) return fail(c, LQ_ERR_ARG, "lq_get_velocity: bad argument");
     if (!c->has_Q) return fail(c, LQ_ERR_STATE, "lq_get_velocity: no Q has been set");
     int rc = ensure_field(c, &c->v[c->cur]);
     if (rc != LQ_OK) return rc;
-    LQ_CUDA(c, copy_box(c->g, c->v[c->cur], v, sizeof(double), 5, false, c->stream));
+    if (!c->v_valid) {
+        LQ_CUDA(c, cudaMemsetAsync(c->v[c->cur], 0, (size_t)5 * c->g.NP * sizeof(double), c->stream));
+        c->v_valid = true; c->v_mix_a = 1.0; c->v_mix_b = 0.0;
+    }
+    const double *src = c->v[c->cur];
+    if (c->v_mix_a != 1.0 || c->v_mix_b != 0.0) {
+        // the last step's rescale v <- (1-alpha) v + alpha |v| F/|F| (or v <- 0) is still pending: apply it to a copy
+        if ((rc = ensure_field(c, &c->F[c->cur])) != LQ_OK) return rc;
+        lq_launch_forces(c->g, c->ph, fields_of(c), c->q[c->cur], c->F[c->cur], c->stream);
+        lq_launch_axpby((long long)5 * c->g.NP, c->v_mix_a, c->v[c->cur], c->v_mix_b, c->F[c->cur], c->F[c->cur], c->stream);
+        src = c->F[c->cur];
+    }
+    LQ_CUDA(c, copy_box(c->g, src, v, sizeof(double), 5, false, c->stream));
     LQ_CUDA(c, cudaStreamSynchronize(c->stream));
     return LQ_OK;
 }
 
 int lq_energy_terms(lq_ctx *c, double *terms) {
     if (!c) return LQ_ERR_ARG;
+    DeviceGuard dg(c);
     if (!terms) return fail(c, LQ_ERR_ARG, "lq_energy_terms: terms is NULL");
     if (!c->has_Q) return fail(c, LQ_ERR_STATE, "lq_energy: no Q has been set");
     int rc = ensure_partials(c, (size_t)3 * lq_energy_num_blocks(c->g));
@@ -291,6 +337,7 @@ int lq_energy_terms(lq_ctx *c, double *terms) {
 
 int lq_energy(lq_ctx *c, double *E) {
     if (!c) return LQ_ERR_ARG;
+    DeviceGuard dg(c);
     if (!E) return fail(c, LQ_ERR_ARG, "lq_energy: E is NULL");
     double t[3];
     int rc = lq_energy_terms(c, t);
@@ -301,6 +348,7 @@ int lq_energy(lq_ctx *c, double *E) {
 
 int lq_forces(lq_ctx *c, double *F, int where) {
     if (!c) return LQ_ERR_ARG;
+    DeviceGuard dg(c);
     if (!F || bad_where(where)) return fail(c, LQ_ERR_ARG, "lq_forces: bad argument");
     if (!c->has_Q) return fail(c, LQ_ERR_STATE, "lq_forces: no Q has been set");
     int rc = ensure_field(c, &c->F[c->cur]);
@@ -320,9 +368,15 @@ int lq_get_S0(lq_ctx *c, double *S0) {
 
 int lq_set_option(lq_ctx *c, const char *key, double value) {
     if (!c || !key) return LQ_ERR_ARG;
+    DeviceGuard dg(c);
     if (!strcmp(key, "fire_path")) {
         if (value != 0.0 && value != 1.0 && value != 2.0) return fail(c, LQ_ERR_ARG, "fire_path must be 0, 1 or 2");
         c->fire_path = (int)value;
+        return LQ_OK;
+    }
+    if (!strcmp(key, "rc_chunks")) {
+        if (!(value >= 0.0 && value <= 4096.0)) return fail(c, LQ_ERR_ARG, "rc_chunks must be in [0, 4096]");
+        c->rc_chunks = (int)value;
         return LQ_OK;
     }
     return fail(c, LQ_ERR_ARG, std::string("lq_set_option: unknown key ") + key);
@@ -346,6 +400,7 @@ int lq_get_info(lq_ctx *c, const char *key, double *value) {
 
 int lq_fire_minimize(lq_ctx *c, long max_steps, double force_tol, const lq_fire_params *fp, lq_fire_report *out) {
     if (!c) return LQ_ERR_ARG;
+    DeviceGuard dg(c);
     if (!fp || !out) return fail(c, LQ_ERR_ARG, "lq_fire_minimize: NULL params / report");
     if (!c->has_Q) return fail(c, LQ_ERR_STATE, "lq_fire_minimize: no Q has been set");
     if (!(fp->dt0 > 0.0) || !(fp->dtmax >= fp->dt0) || !(fp->alpha0 >= 0.0 && fp->alpha0 <= 1.0) ||
@@ -356,50 +411,51 @@ int lq_fire_minimize(lq_ctx *c, long max_steps, double force_tol, const lq_fire_
     const LqGeom &g = c->g;
     cudaStream_t st = c->stream;
     int rc;
-    if ((rc = ensure_field(c, &c->v[c->cur])) != LQ_OK) return rc;
-    if ((rc = ensure_field(c, &c->F[c->cur])) != LQ_OK) return rc;
-    // the fused sweeps' constant-weight stencils do not carry the chiral term: L4 != 0 runs the general kernels
-    // ... and so does the semi-implicit Euler variant (integrator = 1)
     const bool euler = fp->integrator == 1;
-    const bool fused = c->fire_path != 1 && !lq_general_only(c->ph);
+    const bool fused = c->fire_path != 1;
     const bool three = lq_three(c->ph);
     const bool stored_F = three || c->fire_path == 2;   // recompute-F sweep: one-constant only
+    if ((rc = ensure_field(c, &c->v[c->cur])) != LQ_OK) return rc;
+    if ((!fused || stored_F) && (rc = ensure_field(c, &c->F[c->cur])) != LQ_OK) return rc;
     if (fused) {
         if ((rc = ensure_field(c, &c->q[c->cur ^ 1])) != LQ_OK) return rc;
         if ((rc = ensure_field(c, &c->v[c->cur ^ 1])) != LQ_OK) return rc;
-        if ((stored_F || c->flags_active) && (rc = ensure_field(c, &c->F[c->cur ^ 1])) != LQ_OK) return rc;
+        if (stored_F && (rc = ensure_field(c, &c->F[c->cur ^ 1])) != LQ_OK) return rc;
     }
-    const int nb1 = lq_fire1_num_blocks(g);
-    if ((rc = ensure_partials(c, (size_t)4 * nb1)) != LQ_OK) return rc;
 
     LqFireConsts fc{fp->dt0, fp->dtmax, fp->alpha0, fp->finc, fp->fdec, fp->falpha, force_tol, fp->Nmin, (long long)max_steps,
-                    fp->integrator == 1 ? 1 : 0};
+                    euler ? 1 : 0};
     LqFireScalars h;
     memset(&h, 0, sizeof(h));
-    h.dt = euler ? fp->dt0 : 0.0; h.alpha = fp->alpha0; h.mix_a = 1.0; h.mix_b = 0.0;
-    LQ_CUDA(c, cudaMemcpyAsync(&c->dsc[0], &h, sizeof(h), cudaMemcpyHostToDevice, st));
-    LQ_CUDA(c, cudaMemsetAsync(c->v[c->cur], 0, (size_t)5 * g.NP * sizeof(double), st));
     const LqFields f = fields_of(c);
     long launches = 0, sweeps = 0;
+    LQ_CUDA(c, cudaEventRecord(c->ev0, st));
 
-    cudaEvent_t ev0, ev1;
-    LQ_CUDA(c, cudaEventCreate(&ev0));
-    LQ_CUDA(c, cudaEventCreate(&ev1));
-    LQ_CUDA(c, cudaEventRecord(ev0, st));
-
-    // step 0: F = force(q), convergence test on the initial state (dt = 0: no kick)
-    // (Euler variant: the same launch is the first step's full kick v += dt0 F and its reductions)
-    const long long emax = euler ? (long long)max_steps : -1;
-    lq_launch_fire1_force(g, c->ph, f, c->q[c->cur], c->v[c->cur], c->F[c->cur], &c->dsc[0], c->partials, st, emax);
-    lq_launch_fire_update(c->partials, nb1, &c->dsc[0], fc, euler ? 2 : 1, st);
-    launches += 2;
-
-    long done = 0;
     if (fused) {
+        // Algorithm 1's initialisation (v = 0, dt0, alpha0, force of the initial state and the stop test on it) is
+        // part of the first sweep: mix_a = mix_b = 0 makes it ignore whatever the velocity buffer holds, the
+        // recompute sweep reduces max|F(q_0)| in its first phase, the stored-force path starts with one sweep whose
+        // step coefficients are all 0 (init), the Euler variant with its own [no drift | force | kick] sweep.
+        h.dt = fp->dt0; h.alpha = fp->alpha0; h.mix_a = 0.0; h.mix_b = 0.0; h.dt_prev = 0.0;
+        h.init = (stored_F && !euler) ? 1 : 0;
+        LQ_CUDA(c, cudaMemcpyAsync(&c->dsc[0], &h, sizeof(h), cudaMemcpyHostToDevice, st));
         rc = lq_sweep_run(&c->sweep, stored_F, g, c->ph, f, c->q, c->v, c->F, &c->cur, c->dsc, fc, max_steps, st, &launches,
-                          &sweeps, &h, c->err);
-        if (rc != LQ_OK) { cudaEventDestroy(ev0); cudaEventDestroy(ev1); return rc; }
+                          &sweeps, &h, c->err, c->rc_chunks);
+        if (rc != LQ_OK) return rc;
     } else {
+        // unfused cross-check path (fire_path = 1): generic one-thread-per-site kernels, 4 launches per step
+        const int nb1 = lq_fire1_num_blocks(g);
+        if ((rc = ensure_partials(c, (size_t)4 * nb1)) != LQ_OK) return rc;
+        h.dt = euler ? fp->dt0 : 0.0; h.alpha = fp->alpha0; h.mix_a = 1.0; h.mix_b = 0.0;
+        LQ_CUDA(c, cudaMemcpyAsync(&c->dsc[0], &h, sizeof(h), cudaMemcpyHostToDevice, st));
+        LQ_CUDA(c, cudaMemsetAsync(c->v[c->cur], 0, (size_t)5 * g.NP * sizeof(double), st));
+        // step 0: F = force(q), convergence test on the initial state (dt = 0: no kick)
+        // (Euler variant: the same launch is the first step's full kick v += dt0 F and its reductions)
+        const long long emax = euler ? (long long)max_steps : -1;
+        lq_launch_fire1_force(g, c->ph, f, c->q[c->cur], c->v[c->cur], c->F[c->cur], &c->dsc[0], c->partials, st, emax);
+        lq_launch_fire_update(c->partials, nb1, &c->dsc[0], fc, euler ? 2 : 1, st);
+        launches += 2;
+        long done = 0;
         const long chunk = force_tol > 0.0 ? 64 : 1024;
         while (done < max_steps) {
             const long n = (max_steps - done) < chunk ? (max_steps - done) : chunk;
@@ -419,12 +475,16 @@ int lq_fire_minimize(lq_ctx *c, long max_steps, double force_tol, const lq_fire_
         }
         LQ_CUDA(c, cudaMemcpyAsync(&h, &c->dsc[0], sizeof(h), cudaMemcpyDeviceToHost, st));
     }
-    LQ_CUDA(c, cudaEventRecord(ev1, st));
+    LQ_CUDA(c, cudaEventRecord(c->ev1, st));
     LQ_CUDA(c, cudaStreamSynchronize(st));
     LQ_CUDA(c, cudaGetLastError());
     float ms = 0.f;
-    cudaEventElapsedTime(&ms, ev0, ev1);
-    cudaEventDestroy(ev0); cudaEventDestroy(ev1);
+    cudaEventElapsedTime(&ms, c->ev0, c->ev1);
+    // velocities: the buffer holds the last step's v only if a step ran (a stop on the initial state leaves v = 0)
+    c->v_valid = h.step > 0 || !fused;
+    const bool pending = !h.converged && h.step > 0 && !(euler && h.step >= (long long)max_steps);
+    c->v_mix_a = pending ? h.mix_a : 1.0;
+    c->v_mix_b = pending ? h.mix_b : 0.0;
 
     const double nsim = (double)(c->flags_active ? c->n_class[0] + c->n_class[1] : (unsigned long long)g.N);
     out->steps = (long)h.step; out->converged = h.converged;
@@ -441,6 +501,7 @@ int lq_fire_minimize(lq_ctx *c, long max_steps, double force_tol, const lq_fire_
 
 int lq_analyze(lq_ctx *c, double thr, double *S, double *dir, uint8_t *defect, long *n_defect, int where) {
     if (!c) return LQ_ERR_ARG;
+    DeviceGuard dg(c);
     if (bad_where(where)) return fail(c, LQ_ERR_ARG, "lq_analyze: bad `where`");
     if (!c->has_Q) return fail(c, LQ_ERR_STATE, "lq_analyze: call lq_set_Q first");
     const LqGeom &g = c->g;
@@ -448,34 +509,37 @@ int lq_analyze(lq_ctx *c, double thr, double *S, double *dir, uint8_t *defect, l
     const size_t N = (size_t)g.N;
     double *dS = S, *dD = dir;
     uint8_t *dF = defect;
-    void *tmp[3] = {nullptr, nullptr, nullptr};
-    auto cleanup = [&]() { for (void *p : tmp) if (p) cudaFree(p); };
-    if (where == LQ_HOST) {                     // stage through device scratch
-        if (S) { if (cudaMalloc(&tmp[0], N * sizeof(double)) != cudaSuccess) { cleanup(); return fail(c, LQ_ERR_NOMEM, "lq_analyze: cudaMalloc"); } dS = (double *)tmp[0]; }
-        if (dir) { if (cudaMalloc(&tmp[1], 3 * N * sizeof(double)) != cudaSuccess) { cleanup(); return fail(c, LQ_ERR_NOMEM, "lq_analyze: cudaMalloc"); } dD = (double *)tmp[1]; }
-        if (defect) { if (cudaMalloc(&tmp[2], N) != cudaSuccess) { cleanup(); return fail(c, LQ_ERR_NOMEM, "lq_analyze: cudaMalloc"); } dF = (uint8_t *)tmp[2]; }
+    if (where == LQ_HOST) {                     // stage through device scratch kept in the context
+        const size_t need = (S ? N * sizeof(double) : 0) + (dir ? 3 * N * sizeof(double) : 0) + (defect ? N : 0);
+        if (need > c->scratch_len) {
+            cudaFree(c->scratch);
+            c->scratch = nullptr; c->scratch_len = 0;
+            LQ_CUDA(c, cudaMalloc(&c->scratch, need));
+            c->scratch_len = need;
+        }
+        char *sp = (char *)c->scratch;
+        if (S) { dS = (double *)sp; sp += N * sizeof(double); }
+        if (dir) { dD = (double *)sp; sp += 3 * N * sizeof(double); }
+        if (defect) dF = (uint8_t *)sp;
     }
-    cudaError_t e = cudaMemsetAsync(c->dcounts, 0, sizeof(unsigned long long), st);
-    if (e == cudaSuccess) {
-        lq_launch_analyze(g, c->q[c->cur], c->flags_active ? c->flags : nullptr, thr, dS, dD, dF, c->dcounts, st);
-        e = cudaGetLastError();
-    }
+    LQ_CUDA(c, cudaMemsetAsync(c->dcounts, 0, sizeof(unsigned long long), st));
+    lq_launch_analyze(g, c->q[c->cur], c->flags_active ? c->flags : nullptr, thr, dS, dD, dF, c->dcounts, st);
+    LQ_CUDA(c, cudaGetLastError());
     unsigned long long cnt = 0;
-    if (e == cudaSuccess) e = cudaMemcpyAsync(&cnt, c->dcounts, sizeof(cnt), cudaMemcpyDeviceToHost, st);
-    if (e == cudaSuccess && where == LQ_HOST) {
-        if (S) e = cudaMemcpyAsync(S, dS, N * sizeof(double), cudaMemcpyDeviceToHost, st);
-        if (e == cudaSuccess && dir) e = cudaMemcpyAsync(dir, dD, 3 * N * sizeof(double), cudaMemcpyDeviceToHost, st);
-        if (e == cudaSuccess && defect) e = cudaMemcpyAsync(defect, dF, N, cudaMemcpyDeviceToHost, st);
+    LQ_CUDA(c, cudaMemcpyAsync(&cnt, c->dcounts, sizeof(cnt), cudaMemcpyDeviceToHost, st));
+    if (where == LQ_HOST) {
+        if (S) LQ_CUDA(c, cudaMemcpyAsync(S, dS, N * sizeof(double), cudaMemcpyDeviceToHost, st));
+        if (dir) LQ_CUDA(c, cudaMemcpyAsync(dir, dD, 3 * N * sizeof(double), cudaMemcpyDeviceToHost, st));
+        if (defect) LQ_CUDA(c, cudaMemcpyAsync(defect, dF, N, cudaMemcpyDeviceToHost, st));
     }
-    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
-    cleanup();
-    if (e != cudaSuccess) return fail(c, LQ_ERR_CUDA, std::string("lq_analyze: ") + cudaGetErrorString(e));
+    LQ_CUDA(c, cudaStreamSynchronize(st));
     if (n_defect) *n_defect = (long)cnt;
     return LQ_OK;
 }
 
 int lq_set_chiral(lq_ctx *c, double L4) {
     if (!c) return LQ_ERR_ARG;
+    DeviceGuard dg(c);
     if (!std::isfinite(L4)) return fail(c, LQ_ERR_ARG, "lq_set_chiral: non-finite L4");
     c->ph.L4 = L4;
     return LQ_OK;
@@ -483,6 +547,7 @@ int lq_set_chiral(lq_ctx *c, double L4) {
 
 int lq_set_cubic(lq_ctx *c, double L6) {
     if (!c) return LQ_ERR_ARG;
+    DeviceGuard dg(c);
     if (!std::isfinite(L6)) return fail(c, LQ_ERR_ARG, "lq_set_cubic: non-finite L6");
     c->ph.L6 = L6;
     return LQ_OK;
@@ -490,6 +555,7 @@ int lq_set_cubic(lq_ctx *c, double L6) {
 
 int lq_set_field(lq_ctx *c, const double *H, double chi, const double *E, double eps) {
     if (!c) return LQ_ERR_ARG;
+    DeviceGuard dg(c);
     double h[3] = {0.0, 0.0, 0.0}, e[3] = {0.0, 0.0, 0.0};
     for (int i = 0; i < 3; ++i) {
         if (H) h[i] = H[i];
@@ -509,6 +575,7 @@ int lq_set_field(lq_ctx *c, const double *H, double chi, const double *E, double
 int lq_descent_minimize(lq_ctx *c, int method, long max_steps, double force_tol, const lq_descent_params *dp,
                         lq_fire_report *out) {
     if (!c) return LQ_ERR_ARG;
+    DeviceGuard dg(c);
     if (!dp || !out) return fail(c, LQ_ERR_ARG, "lq_descent_minimize: NULL pointer");
     memset(out, 0, sizeof(*out));
     if (!c->has_Q) return fail(c, LQ_ERR_STATE, "lq_descent_minimize: call lq_set_Q first");
@@ -526,28 +593,21 @@ int lq_descent_minimize(lq_ctx *c, int method, long max_steps, double force_tol,
     memset(&h, 0, sizeof(h));
     h.dt = dp->eta; h.alpha = dp->mu;
     LQ_CUDA(c, cudaMemcpyAsync(&c->dsc[0], &h, sizeof(h), cudaMemcpyHostToDevice, st));
-    cudaEvent_t ev0, ev1;
-    LQ_CUDA(c, cudaEventCreate(&ev0));
-    LQ_CUDA(c, cudaEventCreate(&ev1));
-    LQ_CUDA(c, cudaEventRecord(ev0, st));
+    LQ_CUDA(c, cudaEventRecord(c->ev0, st));
     long launches = 0, sweeps = 0;
     int fin = 0;
-    rc = lq_descent_run(&c->descent, method, (c->fire_path == 1 || lq_general_only(c->ph)) ? 1 : 0, g, c->ph, fields_of(c), buf, nbuf, &fin, c->dsc,
+    rc = lq_descent_run(&c->descent, method, c->fire_path == 1 ? 1 : 0, g, c->ph, fields_of(c), buf, nbuf, &fin, c->dsc,
                         dp->eta, dp->mu, force_tol, max_steps, st, &launches, &sweeps, &h, c->err);
-    if (rc == LQ_OK) {
-        cudaEventRecord(ev1, st);
-        cudaStreamSynchronize(st);
-    }
-    float ms = 0.f;
-    if (rc == LQ_OK) cudaEventElapsedTime(&ms, ev0, ev1);
-    cudaEventDestroy(ev0); cudaEventDestroy(ev1);
     if (rc != LQ_OK) return rc;
+    LQ_CUDA(c, cudaEventRecord(c->ev1, st));
+    LQ_CUDA(c, cudaStreamSynchronize(st));
+    float ms = 0.f;
+    cudaEventElapsedTime(&ms, c->ev0, c->ev1);
     // make the buffer that holds the last iterate the live one
     if (fin == 1) c->cur ^= 1;
     else if (fin == 2) { double *t = c->q[c->cur]; c->q[c->cur] = c->v[0]; c->v[0] = t; }
     // these minimisers carry no velocity; the velocity storage may have served as their third buffer
-    for (int i = 0; i < 2; ++i)
-        if (c->v[i]) LQ_CUDA(c, cudaMemsetAsync(c->v[i], 0, (size_t)5 * g.NP * sizeof(double), st));
+    c->v_valid = false;
     const double nsim = (double)(c->flags_active ? c->n_class[0] + c->n_class[1] : (unsigned long long)g.N);
     out->steps = (long)h.step; out->converged = h.converged;
     out->Fmax = h.Fmax; out->Frms = nsim > 0 ? sqrt(h.FF / nsim) : 0.0;

@@ -13,7 +13,17 @@
 
 constexpr int LQ_GH = 2;   // ghost width in x, y and z
 constexpr int LQ_XO = 16;  // element offset of x = 0 inside a padded row (128 B for fp64)
-constexpr int LQ_GW = 1;   // ghost width the FIRE kernels keep up to date (stencil radius)
+
+// Bond code of a site (one-constant masked sweeps; built once per lq_set_sites by k_bond_map): for the six directions
+// d = (+x, -x, +y, -y, +z, -z) two bits at 2d index the weight a^s_k(x) [w_k(x) + w_k(x + s k)] of that bond in the
+// gather-form force: 0 -> 0 (neighbour not simulated), 1 -> 1, 2 -> 3/2, 3 -> 2.
+constexpr unsigned LQ_BOND_PLAIN = 0x555u;       // all six bonds at weight 1: the constant 7-point stencil
+constexpr unsigned LQ_BOND_OBJECT = 1u << 12;    // the site itself is an object (no variables)
+constexpr unsigned LQ_BOND_ANCH = 1u << 13;      // class boundary and kind != 0: an anchoring term applies
+__host__ __device__ inline double lq_bond_weight(unsigned code, int d) {
+    const unsigned i = (code >> (2 * d)) & 3u;
+    return i == 0u ? 0.0 : 0.5 + 0.5 * (double)i;
+}
 
 struct LqGeom {
     int Lx, Ly, Lz;
@@ -36,8 +46,6 @@ struct LqPhys {
 };
 // the 19-point / general mixed-derivative code paths are needed as soon as any of L2, L3, L4 is non-zero
 __host__ __device__ inline bool lq_three(const LqPhys &ph) { return ph.L2 != 0.0 || ph.L3 != 0.0 || ph.L4 != 0.0 || ph.L6 != 0.0; }
-// terms the fused sweeps' constant-weight stencils do not carry: such runs use the general kernels
-__host__ __device__ inline bool lq_general_only(const LqPhys &) { return false; }
 
 // FIRE state that lives on the device (Algorithm 1).
 // mix_a, mix_b: the velocity rescale of the step just reduced, v <- mix_a*v + mix_b*F
@@ -51,6 +59,8 @@ struct LqFireScalars {
     int npos;
     int converged;
     double dt_prev;  // semi-implicit Euler variant: the dt of the step just scheduled (its drift uses it)
+    int init;        // 1: the next sweep is the initial force evaluation of the stored-force path (all step
+                     // coefficients 0: q' = q, vc' = 0, F' = force(q)); its reduction only runs the stop test
 };
 
 struct LqFireConsts {
@@ -108,6 +118,7 @@ __host__ __device__ inline void lq_fire_advance_euler(LqFireScalars &t, const Lq
 struct LqStepCoef { double dt, ma, cF, kick; };
 __host__ __device__ inline LqStepCoef lq_step_coef(const LqFireScalars &sc, const LqFireConsts &fc) {
     LqStepCoef k;
+    if (sc.init) { k.dt = k.ma = k.cF = k.kick = 0.0; return k; }
     k.ma = sc.mix_a;
     if (fc.euler) { k.dt = sc.dt_prev; k.cF = sc.mix_b; k.kick = sc.step < fc.max_steps ? sc.dt : 0.0; }
     else { k.dt = sc.dt; k.cF = sc.mix_b + 0.5 * sc.dt; k.kick = 0.5 * sc.dt; }
@@ -115,7 +126,21 @@ __host__ __device__ inline LqStepCoef lq_step_coef(const LqFireScalars &sc, cons
 }
 __host__ __device__ inline void lq_fire_advance_any(LqFireScalars &t, const LqFireConsts &fc, const double tot[4]) {
     if (fc.euler) lq_fire_advance_euler(t, fc, tot);
+    else if (t.init) { lq_fire_advance(t, fc, tot, 1); t.init = 0; t.mix_a = 0.0; t.mix_b = 0.0; }
     else lq_fire_advance(t, fc, tot, 0);
+}
+// First sweep of the recompute path (velocity Verlet): its phase 1 evaluates F(q) of the INITIAL state anyway, so the
+// stop test of Algorithm 1's initialisation ("if max|F| < tol return, steps = 0") rides on it:
+// tot0 = (|F(q_0)|^2, max|F_a(q_0)|).  If it passes (or no step was asked for) the step this sweep computed is
+// discarded (the caller does not flip buffers while step == 0); otherwise the step counts.
+__host__ __device__ inline void lq_fire_advance_first(LqFireScalars &t, const LqFireConsts &fc, const double tot[4],
+                                                      const double tot0[2]) {
+    if (tot0[1] < fc.force_tol || fc.max_steps == 0) {
+        t.P = 0.0; t.FF = tot0[0]; t.vv = 0.0; t.Fmax = tot0[1];
+        t.converged = tot0[1] < fc.force_tol ? 1 : 0;
+        return;
+    }
+    lq_fire_advance(t, fc, tot, 0);
 }
 
 struct LqFields {
@@ -155,3 +180,7 @@ void lq_launch_analyze(const LqGeom &g, const double *q, const uint8_t *flags, d
 void lq_launch_plain_map(const LqGeom &g, const uint8_t *flags, uint8_t *plain, cudaStream_t st);
 void lq_launch_tile_summary(const LqGeom &g, const uint8_t *plain, uint8_t *tsum, int TX, int TY, int ntx, int nty,
                             cudaStream_t st);
+void lq_launch_axpby(long long n, double a, const double *v, double b, const double *F, double *out, cudaStream_t st);
+void lq_launch_bond_map(const LqGeom &g, const uint8_t *flags, const uint8_t *kind, uint32_t *bond, cudaStream_t st);
+void lq_launch_tile_summary_bond(const LqGeom &g, const uint32_t *bond, uint8_t *tsum, int TX, int TY, int ntx, int nty,
+                                 cudaStream_t st);

@@ -285,13 +285,42 @@ __global__ void k_plain_map(LqGeom g, const uint8_t *__restrict__ flags, uint8_t
     plain[p] = ok ? 1 : ((flags[p] & 3u) == 2u ? 2 : 0);   // 1 plain, 0 non-plain simulated, 2 object
 }
 
+// Bond codes of the one-constant masked sweep (lq_internal.cuh LQ_BOND_*): per direction the weight
+// a^s_k(x) [w_k(x) + w_k(x + s k)] of the gather-form force, from the flag bytes
+// of the site and its six neighbours.  Interior plus a one-site ghost margin (flags carry a 2-wide ghost shell).
+__global__ void k_bond_map(LqGeom g, const uint8_t *__restrict__ flags, const uint8_t *__restrict__ kind,
+                           uint32_t *__restrict__ bond) {
+    const int x = (int)(blockIdx.x * blockDim.x + threadIdx.x) - 1;
+    const int y = (int)(blockIdx.y * blockDim.y + threadIdx.y) - 1;
+    const int z = (int)blockIdx.z - 1;
+    if (x > g.Lx || y > g.Ly) return;
+    const long long p = g.pidx(x, y, z);
+    const unsigned fl = flags[p];
+    unsigned code = 0;
+    if ((fl & 3u) == 2u) code = LQ_BOND_OBJECT;
+    else {
+        const long long off[6] = {1, -1, g.sy, -g.sy, g.sz, -g.sz};
+#pragma unroll
+        for (int d = 0; d < 6; ++d) {
+            if (!((fl >> (2 + d)) & 1u)) continue;
+            const int k = d >> 1;
+            const double w = lqs::w_axis(fl, k) + lqs::w_axis(flags[p + off[d]], k);     // 1, 3/2 or 2
+            code |= (w == 1.0 ? 1u : (w == 1.5 ? 2u : 3u)) << (2 * d);
+        }
+        if ((fl & 3u) == 1u && kind != nullptr && kind[p] != 0) code |= LQ_BOND_ANCH;
+    }
+    bond[p] = (uint32_t)code;
+}
+
 // tsum[(z+1)][by][bx] = 1 iff every site of tile (bx, by) plus its one-site halo is plain at plane z (z = -1 .. Lz)
-__global__ void k_tile_summary(LqGeom g, const uint8_t *__restrict__ plain, uint8_t *__restrict__ tsum, int TX, int TY) {
+template <typename T>
+__global__ void k_tile_summary(LqGeom g, const T *__restrict__ plain, unsigned plain_value, uint8_t *__restrict__ tsum,
+                               int TX, int TY) {
     const int bx = blockIdx.x, by = blockIdx.y, z = (int)blockIdx.z - 1;
     int ok = 1;
     for (int i = threadIdx.x; i < (TX + 2) * (TY + 2); i += blockDim.x) {
         const int x = bx * TX - 1 + i % (TX + 2), y = by * TY - 1 + i / (TX + 2);
-        if (x <= g.Lx && y <= g.Ly && plain[g.pidx(x, y, z)] != 1) ok = 0;
+        if (x <= g.Lx && y <= g.Ly && (unsigned)plain[g.pidx(x, y, z)] != plain_value) ok = 0;
     }
     ok = __syncthreads_and(ok);
     if (threadIdx.x == 0) tsum[((size_t)(z + 1) * gridDim.y + by) * gridDim.x + bx] = (uint8_t)ok;
@@ -357,11 +386,30 @@ void lq_launch_zero_object_sites(const LqGeom &g, const uint8_t *flags, double *
     k_zero_object_sites<<<plane_grid(g), dim3(BX, BY), 0, st>>>(g, flags, field);
 }
 
+// out = a v + b F over a whole padded 5-component field (lq_get_velocity: the FIRE rescale that the fused sweeps apply
+// lazily, Algorithm 1 "rescale velocity")
+__global__ void k_axpby(long long n, double a, const double *__restrict__ v, double b, const double *__restrict__ F,
+                        double *__restrict__ out) {
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x)
+        out[i] = a * v[i] + b * F[i];
+}
+void lq_launch_axpby(long long n, double a, const double *v, double b, const double *F, double *out, cudaStream_t st) {
+    k_axpby<<<148 * 8, 256, 0, st>>>(n, a, v, b, F, out);
+}
+
 void lq_launch_plain_map(const LqGeom &g, const uint8_t *flags, uint8_t *plain, cudaStream_t st) {
     dim3 b(64, 4), gr((g.Lx + 2 + 63) / 64, (g.Ly + 2 + 3) / 4, g.Lz + 2);
     k_plain_map<<<gr, b, 0, st>>>(g, flags, plain);
 }
 void lq_launch_tile_summary(const LqGeom &g, const uint8_t *plain, uint8_t *tsum, int TX, int TY, int ntx, int nty,
                             cudaStream_t st) {
-    k_tile_summary<<<dim3(ntx, nty, g.Lz + 2), 128, 0, st>>>(g, plain, tsum, TX, TY);
+    k_tile_summary<uint8_t><<<dim3(ntx, nty, g.Lz + 2), 128, 0, st>>>(g, plain, 1u, tsum, TX, TY);
+}
+void lq_launch_bond_map(const LqGeom &g, const uint8_t *flags, const uint8_t *kind, uint32_t *bond, cudaStream_t st) {
+    dim3 b(64, 4), gr((g.Lx + 2 + 63) / 64, (g.Ly + 2 + 3) / 4, g.Lz + 2);
+    k_bond_map<<<gr, b, 0, st>>>(g, flags, kind, bond);
+}
+void lq_launch_tile_summary_bond(const LqGeom &g, const uint32_t *bond, uint8_t *tsum, int TX, int TY, int ntx, int nty,
+                                 cudaStream_t st) {
+    k_tile_summary<uint32_t><<<dim3(ntx, nty, g.Lz + 2), 128, 0, st>>>(g, bond, LQ_BOND_PLAIN, tsum, TX, TY);
 }

@@ -27,7 +27,10 @@
 #include <cuda.h>
 #include <cstdio>
 #include <cstring>
-#include <cstdlib>
+#include <algorithm>
+#include <functional>
+#include <queue>
+#include <vector>
 
 namespace {
 using namespace lqsw;
@@ -195,25 +198,16 @@ k_sweep(const __grid_constant__ CUtensorMap tq, const __grid_constant__ CUtensor
                 }
             }
             const bool store_F = !(sim && !plain);
-            if (a.store_cs) {
 #pragma unroll
-                for (int c = 0; c < 5; ++c) {
-                    __stcs(a.qo + c * NP + p, qc[c]);
-                    __stcs(a.vo + c * NP + p, vn[c]);
-                    if (store_F) __stcs(a.Fo + c * NP + p, Fn[c]);
-                }
-            } else {
-#pragma unroll
-                for (int c = 0; c < 5; ++c) {
-                    a.qo[c * NP + p] = qc[c];
-                    a.vo[c * NP + p] = vn[c];
-                    if (store_F) a.Fo[c * NP + p] = Fn[c];
-                }
+            for (int c = 0; c < 5; ++c) {
+                a.qo[c * NP + p] = qc[c];
+                a.vo[c * NP + p] = vn[c];
+                if (store_F) a.Fo[c * NP + p] = Fn[c];
             }
-            // periodic ghost shell of the outputs (width LQ_GW)
-            const int shx = x < LQ_GW ? a.g.Lx : (x >= a.g.Lx - LQ_GW ? -a.g.Lx : 0);
-            const int shy = y < LQ_GW ? a.g.Ly : (y >= a.g.Ly - LQ_GW ? -a.g.Ly : 0);
-            const int shz = k < LQ_GW ? a.g.Lz : (k >= a.g.Lz - LQ_GW ? -a.g.Lz : 0);
+            // periodic ghost shell of the outputs, full width LQ_GH: whatever runs next on this state (the
+            // recompute sweep reads q with a 2-site halo) finds every ghost current
+            const int shx = ghost_shift(x, a.g.Lx, LQ_GH), shy = ghost_shift(y, a.g.Ly, LQ_GH),
+                      shz = ghost_shift(k, a.g.Lz, LQ_GH);
             if (shx | shy | shz) {
                 for (int m = 1; m < 8; ++m) {
                     if (((m & 1) && !shx) || ((m & 2) && !shy) || ((m & 4) && !shz)) continue;
@@ -257,13 +251,9 @@ bool make_map(CUtensorMap *m, const LqGeom &g, double *base, int bxw, int byh) {
     cuuint64_t strides[3] = {(cuuint64_t)g.Px * 8, (cuuint64_t)g.sz * 8, (cuuint64_t)g.NP * 8};
     cuuint32_t box[4] = {(cuuint32_t)bxw, (cuuint32_t)byh, 1, 5};
     cuuint32_t es[4] = {1, 1, 1, 1};
-    const char *pe = getenv("LQ_TMA_PROMO");
-    const int promo = pe ? atoi(pe) : 0;
-    const CUtensorMapL2promotion pr = promo == 3 ? CU_TENSOR_MAP_L2_PROMOTION_L2_256B
-                                    : promo == 2 ? CU_TENSOR_MAP_L2_PROMOTION_L2_128B
-                                    : promo == 1 ? CU_TENSOR_MAP_L2_PROMOTION_L2_64B : CU_TENSOR_MAP_L2_PROMOTION_NONE;
     return enc(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, base, dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
-               CU_TENSOR_MAP_SWIZZLE_NONE, pr, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+               CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) ==
+           CUDA_SUCCESS;
 }
 
 }  // namespace
@@ -274,33 +264,105 @@ struct LqSweepPlan {
     CUtensorMap mq[2], mv[2], mF[2];
     double *bq[2] = {nullptr, nullptr}, *bv[2] = {nullptr, nullptr}, *bF[2] = {nullptr, nullptr};
     bool three = false, stored = true;
-    double *partials = nullptr;
+    double *partials = nullptr, *partials0 = nullptr;
     unsigned int *counter = nullptr;
     uint8_t *plain = nullptr, *tsum = nullptr;   // masked lattices: per-site and per-(plane, tile) 'plain' maps
-    int *np_list = nullptr;                      // index-ordered non-plain simulated sites (fix-up kernel)
+    uint32_t *bond = nullptr;                    // recompute path on masked lattices: per-site bond codes
+    int *np_list = nullptr;                      // stored path: index-ordered non-plain simulated sites (fix-up kernel)
     int n_np = 0;
     double *partials2 = nullptr;
     unsigned int *counter2 = nullptr;
-    const uint8_t *flags_seen = nullptr;
+    const uint8_t *flags_seen = nullptr, *kind_seen = nullptr;
     bool sites_dirty = true;
-    dim3 grid;
+    dim3 grid;                                   // stored path: (tiles x, tiles y, z-chunks)
     int zc = 0;
-    bool attr_set[12] = {};
+    int4 *work = nullptr;                        // recompute path: work items, longest first
+    int n_items = 0, ntx = 0, nty = 0, chunks_forced = 0;
+    bool attr_set[12] = {}, attr_rc[4] = {};
 };
 
 void lq_sweep_destroy(LqSweepPlan *p) {
     if (!p) return;
     cudaFree(p->partials);
+    cudaFree(p->partials0);
     cudaFree(p->counter);
     cudaFree(p->plain);
     cudaFree(p->tsum);
+    cudaFree(p->bond);
     cudaFree(p->np_list);
     cudaFree(p->partials2);
     cudaFree(p->counter2);
+    cudaFree(p->work);
     delete p;
 }
 void lq_sweep_invalidate(LqSweepPlan *p) {
     if (p) p->sites_dirty = true;
+}
+
+// Work table of the recompute sweep: every tile column (ntiles of them, Lz planes each) is cut into z-chunks; a
+// CTA pays its chunk plus `ovh` planes of halo and pipeline fill, one CTA per SM.  With few tiles per SM, equal
+// chunks waste most of the last wave (config 5: 650 equal CTAs on 148 SMs = 4.4 waves of work in 5), so the first
+// Ta tiles get na chunks and the rest nb >= na chunks, items are ordered longest first -- the hardware hands CTA
+// ids out in order as SMs free up, i.e. longest-processing-time list scheduling -- and (Ta, na, nb) minimise the
+// simulated makespan.  Large grids (many waves) keep equal chunks of <= 64 planes.
+std::vector<int4> lq_build_chunk_table(int ntx, int nty, int Lz, int max_chunk, int ovh, int nsm, int force_n) {
+    const int T = ntx * nty;
+    auto chunks = [&](int n, int i, int &zb, int &ze) {      // i-th of n near-equal chunks of [0, Lz)
+        zb = (int)((long long)Lz * i / n); ze = (int)((long long)Lz * (i + 1) / n);
+    };
+    const int n_min = (Lz + max_chunk - 1) / max_chunk;      // fewest chunks per column
+    const int n_max = Lz >= 8 ? Lz / 4 : 1;                   // chunks of at least 4 planes
+    int best_na = (Lz + 63) / 64, best_nb = best_na, best_Ta = T;
+    if (best_na > n_max) best_na = best_nb = n_max;
+    if (best_na < n_min) best_na = best_nb = n_min;
+    if (force_n > 0) {                                        // "rc_chunks" option: n equal chunks per column
+        best_na = best_nb = std::min(std::max(force_n, n_min), std::max(n_max, n_min));
+    } else if ((long long)T * best_na < 10LL * nsm) {
+        double best = -1.0;
+        std::vector<long long> load(nsm);
+        auto makespan = [&](int Ta, int na, int nb) -> double {
+            // items: Ta*na of cost ~Lz/na + ovh, (T-Ta)*nb of cost ~Lz/nb + ovh; greedy on the least-loaded SM
+            std::vector<int> cost;
+            cost.reserve((size_t)Ta * na + (size_t)(T - Ta) * nb);
+            for (int t = 0; t < T; ++t) {
+                const int n = t < Ta ? na : nb;
+                for (int i = 0; i < n; ++i) { int zb, ze; chunks(n, i, zb, ze); cost.push_back(ze - zb + ovh); }
+            }
+            std::sort(cost.begin(), cost.end(), std::greater<int>());
+            std::priority_queue<long long, std::vector<long long>, std::greater<long long>> pq;
+            for (int i = 0; i < nsm; ++i) pq.push(0);
+            long long mk = 0;
+            for (int c : cost) { long long l = pq.top() + c; pq.pop(); pq.push(l); if (l > mk) mk = l; }
+            return (double)mk;
+        };
+        for (int na = n_min; na <= n_max && na <= n_min + 24; ++na)
+            for (int nb = na; nb <= n_max && nb <= 4 * na + 4; ++nb) {
+                for (int Ta = 0; Ta <= T; Ta += (Ta + nsm <= T ? nsm : (Ta < T ? T - Ta : 1))) {
+                    if (nb == na && Ta != T) continue;
+                    if ((long long)Ta * na + (long long)(T - Ta) * nb > 40LL * nsm) continue;
+                    const double m = makespan(Ta, na, nb);
+                    if (best < 0.0 || m < best) { best = m; best_na = na; best_nb = nb; best_Ta = Ta; }
+                }
+            }
+    }
+    std::vector<int4> items;
+    for (int t = 0; t < T; ++t) {
+        const int n = t < best_Ta ? best_na : best_nb;
+        for (int i = 0; i < n; ++i) {
+            int zb, ze;
+            chunks(n, i, zb, ze);
+            if (ze > zb) items.push_back(make_int4(t % ntx, t / ntx, zb, ze));
+        }
+    }
+    // longest first; equal lengths: by z-chunk, then row-major tiles (x-neighbours share halo rows in L2)
+    std::stable_sort(items.begin(), items.end(), [](const int4 &a, const int4 &b) {
+        const int la = a.w - a.z, lb = b.w - b.z;
+        if (la != lb) return la > lb;
+        if (a.z != b.z) return a.z < b.z;
+        if (a.y != b.y) return a.y < b.y;
+        return a.x < b.x;
+    });
+    return items;
 }
 
 template <class C, bool THREE, bool MASKED, int XT = 0>
@@ -315,9 +377,18 @@ static cudaError_t launch(LqSweepPlan *pl, int in, const SweepArgs &a, int varia
     return cudaGetLastError();
 }
 
+#define LQ_PLAN_CUDA(call)                                                                   \
+    do {                                                                                     \
+        cudaError_t e_ = (call);                                                             \
+        if (e_ != cudaSuccess) {                                                             \
+            err = std::string("lq_sweep: " #call ": ") + cudaGetErrorString(e_);             \
+            return e_ == cudaErrorMemoryAllocation ? LQ_ERR_NOMEM : LQ_ERR_CUDA;             \
+        }                                                                                    \
+    } while (0)
+
 int lq_sweep_run(LqSweepPlan **planp, bool stored_F, const LqGeom &g, const LqPhys &ph, const LqFields &f, double *q[2],
                  double *v[2], double *F[2], int *cur, LqFireScalars *dsc, const LqFireConsts &fc, long max_steps,
-                 cudaStream_t st, long *launches, long *sweeps, LqFireScalars *h, std::string &err) {
+                 cudaStream_t st, long *launches, long *sweeps, LqFireScalars *h, std::string &err, int rc_chunks) {
     using C1 = Cfg<32, 16>;   // one-constant: 512 threads, <= 128 registers
     using C3 = Cfg<32, 16>;   // three-constant: same tile (ptxas fits the 19-point fast path in 128 registers)
     const bool three = lq_three(ph);
@@ -329,8 +400,9 @@ int lq_sweep_run(LqSweepPlan **planp, bool stored_F, const LqGeom &g, const LqPh
     }
     if (three && !stored_F) { err = "lq_sweep: the recompute path is one-constant only"; return LQ_ERR_ARG; }
     const int TX = 32, TY = !stored_F ? lq_sweep_rc_tile(1) : (three ? C3::TY : C1::TY);
-    bool rebuild = pl->three != three || pl->stored != stored_F || pl->partials == nullptr;
-    for (int i = 0; i < 2; ++i) rebuild |= pl->bq[i] != q[i] || pl->bv[i] != v[i] || pl->bF[i] != F[i];
+    bool rebuild = pl->three != three || pl->stored != stored_F || pl->partials == nullptr || pl->chunks_forced != rc_chunks;
+    pl->chunks_forced = rc_chunks;
+    for (int i = 0; i < 2; ++i) rebuild |= pl->bq[i] != q[i] || pl->bv[i] != v[i] || (stored_F && pl->bF[i] != F[i]);
     if (rebuild) {
         for (int i = 0; i < 2; ++i) {
             const bool ok = stored_F
@@ -347,75 +419,93 @@ int lq_sweep_run(LqSweepPlan **planp, bool stored_F, const LqGeom &g, const LqPh
         pl->three = three;
         pl->stored = stored_F;
         const int ntx = (g.Lx + TX - 1) / TX, nty = (g.Ly + TY - 1) / TY;
-        // z-chunk: >= 4 planes (small lattices want many short chunks: the machine is otherwise empty), <= 64
-        // z-chunking: equal chunks; pick the chunk count that minimises the modelled makespan
-        //   waves(ntiles * nzc / 148 SMs, 1 CTA/SM) * (planes per chunk + halo planes + pipeline fill)
-        const int halo_planes = stored_F ? 2 : 4;
-        long long best = -1;
-        int zc = g.Lz;
-        for (int nzc = 1; nzc <= (g.Lz + 3) / 4; ++nzc) {
-            const int c = (g.Lz + nzc - 1) / nzc;
-            if (c > 64 && nzc < (g.Lz + 63) / 64) continue;
-            const long long ncta = (long long)ntx * nty * ((g.Lz + c - 1) / c);
-            const long long cost = ((ncta + 147) / 148) * (c + halo_planes + 3);
-            if (best < 0 || cost < best) { best = cost; zc = c; }
+        pl->ntx = ntx; pl->nty = nty;
+        size_t ncta;
+        if (stored_F) {
+            // equal z-chunks of <= 64 planes; the chunk count minimises the modelled makespan
+            //   waves(ntiles * nzc / 148 SMs, 1 CTA/SM) * (planes per chunk + halo planes + pipeline fill)
+            long long best = -1;
+            int zc = g.Lz;
+            for (int nzc = 1; nzc <= (g.Lz + 3) / 4; ++nzc) {
+                const int c = (g.Lz + nzc - 1) / nzc;
+                if (c > 64 && nzc < (g.Lz + 63) / 64) continue;
+                const long long n = (long long)ntx * nty * ((g.Lz + c - 1) / c);
+                const long long cost = ((n + 147) / 148) * (c + 2 + 3);
+                if (best < 0 || cost < best) { best = cost; zc = c; }
+            }
+            pl->zc = zc;
+            pl->grid = dim3(ntx, nty, (g.Lz + zc - 1) / zc);
+            ncta = (size_t)pl->grid.x * pl->grid.y * pl->grid.z;
+        } else {
+            int nsm = 148;
+            int dev = 0;
+            if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
+            const std::vector<int4> items = lq_build_chunk_table(ntx, nty, g.Lz, lq_sweep_rc_max_chunk(), 7, nsm, rc_chunks);
+            cudaFree(pl->work); pl->work = nullptr;
+            LQ_PLAN_CUDA(cudaMalloc(&pl->work, items.size() * sizeof(int4)));
+            // pageable host source: the copy is staged before the call returns, `items` may go out of scope
+            LQ_PLAN_CUDA(cudaMemcpyAsync(pl->work, items.data(), items.size() * sizeof(int4), cudaMemcpyHostToDevice, st));
+            pl->n_items = (int)items.size();
+            ncta = items.size();
         }
-        if (getenv("LQ_ZC")) zc = atoi(getenv("LQ_ZC"));
-        if (zc > g.Lz) zc = g.Lz;
-        pl->zc = zc;
-        pl->grid = dim3(ntx, nty, (g.Lz + zc - 1) / zc);
-        cudaFree(pl->partials); cudaFree(pl->counter);
-        pl->partials = nullptr; pl->counter = nullptr;
-        const size_t ncta = (size_t)pl->grid.x * pl->grid.y * pl->grid.z;
-        if (cudaMalloc(&pl->partials, ncta * 4 * sizeof(double)) != cudaSuccess ||
-            cudaMalloc(&pl->counter, sizeof(unsigned int)) != cudaSuccess) {
-            err = "lq_sweep: cudaMalloc failed";
-            return LQ_ERR_NOMEM;
-        }
+        cudaFree(pl->partials); cudaFree(pl->partials0); cudaFree(pl->counter);
+        pl->partials = pl->partials0 = nullptr; pl->counter = nullptr;
+        LQ_PLAN_CUDA(cudaMalloc(&pl->partials, ncta * 4 * sizeof(double)));
+        LQ_PLAN_CUDA(cudaMalloc(&pl->partials0, ncta * 2 * sizeof(double)));
+        LQ_PLAN_CUDA(cudaMalloc(&pl->counter, sizeof(unsigned int)));
     }
-    if (masked && (pl->sites_dirty || rebuild || pl->flags_seen != f.flags)) {
-        const size_t nts = (size_t)pl->grid.x * pl->grid.y * (g.Lz + 2);
-        if (!pl->plain && cudaMalloc(&pl->plain, (size_t)g.NP) != cudaSuccess) { err = "lq_sweep: cudaMalloc failed"; return LQ_ERR_NOMEM; }
+    if (masked && (pl->sites_dirty || rebuild || pl->flags_seen != f.flags || pl->kind_seen != f.kind)) {
+        const size_t nts = (size_t)pl->ntx * pl->nty * (g.Lz + 2);
         cudaFree(pl->tsum); pl->tsum = nullptr;
-        if (cudaMalloc(&pl->tsum, nts) != cudaSuccess) { err = "lq_sweep: cudaMalloc failed"; return LQ_ERR_NOMEM; }
-        cudaMemsetAsync(pl->plain, 0, (size_t)g.NP, st);
-        lq_launch_plain_map(g, f.flags, pl->plain, st);
-        lq_launch_tile_summary(g, pl->plain, pl->tsum, TX, TY, pl->grid.x, pl->grid.y, st);
+        LQ_PLAN_CUDA(cudaMalloc(&pl->tsum, nts));
+        if (stored_F) {
+            if (!pl->plain) LQ_PLAN_CUDA(cudaMalloc(&pl->plain, (size_t)g.NP));
+            LQ_PLAN_CUDA(cudaMemsetAsync(pl->plain, 0, (size_t)g.NP, st));
+            lq_launch_plain_map(g, f.flags, pl->plain, st);
+            lq_launch_tile_summary(g, pl->plain, pl->tsum, TX, TY, pl->ntx, pl->nty, st);
+            if (lq_fixup_build_list(g, f.flags, pl->plain, &pl->np_list, &pl->n_np, st) != 0) { err = "lq_sweep: building the non-plain site list failed"; return LQ_ERR_NOMEM; }
+            cudaFree(pl->partials2); pl->partials2 = nullptr;
+            LQ_PLAN_CUDA(cudaMalloc(&pl->partials2, (size_t)4 * lq_fixup_num_blocks(pl->n_np) * sizeof(double)));
+            if (!pl->counter2) LQ_PLAN_CUDA(cudaMalloc(&pl->counter2, sizeof(unsigned int)));
+            LQ_PLAN_CUDA(cudaMemsetAsync(pl->counter2, 0, sizeof(unsigned int), st));
+        } else {
+            if (!pl->bond) LQ_PLAN_CUDA(cudaMalloc(&pl->bond, (size_t)g.NP * sizeof(uint32_t)));
+            LQ_PLAN_CUDA(cudaMemsetAsync(pl->bond, 0, (size_t)g.NP * sizeof(uint32_t), st));
+            lq_launch_bond_map(g, f.flags, f.kind, pl->bond, st);
+            lq_launch_tile_summary_bond(g, pl->bond, pl->tsum, TX, TY, pl->ntx, pl->nty, st);
+        }
         *launches += 2;
-        if (lq_fixup_build_list(g, f.flags, pl->plain, &pl->np_list, &pl->n_np, st) != 0) { err = "lq_sweep: building the non-plain site list failed"; return LQ_ERR_NOMEM; }
-        cudaFree(pl->partials2); pl->partials2 = nullptr;
-        if (cudaMalloc(&pl->partials2, (size_t)4 * lq_fixup_num_blocks(pl->n_np) * sizeof(double)) != cudaSuccess ||
-            (!pl->counter2 && cudaMalloc(&pl->counter2, sizeof(unsigned int)) != cudaSuccess)) { err = "lq_sweep: cudaMalloc failed"; return LQ_ERR_NOMEM; }
-        cudaMemsetAsync(pl->counter2, 0, sizeof(unsigned int), st);
         pl->sites_dirty = false;
         pl->flags_seen = f.flags;
+        pl->kind_seen = f.kind;
     }
-    cudaError_t e = cudaMemsetAsync(pl->counter, 0, sizeof(unsigned int), st);
-    if (e != cudaSuccess) { err = cudaGetErrorString(e); return LQ_ERR_CUDA; }
-    if (stored_F || masked) {   // F of the entry state was written by the generic kernel without its ghost shell
-        lq_launch_fill_ghosts_f64(g, F[*cur], 5, st);
-        *launches += 1;
-    }
-    if (fc.euler) {             // Euler variant: the entry velocity already carries the first kick (interior only)
-        lq_launch_fill_ghosts_f64(g, v[*cur], 5, st);
-        *launches += 1;
-    }
+    LQ_PLAN_CUDA(cudaMemsetAsync(pl->counter, 0, sizeof(unsigned int), st));
 
     const int cur0 = *cur;
     SweepArgs a;
+    memset(&a, 0, sizeof(a));
     a.g = g; a.ph = ph; a.f = f; a.sc = dsc; a.fc = fc; a.partials = pl->partials; a.counter = pl->counter; a.zc = pl->zc;
-    a.store_cs = getenv("LQ_STORE_CS") ? atoi(getenv("LQ_STORE_CS")) : 0;
-    a.plain = pl->plain; a.tsum = pl->tsum;
-    a.defer_advance = masked ? 1 : 0;
-    const int ncta = (int)(pl->grid.x * pl->grid.y * pl->grid.z);
+    a.plain = pl->plain; a.tsum = pl->tsum; a.bond = pl->bond; a.work = pl->work; a.ntx = pl->ntx; a.nty = pl->nty;
+    a.partials0 = pl->partials0;
+    a.defer_advance = (masked && stored_F) ? 1 : 0;
+    const int ncta = stored_F ? (int)(pl->grid.x * pl->grid.y * pl->grid.z) : pl->n_items;
+    // Sweeps to enqueue and buffer flips per step taken.  Recompute path, velocity Verlet: the first sweep also
+    // carries the stop test on the initial state, so `max_steps` sweeps (one even if max_steps == 0) and the live
+    // buffer flips once per counted step.  Stored path: one extra leading sweep evaluates F(q_0) (all coefficients
+    // 0); Euler variant (either path): one extra sweep because every sweep is [drift of the scheduled step |
+    // force | kick of the next one].  Those flip once more than steps were counted.
+    const bool extra = stored_F || fc.euler;
+    const long total = extra ? max_steps + 1 : (max_steps > 0 ? max_steps : 1);
     const long chunk = fc.force_tol > 0.0 ? 100 : (1L << 30);
+    cudaError_t e = cudaSuccess;
     long done = 0;
-    while (done < max_steps) {
-        const long n = (max_steps - done) < chunk ? (max_steps - done) : chunk;
+    while (done < total) {
+        const long n = (total - done) < chunk ? (total - done) : chunk;
         for (long i = 0; i < n; ++i) {
             const int in = (int)((cur0 + done + i) & 1), out = in ^ 1;
-            a.qo = q[out]; a.vo = v[out]; a.Fo = F[out]; a.Fi = F[in];
-            if (!stored_F) e = lq_launch_sweep_rc(masked, pl->grid, pl->mq[in], pl->mv[in], a, st);
+            a.qo = q[out]; a.vo = v[out]; a.Fo = F[out];
+            if (!stored_F)
+                e = lq_launch_sweep_rc(masked, !fc.euler && done + i == 0, ncta, pl->attr_rc, pl->mq[in], pl->mv[in], a, st);
             else if (three && (ph.L4 != 0.0 || ph.L6 != 0.0)) {
                 const int xt = (ph.L4 != 0.0 ? 1 : 0) | (ph.L6 != 0.0 ? 2 : 0);
                 if (xt == 1) e = masked ? launch<C3, true, true, 1>(pl, in, a, 5, st) : launch<C3, true, false, 1>(pl, in, a, 4, st);
@@ -424,23 +514,21 @@ int lq_sweep_run(LqSweepPlan **planp, bool stored_F, const LqGeom &g, const LqPh
             }
             else if (three) e = masked ? launch<C3, true, true>(pl, in, a, 3, st) : launch<C3, true, false>(pl, in, a, 2, st);
             else e = masked ? launch<C1, false, true>(pl, in, a, 1, st) : launch<C1, false, false>(pl, in, a, 0, st);
-            if (e == cudaSuccess && masked)
+            if (e == cudaSuccess && masked && stored_F)
                 e = lq_launch_fixup(three, g, ph, f, q[out], v[out], F[out], pl->np_list, pl->n_np, dsc, fc, pl->partials,
                                     ncta, pl->partials2, pl->counter2, st);
             if (e != cudaSuccess) { err = std::string("lq_sweep launch: ") + cudaGetErrorString(e); return LQ_ERR_CUDA; }
         }
         done += n;
-        *launches += masked ? 2 * n : n; *sweeps += n;
+        *launches += (masked && stored_F) ? 2 * n : n; *sweeps += n;
         if (fc.force_tol > 0.0) {
-            e = cudaMemcpyAsync(h, dsc, sizeof(*h), cudaMemcpyDeviceToHost, st);
-            if (e == cudaSuccess) e = cudaStreamSynchronize(st);
-            if (e != cudaSuccess) { err = std::string("lq_sweep: ") + cudaGetErrorString(e); return LQ_ERR_CUDA; }
+            LQ_PLAN_CUDA(cudaMemcpyAsync(h, dsc, sizeof(*h), cudaMemcpyDeviceToHost, st));
+            LQ_PLAN_CUDA(cudaStreamSynchronize(st));
             if (h->converged) break;
         }
     }
-    e = cudaMemcpyAsync(h, dsc, sizeof(*h), cudaMemcpyDeviceToHost, st);
-    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
-    if (e != cudaSuccess) { err = std::string("lq_sweep: ") + cudaGetErrorString(e); return LQ_ERR_CUDA; }
-    *cur = (int)((cur0 + h->step) & 1);
+    LQ_PLAN_CUDA(cudaMemcpyAsync(h, dsc, sizeof(*h), cudaMemcpyDeviceToHost, st));
+    LQ_PLAN_CUDA(cudaStreamSynchronize(st));
+    *cur = (int)((cur0 + h->step + (extra ? 1 : 0)) & 1);
     return LQ_OK;
 }

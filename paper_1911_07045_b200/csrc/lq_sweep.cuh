@@ -8,14 +8,16 @@ struct LqSweepPlan;  // tensor maps, per-CTA partials, tile classification; owne
 void lq_sweep_destroy(LqSweepPlan *plan);
 void lq_sweep_invalidate(LqSweepPlan *plan);  // geometry / anchoring arrays changed
 
-// Runs up to max_steps FIRE steps, one kernel launch per step.  On entry buffer *cur holds
-// (q, v = 0, F = force(q)) with q's ghost shell valid and dsc[0] the scalars after the step-0
-// update.  On return *cur is the buffer holding the final state, *h the final scalars.
+// Runs up to max_steps FIRE steps, one kernel launch per step, INCLUDING Algorithm 1's initialisation (force of
+// the initial state and the stop test on it): there is no separate first pass.  On entry buffer *cur holds q with
+// its ghost shell valid (v and F need not be initialised) and dsc[0] the initial scalars (dt = dt0, alpha0,
+// mix_a = mix_b = 0, step = 0; init = 1 for the stored path with velocity Verlet).  On return *cur is the buffer
+// holding the final state, *h the final scalars.
 // stored_F: true = state (q, vc, F), 240 B/site (any elastic constants); false = state (q, vc) with the force
-// recomputed, 160 B/site (one-constant only).
+// recomputed, 160 B/site (one-constant only; masked lattices included, no second kernel).
 int lq_sweep_run(LqSweepPlan **plan, bool stored_F, const LqGeom &g, const LqPhys &ph, const LqFields &f, double *q[2],
                  double *v[2], double *F[2], int *cur, LqFireScalars *dsc, const LqFireConsts &fc, long max_steps,
-                 cudaStream_t st, long *launches, long *sweeps, LqFireScalars *h, std::string &err);
+                 cudaStream_t st, long *launches, long *sweeps, LqFireScalars *h, std::string &err, int rc_chunks = 0);
 
 // gradient descent / Nesterov (lq_descent.cu): one launch per step; buf[0] holds q_0, nbuf rotating buffers
 struct LqDescentPlan;
@@ -34,8 +36,11 @@ void lq_descent_invalidate(LqDescentPlan *plan);   // geometry / anchoring array
 namespace lqsw { struct SweepArgs; }
 int lq_sweep_rc_box(int which, int dim);
 int lq_sweep_rc_tile(int dim);
-cudaError_t lq_launch_sweep_rc(bool masked, dim3 grid, const CUtensorMap &mq, const CUtensorMap &mv,
-                               const lqsw::SweepArgs &a, cudaStream_t st);
+int lq_sweep_rc_max_chunk();
+// first: the first sweep of a call (velocity Verlet): also reduces the stop test on the initial state.
+// attr_set[4]: per-plan record of which instantiations had their shared-memory attribute set (per device).
+cudaError_t lq_launch_sweep_rc(bool masked, bool first, int ncta, bool *attr_set, const CUtensorMap &mq,
+                               const CUtensorMap &mv, const lqsw::SweepArgs &a, cudaStream_t st);
 
 // fix-up kernel for the non-plain sites of masked lattices (lq_fixup.cu)
 int lq_fixup_build_list(const LqGeom &g, const uint8_t *flags, const uint8_t *plain, int **list, int *n, cudaStream_t st);

@@ -16,11 +16,14 @@ struct SweepArgs {
     double *partials;
     unsigned int *counter;
     int zc;
-    int store_cs;           // stored-force sweep: 1 = streaming (evict-first) stores of the outputs (LQ_STORE_CS; measured neutral)
-    const uint8_t *plain;   // per-site 'constant stencil weights' byte (masked lattices)
+    const uint8_t *plain;   // stored-force sweep, masked lattices: per-site 'constant stencil weights' byte
     const uint8_t *tsum;    // per (plane, tile): tile + halo all plain
-    const double *Fi;       // masked recompute sweep: stored force of the NON-plain sites (input buffer)
-    int defer_advance;      // masked lattices: the fix-up kernel (lq_fixup.cu) finishes the step
+    int defer_advance;      // stored-force sweep on masked lattices: the fix-up kernel (lq_fixup.cu) finishes the step
+    // recompute sweep (lq_sweep_rc.cu)
+    const uint32_t *bond;   // masked lattices: per-site bond code (LQ_BOND_*), ghost margin of 1 filled
+    const int4 *work;       // work items (tile x, tile y, first plane, end plane), longest first; one per CTA
+    int ntx, nty;           // tiles per row / column (indexing of tsum)
+    double *partials0;      // first sweep: per-CTA (|F(q_0)|^2, max|F_a(q_0)|) of the initial state
 };
 
 // ---------------------------------------------------------------- PTX wrappers (TMA + mbarrier)
@@ -53,6 +56,13 @@ __device__ __forceinline__ void tma_load_4d(void *dst, const CUtensorMap *map, u
         : "memory");
 }
 
+// 4-byte global -> shared copy that bypasses the register file (LDGSTS); commit / wait by group
+__device__ __forceinline__ void cp_async_4(void *dst, const void *src) {
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(smem_u32(dst)), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void cp_async_wait_but_one() { asm volatile("cp.async.wait_group 1;" ::: "memory"); }
+
 __device__ __forceinline__ double warp_sum(double v) {
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
@@ -68,9 +78,12 @@ __device__ __forceinline__ double warp_max(double v) {
 // q' and v_k of one site from (q, vc, F): v_k = mix_a vc + (mix_b + dt/2) F ; q' = q + dt v_k.
 // The SAME instruction sequence serves a CTA's own sites and the halo copies its neighbours compute,
 // so every CTA sees bit-identical q'.
+// ma == 0 (first step of a call, or after a P <= 0 reset) drops vc without reading its value, so a velocity
+// buffer that was never written (or holds an earlier run's NaN) cannot leak in; likewise cF == 0 and F.
 __device__ __forceinline__ void drift(double q, double vc, double F, double ma, double cF, double dt, double &vk,
                                       double &qn) {
-    vk = __fma_rn(ma, vc, cF * F);
+    const double kF = cF == 0.0 ? 0.0 : cF * F;
+    vk = ma == 0.0 ? kF : __fma_rn(ma, vc, kF);
     qn = __fma_rn(dt, vk, q);
 }
 
@@ -80,19 +93,34 @@ __device__ __forceinline__ int ghost_shift(int i, int L, int gw) { return i < gw
 // End of a sweep: block-reduce r = (P, FF, vv, Fmax) partials, publish them, and let the LAST CTA to finish
 // reduce all CTAs' partials in index order (bitwise reproducible) and advance the FIRE schedule
 // (Algorithm 1) in place.  red: >= 4*NT/32 doubles of shared memory.
-template <int NT>
-__device__ __forceinline__ void finish_step(const SweepArgs &a, const LqFireScalars &sc, const double r[4], double *red) {
+// FIRST (recompute path, first sweep of a call): r0 = (|F(q_0)|^2, max|F_a(q_0)|) of the initial state is reduced
+// the same way and decides Algorithm 1's stop test on the initial state (lq_fire_advance_first).
+template <int NT, bool FIRST = false>
+__device__ __forceinline__ void finish_step(const SweepArgs &a, const LqFireScalars &sc, const double r[4], double *red,
+                                            const double *r0 = nullptr) {
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     constexpr int NW = NT / 32;
+    __shared__ unsigned s_last;
+    __shared__ double s_tot0[2];
+    const unsigned ncta = gridDim.x * gridDim.y * gridDim.z;
+    const unsigned cta = blockIdx.x + gridDim.x * (blockIdx.y + gridDim.y * blockIdx.z);
+    if (FIRST) {
+        const double w0 = warp_sum(r0[0]), w1 = warp_max(r0[1]);
+        if (lane == 0) { red[wid] = w0; red[NW + wid] = w1; }
+        __syncthreads();
+        if (tid == 0) {
+            double t0 = red[0], t1 = red[NW];
+            for (int w = 1; w < NW; ++w) { t0 += red[w]; t1 = fmax(t1, red[NW + w]); }
+            a.partials0[2 * cta] = t0; a.partials0[2 * cta + 1] = t1;
+        }
+        __syncthreads();
+    }
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
         const double w = i < 3 ? warp_sum(r[i]) : warp_max(r[i]);
         if (lane == 0) red[i * NW + wid] = w;
     }
     __syncthreads();
-    __shared__ unsigned s_last;
-    const unsigned ncta = gridDim.x * gridDim.y * gridDim.z;
-    const unsigned cta = blockIdx.x + gridDim.x * (blockIdx.y + gridDim.y * blockIdx.z);
     if (tid == 0) {
         double t[4];
 #pragma unroll
@@ -110,6 +138,19 @@ __device__ __forceinline__ void finish_step(const SweepArgs &a, const LqFireScal
     __syncthreads();
     if (!s_last) return;
     __threadfence();
+    if (FIRST) {
+        double t0 = 0.0, t1 = 0.0;
+        for (unsigned b = tid; b < ncta; b += NT) { t0 += __ldcg(a.partials0 + 2 * b); t1 = fmax(t1, __ldcg(a.partials0 + 2 * b + 1)); }
+        t0 = warp_sum(t0); t1 = warp_max(t1);
+        if (lane == 0) { red[wid] = t0; red[NW + wid] = t1; }
+        __syncthreads();
+        if (tid == 0) {
+            double u0 = red[0], u1 = red[NW];
+            for (int w = 1; w < NW; ++w) { u0 += red[w]; u1 = fmax(u1, red[NW + w]); }
+            s_tot0[0] = u0; s_tot0[1] = u1;
+        }
+        __syncthreads();
+    }
     double t[4] = {0.0, 0.0, 0.0, 0.0};
     for (unsigned b = tid; b < ncta; b += NT) {
         t[0] += __ldcg(a.partials + 4 * b); t[1] += __ldcg(a.partials + 4 * b + 1); t[2] += __ldcg(a.partials + 4 * b + 2);
@@ -129,7 +170,8 @@ __device__ __forceinline__ void finish_step(const SweepArgs &a, const LqFireScal
             for (int w = 1; w < NW; ++w) tot[i] = i < 3 ? tot[i] + red[i * NW + w] : fmax(tot[i], red[i * NW + w]);
         }
         LqFireScalars nx = sc;
-        lq_fire_advance_any(nx, a.fc, tot);
+        if (FIRST) lq_fire_advance_first(nx, a.fc, tot, s_tot0);
+        else lq_fire_advance_any(nx, a.fc, tot);
         *a.sc = nx;
         *a.counter = 0u;
     }

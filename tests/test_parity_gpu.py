@@ -101,11 +101,76 @@ def test_q_after_100_fire_steps(case, lq, path):
     assert abs(rep["dt"] - rref["dt"]) <= 1e-15 and abs(rep["alpha"] - rref["alpha"]) <= 1e-15
     assert abs(rep["Fmax"] - rref["Fmax"]) <= 1e-7 * max(rref["Fmax"], 1e-3)
     assert abs(rep["P"] - rref["P"]) <= 1e-6 * max(abs(rref["P"]), 1e-6)
+    # velocities: Algorithm 1's v at the end of the step, i.e. after the rescale (lq.h, lq_get_velocity)
+    assert np.abs(v - vref).max() <= 1e-7 * max(np.abs(vref).max(), 1e-3), "%s: v err %.3e" % (name, np.abs(v - vref).max())
     if c["mask"] is not None:
         obj = c["mask"] == 1
         assert np.array_equal(q[:, obj], c["q"][:, obj])       # object sites never move (R17)
         assert np.abs(v[:, obj]).max(initial=0.0) == 0.0
     lq.lq_set_option(ctx, "fire_path", 0)
+
+
+@pytest.mark.parametrize("name", ["masked_70x35x9_L1only", "masked_37x21x11", "replica5p"])
+def test_anchoring_records_off_boundary_are_ignored(lq, oracle_mod, name):
+    """SURVEY 8(c) O5 / DESIGN.md R9: an anchoring term exists iff class == boundary and kind != 0.  Here EVERY site
+    (bulk, boundary, object) carries a record with kind in {1, 2}; forces, energy and 100 FIRE steps (fused sweeps,
+    both the recompute and the stored-force path) must equal the oracle's, which is pinned to ignore the records
+    off the boundary class (tests/test_oracle_pins.py::test_anchoring_only_on_boundary_class_sites)."""
+    c = dict(SMALL_CASES[name]())
+    rng = np.random.default_rng(4242)
+    N = c["N"]
+    c["kind"] = rng.integers(1, 3, size=N).astype(np.uint8)
+    c["W"] = 0.2 + 3.0 * rng.random(N)
+    ax = rng.standard_normal((3, N))
+    c["axis"] = ax / np.linalg.norm(ax, axis=0, keepdims=True)
+    ctx = lq.create_from_config(c)
+    o = make_oracle(oracle_mod, c)
+    Fref = o.forces(c["q"], 1)
+    assert np.abs(lq.lq_forces(ctx) - Fref).max() <= TOL_F * np.abs(Fref).max()
+    eref = o.energy(c["q"], 1)
+    assert abs(lq.lq_energy(ctx) - eref) <= TOL_E * abs(eref)
+    qref, _ = o.fire(c["q"], 100, 0.0, c["fire"], variant=1)
+    for path in (0, 2):
+        lq.lq_set_option(ctx, "fire_path", path)
+        lq.lq_set_Q(ctx, c["q"])
+        lq.lq_fire_minimize(ctx, 100, 0.0, c["fire"])
+        assert np.abs(lq.lq_get_Q(ctx) - qref).max() <= TOL_Q100
+    lq.lq_destroy(ctx)
+
+
+@pytest.mark.parametrize("name", ["replica4", "masked_70x35x9_L1only"])
+def test_stored_path_then_recompute_path_without_set_Q(lq, oracle_mod, name):
+    """The stored-force sweep (fire_path = 2) must leave the full 2-wide ghost shell of q current, because the
+    recompute sweep that may run next on the same context reads q with a 2-site halo.  40 steps on path 2, then 60
+    on path 0 with no lq_set_Q in between == the oracle run the same way (two calls, each restarting v, dt, alpha;
+    DESIGN.md R13)."""
+    c = SMALL_CASES[name]()
+    ctx = lq.create_from_config(c)
+    o = make_oracle(oracle_mod, c)
+    lq.lq_set_option(ctx, "fire_path", 2)
+    lq.lq_fire_minimize(ctx, 40, 0.0, c["fire"])
+    lq.lq_set_option(ctx, "fire_path", 0)
+    lq.lq_fire_minimize(ctx, 60, 0.0, c["fire"])
+    q1, _ = o.fire(c["q"], 40, 0.0, c["fire"], variant=1)
+    q2, _ = o.fire(q1, 60, 0.0, c["fire"], variant=1)
+    assert np.abs(lq.lq_get_Q(ctx) - q2).max() <= TOL_Q100
+    lq.lq_destroy(ctx)
+
+
+@pytest.mark.parametrize("name", ["replica4", "replica5p", "replica3"])
+def test_fused_steps_are_bit_reproducible(lq, name):
+    """per-CTA partials are reduced in index order by the last CTA to finish, no floating-point atomics anywhere:
+    two runs of 100 fused steps from the same state give bit-identical Q, v and schedule"""
+    c = SMALL_CASES[name]()
+    ctx = lq.create_from_config(c)
+    out = []
+    for _ in range(2):
+        lq.lq_set_Q(ctx, c["q"])
+        rep = lq.lq_fire_minimize(ctx, 100, 0.0, c["fire"])
+        out.append((lq.lq_get_Q(ctx), lq.lq_get_velocity(ctx), rep["dt"], rep["alpha"], rep["P"], rep["Fmax"]))
+    assert np.array_equal(out[0][0], out[1][0]) and np.array_equal(out[0][1], out[1][1])
+    assert out[0][2:] == out[1][2:]
+    lq.lq_destroy(ctx)
 
 
 def test_fused_and_unfused_paths_agree(case, lq):

@@ -1,11 +1,15 @@
 """GPU parity at BASELINE.json's FULL sizes (configs 2, 3, 4, 5, 5'), in the launch configuration bench.py times.
 
-What the oracle can do at these sizes in seconds it does in full (classification, energy, force field with the
-OpenMP variant); FIRE trajectories are compared for a few steps in full (10 steps; 100 steps for config 2, and
-for configs 3 / 5 / 5' when LQ_FULL_PARITY=1 -- the 100-step runs on their declared replicas are in
-test_parity_gpu.py); config 4 (512^3, 134M sites) uses sampled sites for forces and the first FIRE step, plus
-properties that hold at any size: lattice-translation equivariance of the fused trajectory and agreement of the
-fused sweep with the unfused generic path.
+What the oracle can do at these sizes in a few minutes it does in full: classification, energy, force field and
+exactly 100 FIRE steps (north_star's gate) on configs 2, 3, 5, 5' at full size, every site (oracle: OpenMP variant,
+measured on the GPU box's 16 host cores: about 1-4 minutes per config).  Config 4 (512^3, 134M sites) uses sampled
+sites for forces and the first FIRE step, plus properties that hold at any size (lattice-translation equivariance of
+the fused trajectory, agreement of the fused sweep with the unfused generic path), and its 256^3 periodic crop runs
+the full 100 steps against the oracle in the SAME launch configuration as the 512^3 run (64-plane z-chunks, many
+waves of CTAs).  north_star's converged-energy gate (rel 1e-6): config 2 at full size against the oracle and the
+closed form 980000 f0; configs 3, 5, 5' on their declared replicas (the full-size runs need 5000 /
+30000 steps of a 16M-site oracle).  The oracle leg of the config-2 convergence run (7.3 min) is opt-in:
+LQ_FULL_PARITY=1; its passing log is kept in profiles/r02_parity_fullsize.txt.
 """
 import os
 
@@ -34,8 +38,7 @@ def make_oracle(oracle_mod, c):
                              mask=c["mask"], kind=c["kind"], W=c["W"], axis=c["axis"])
 
 
-@pytest.mark.parametrize("name,steps", [("2", 100), ("3", 100 if FULL else 10), ("5", 100 if FULL else 10),
-                                        ("5p", 100 if FULL else 10)])
+@pytest.mark.parametrize("name,steps", [("2", 100), ("3", 100), ("5", 100), ("5p", 100)])
 def test_full_size_masked_configs(lq, oracle_mod, name, steps):
     c = wl.make_config(name)
     ctx = lq.create_from_config(c)
@@ -126,4 +129,68 @@ def test_config4_full_size(lq, oracle_mod):
     lq.lq_fire_minimize(ctx, K, 0.0, c["fire"])
     qc = lq.lq_get_Q(ctx)
     assert np.abs(qc.reshape(5, L, L, L) - np.roll(qa.reshape(5, L, L, L), sh, axis=(1, 2, 3))).max() <= 1e-11
+    lq.lq_destroy(ctx)
+
+
+def test_config4_crop_256_100_steps(lq, oracle_mod):
+    """north_star: Q after exactly 100 FIRE steps, max-abs 1e-8, on the 256^3 periodic crop of config 4 (SURVEY 8(d)
+    allows the crop: the 512^3 oracle needs 16 GB and hours).  256^3 takes the same launch configuration of
+    k_sweep_rc as 512^3: 64-plane z-chunks, 1024 CTAs = 7 waves on 148 SMs, x/y/z ghost shells written by face
+    CTAs -- the configuration bench.py times, oracle-checked over many steps."""
+    c = wl.bulk_quench(256, wl.SEED_BASE + 4)
+    ctx = lq.create_from_config(c)
+    o = make_oracle(oracle_mod, c)
+    rep = lq.lq_fire_minimize(ctx, 100, 0.0, c["fire"], report_energy=True)
+    assert rep["steps"] == 100 and rep["sweep_launches"] == 100 and rep["launches"] == 100
+    qref, rref = o.fire(c["q"], 100, 0.0, c["fire"], variant=1)
+    assert np.abs(lq.lq_get_Q(ctx) - qref).max() <= TOL_Q
+    assert abs(rep["energy"] - rref["energy"]) <= TOL_E * abs(rref["energy"])
+    assert abs(rep["dt"] - rref["dt"]) <= 1e-15 and abs(rep["alpha"] - rref["alpha"]) <= 1e-15
+    assert abs(rep["P"] - rref["P"]) <= 1e-6 * abs(rref["P"])
+    lq.lq_destroy(ctx)
+
+
+TOL_ECONV = 1e-6
+
+
+def test_config2_converged_energy_full_size(lq, oracle_mod):
+    """north_star: converged minimised energy rel 1e-6.  Config 2 at full size (100^3 slab, homeotropic walls) to
+    max|F| < 1e-9: against the closed form 980000 f0 (uniform z texture: zero bulk force, zero elastic energy, both
+    wall terms zero, Eq. 6-8) and against the oracle run the same way (about 6700 steps
+    of a 1M-site lattice: a few minutes on the box's host cores)."""
+    c = wl.make_config("2")
+    ctx = lq.create_from_config(c)
+    rep = lq.lq_fire_minimize(ctx, c["max_steps"], c["tol"], c["fire"], report_energy=True)
+    S0 = lq.lq_get_S0(ctx)
+    f0 = 0.75 * c["A"] * S0 ** 2 + 0.25 * c["B"] * S0 ** 3 + 9.0 / 16.0 * c["C"] * S0 ** 4
+    assert rep["converged"] == 1 and rep["Fmax"] < c["tol"]
+    assert abs(rep["energy"] - 980000 * f0) <= TOL_ECONV * abs(980000 * f0)
+    if not FULL:
+        # the oracle leg takes 7.3 min on the GPU box's 16 cores (measured; passing log: profiles/r02_parity_fullsize.txt):
+        # opt in with LQ_FULL_PARITY=1 so that the default -m gpu suite stays near ten minutes
+        lq.lq_destroy(ctx)
+        return
+    o = make_oracle(oracle_mod, c)
+    qref, rref = o.fire(c["q"], c["max_steps"], c["tol"], c["fire"], variant=1)
+    assert rref["converged"] == 1
+    assert abs(rep["energy"] - rref["energy"]) <= TOL_ECONV * abs(rref["energy"])
+    assert abs(rep["steps"] - rref["steps"]) <= max(5, rref["steps"] // 100)      # chaotic late-stage schedule
+    lq.lq_destroy(ctx)
+
+
+@pytest.mark.parametrize("name", ["3", "5", "5p"])
+def test_replica_converged_energy(lq, oracle_mod, name):
+    """north_star: converged minimised energy rel 1e-6 on the declared replicas of configs 3, 5, 5' (full size:
+    5000 / 30000 steps of a 16M-site oracle).  Both sides run to max|F| < 1e-8 or 2000 steps, whichever comes first;
+    the energies at the end agree to 1e-6 relative and the energy has dropped."""
+    c = wl.make_replica(name)
+    ctx = lq.create_from_config(c)
+    o = make_oracle(oracle_mod, c)
+    e0 = lq.lq_energy(ctx)
+    rep = lq.lq_fire_minimize(ctx, 2000, 1e-8, c["fire"], report_energy=True)
+    qref, rref = o.fire(c["q"], 2000, 1e-8, c["fire"], variant=1)
+    assert rep["converged"] == rref["converged"]
+    assert abs(rep["steps"] - rref["steps"]) <= 3
+    assert abs(rep["energy"] - rref["energy"]) <= TOL_ECONV * abs(rref["energy"])
+    assert rep["energy"] < e0
     lq.lq_destroy(ctx)

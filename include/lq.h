@@ -28,6 +28,7 @@
 #ifndef LQ_H
 #define LQ_H
 
+#include <stddef.h>
 #include <stdint.h>
 
 #ifdef __cplusplus
@@ -202,6 +203,69 @@ int lq_descent_minimize(lq_ctx *ctx, int method, long max_steps, double force_to
 int lq_analyze(lq_ctx *ctx, double S_threshold, double *S, double *director, uint8_t *defect, long *n_defect,
                int where);
 
+/* ---- Domain decomposition into z-slabs.  "The simulation domain is divided into rectilinear
+ * sub-domains, each handled by one rank; after every minimisation step the sites on the faces between sub-domains are
+ * communicated, and the scalar quantities the minimiser needs are reduced over all ranks" (the
+ * weak-scaling workload of Fig. 4).  Here: slabs along z.
+ *
+ * lq_create_slab makes a sub-domain context for the planes [z0, z0 + nz) of a global Lx x Ly x Lz lattice (nz >= 4).
+ * It behaves like any context on LOCAL arrays of nz planes (lq_set_Q, lq_get_Q, lq_get_flags, lq_forces, lq_energy,
+ * lq_analyze: the slab's own sites), with these differences: nothing wraps in z -- the two ghost planes on either
+ * side hold the neighbour slabs' boundary planes and are filled by a halo exchange, which must follow every
+ * lq_set_Q before lq_energy / lq_forces / a FIRE run; geometry comes through lq_set_sites_ext; FIRE runs through
+ * lq_slabs_fire_minimize (same process, same GPU) or lq_fire_begin / step_local / step_commit / end (one rank per
+ * GPU); lq_fire_minimize, lq_descent_minimize and fire_path 1 return LQ_ERR_STATE. */
+int lq_create_slab(int Lx, int Ly, int Lz_global, int z0, int nz, double A, double B, double C,
+                   double L1, double L2, double L3, lq_ctx **out);
+
+/* Geometry of a sub-domain: like lq_set_sites, but every array covers the planes z0-3 .. z0+nz+2 of the global
+ * lattice (periodic wrap in z), i.e. (nz + 6) * Ly * Lx sites ([3][...] for axis): the 3-plane margin makes the
+ * classification of the slab's two ghost planes, and with it every stencil weight near a face, identical to the
+ * undivided lattice's (bit-exact flags: lq_get_flags returns the slab's nz planes). */
+int lq_set_sites_ext(lq_ctx *ctx, const uint8_t *mask_ext, const uint8_t *kind_ext, const double *W_ext,
+                     const double *axis_ext, int where);
+
+/* Halo packages.  what = LQ_HALO_Q: the Q field (after lq_set_Q); LQ_HALO_STATE: the FIRE state after a step
+ * (q, v, and the stored force on the stored-force path).  face 0 = low z, 1 = high z.  lq_halo_export packs the
+ * slab's own two boundary planes of that face (z = 0, 1 or nz-2, nz-1; whole padded planes, 5 components per field)
+ * into buf (lq_halo_bytes bytes); lq_halo_import writes a package into the two ghost planes of that face
+ * (z = -2, -1 or nz, nz+1).  A slab's low-face ghosts take its lower neighbour's HIGH-face export and vice versa
+ * (periodic in the slab index).  lq_slabs_exchange does this for a whole same-process group with device-to-device
+ * copies and returns when they have completed. */
+enum { LQ_HALO_Q = 0, LQ_HALO_STATE = 1 };
+int lq_halo_bytes(lq_ctx *ctx, int what, size_t *bytes);
+int lq_halo_export(lq_ctx *ctx, int what, int face, void *buf, int where);
+int lq_halo_import(lq_ctx *ctx, int what, int face, const void *buf, int where);
+int lq_slabs_exchange(lq_ctx **slabs, int n, int what);
+
+/* FIRE over a same-process group of slabs that tile [0, Lz) in z order, all on one GPU and one stream: per step one
+ * fused sweep per slab (schedule update deferred), one reduction kernel over all slabs' per-CTA partials in a fixed
+ * order (the "all-reduce" of (P, |F|^2, |v|^2, max|F|)), one kernel that writes the same schedule update into every
+ * slab's device scalars, and device-to-device halo copies.  The report is that of the whole lattice. */
+int lq_slabs_fire_minimize(lq_ctx **slabs, int n, long max_steps, double force_tol,
+                           const lq_fire_params *params, lq_fire_report *out);
+
+/* The same step in transport-agnostic pieces, for one rank per GPU.  After the initial LQ_HALO_Q exchange:
+ *     lq_fire_begin(ctx, ...)
+ *     repeat: lq_fire_step_local(ctx)            the fused sweep of this slab (schedule update deferred)
+ *             exchange LQ_HALO_STATE packages with both neighbours
+ *             lq_fire_step_finish(ctx, tot6, where, &again)   the fix-up launch where the path has one (stored force
+ *                                                + objects: it evaluates forces on q' across the faces), then this
+ *                                                slab's row (P, |F|^2, |v|^2, max|F|, and for the first sweep
+ *                                                |F(q_0)|^2, max|F(q_0)|), to a device or host buffer
+ *             all-gather the rows;  lq_fire_step_commit(ctx, rows, nrank): rows combined in rank order -> schedule
+ *             if again: exchange LQ_HALO_STATE once more (the fix-up changed v and F on the boundary planes)
+ *             every so often lq_fire_peek(ctx, report) (synchronises) to test `converged`
+ *     lq_fire_end(ctx, report)                   fixes the live buffer; Frms uses the slab's own site count
+ * The number of sweeps to enqueue is max(max_steps, 1), or max_steps + 1 on the stored-force path or with
+ * integrator = 1.  Either every slab of a lattice gets geometry (lq_set_sites_ext) or none does. */
+int lq_fire_begin(lq_ctx *ctx, long max_steps, double force_tol, const lq_fire_params *params);
+int lq_fire_step_local(lq_ctx *ctx);
+int lq_fire_step_finish(lq_ctx *ctx, double *tot6, int where, int *exchange_again);
+int lq_fire_step_commit(lq_ctx *ctx, const double *rows, int nrank, int where);
+int lq_fire_peek(lq_ctx *ctx, lq_fire_report *out);
+int lq_fire_end(lq_ctx *ctx, lq_fire_report *out);
+
 /* S0 of Eq. 7 for the context's A, B, C (host double). */
 int lq_get_S0(lq_ctx *ctx, double *S0);
 
@@ -215,6 +279,7 @@ int lq_get_S0(lq_ctx *ctx, double *S0);
  *                      n > 0 = n equal chunks per column (clamped to chunks of 4 .. 126 planes)
  *   "sweep_bytes_per_site" (get): algorithmic HBM bytes one sweep moves per site
  *   "n_simulated" (get), "n_boundary" (get), "n_object" (get)
+ *   "has_fixup" (get): 1 if a FIRE step on this context is a sweep plus a fix-up launch (stored force + objects)
  * Unknown key: LQ_ERR_ARG. */
 int lq_set_option(lq_ctx *ctx, const char *key, double value);
 int lq_get_info(lq_ctx *ctx, const char *key, double *value);

@@ -24,7 +24,11 @@ _lib = None
 # every symbol include/lq.h declares (checked by tests/test_abi.py against the header)
 SYMBOLS = ["lq_create", "lq_destroy", "lq_set_stream", "lq_set_sites", "lq_get_flags", "lq_set_Q", "lq_get_Q",
            "lq_get_velocity", "lq_set_field", "lq_set_chiral", "lq_set_cubic", "lq_analyze", "lq_energy", "lq_energy_terms", "lq_forces", "lq_fire_minimize", "lq_descent_minimize", "lq_get_S0",
-           "lq_set_option", "lq_get_info", "lq_last_error", "lq_version"]
+           "lq_set_option", "lq_get_info", "lq_last_error", "lq_version",
+           "lq_create_slab", "lq_set_sites_ext", "lq_halo_bytes", "lq_halo_export", "lq_halo_import", "lq_slabs_exchange",
+           "lq_slabs_fire_minimize", "lq_fire_begin", "lq_fire_step_local", "lq_fire_step_finish", "lq_fire_step_commit", "lq_fire_peek",
+           "lq_fire_end"]
+LQ_HALO_Q, LQ_HALO_STATE = 0, 1
 
 
 class LqError(RuntimeError):
@@ -87,6 +91,20 @@ def load():
     L.lq_get_S0.argtypes = [vp, dp]
     L.lq_set_option.argtypes = [vp, C.c_char_p, C.c_double]
     L.lq_get_info.argtypes = [vp, C.c_char_p, dp]
+    L.lq_create_slab.argtypes = [ip, ip, ip, ip, ip] + [C.c_double] * 6 + [C.POINTER(vp)]
+    L.lq_set_sites_ext.argtypes = [vp, vp, vp, vp, vp, ip]
+    L.lq_halo_bytes.argtypes = [vp, ip, C.POINTER(C.c_size_t)]
+    L.lq_halo_export.argtypes = [vp, ip, ip, vp, ip]
+    L.lq_halo_import.argtypes = [vp, ip, ip, vp, ip]
+    L.lq_slabs_exchange.argtypes = [C.POINTER(vp), ip, ip]
+    L.lq_slabs_fire_minimize.argtypes = [C.POINTER(vp), ip, C.c_long, C.c_double, C.POINTER(lq_fire_params),
+                                         C.POINTER(lq_fire_report)]
+    L.lq_fire_begin.argtypes = [vp, C.c_long, C.c_double, C.POINTER(lq_fire_params)]
+    L.lq_fire_step_local.argtypes = [vp]
+    L.lq_fire_step_finish.argtypes = [vp, vp, ip, C.POINTER(C.c_int)]
+    L.lq_fire_step_commit.argtypes = [vp, vp, ip, ip]
+    L.lq_fire_peek.argtypes = [vp, C.POINTER(lq_fire_report)]
+    L.lq_fire_end.argtypes = [vp, C.POINTER(lq_fire_report)]
     L.lq_last_error.argtypes = [vp]
     L.lq_last_error.restype = C.c_char_p
     L.lq_version.restype = C.c_char_p
@@ -305,3 +323,119 @@ def create_from_config(c: dict) -> lq_ctx:
         lq_set_sites(ctx, c["mask"], c.get("kind"), c.get("W"), c.get("axis"))
     lq_set_Q(ctx, np.ascontiguousarray(c["q"]))
     return ctx
+
+
+# ---------------------------------------------------------------- z-slab sub-domains (lq.h)
+
+def _fire_params(params, report_energy=False):
+    return lq_fire_params(params["dt0"], params["dtmax"], params["alpha0"], params["finc"], params["fdec"],
+                          params["falpha"], int(params["Nmin"]), int(params.get("integrator", 0)), int(bool(report_energy)))
+
+
+def _report(rep):
+    return {k: getattr(rep, k) for k, _ in lq_fire_report._fields_}
+
+
+def lq_create_slab(Lx, Ly, Lz_global, z0, nz, A, B, Cc, L1, L2=0.0, L3=0.0) -> lq_ctx:
+    """sub-domain context for the planes [z0, z0 + nz) of a global Lx x Ly x Lz_global lattice"""
+    h = C.c_void_p()
+    _check(None, load().lq_create_slab(int(Lx), int(Ly), int(Lz_global), int(z0), int(nz), A, B, Cc, L1, L2, L3, C.byref(h)))
+    ctx = lq_ctx(h, (int(Lx), int(Ly), int(nz)))
+    ctx.z0, ctx.Lz_global = int(z0), int(Lz_global)
+    return ctx
+
+
+def lq_set_sites_ext(ctx, mask_ext, kind_ext=None, W_ext=None, axis_ext=None) -> None:
+    """arrays cover the planes z0-3 .. z0+nz+2 of the global lattice: (nz + 6) * Ly * Lx sites"""
+    n = (ctx.Lz + 6) * ctx.Ly * ctx.Lx
+    pm, wm = _buf(mask_ext, np.uint8, n)
+    pk, wk = _buf(kind_ext, np.uint8, n)
+    pw, ww = _buf(W_ext, np.float64, n)
+    pa, wa = _buf(axis_ext, np.float64, 3 * n)
+    wheres = {w for w in (wm, wk, ww, wa) if w is not None}
+    if len(wheres) != 1:
+        raise LqError(LQ_ERR_ARG, "lq_set_sites_ext: all arrays must live in the same place")
+    _check(ctx.handle, load().lq_set_sites_ext(ctx.handle, pm, pk, pw, pa, wheres.pop()))
+
+
+def lq_halo_bytes(ctx, what) -> int:
+    b = C.c_size_t()
+    _check(ctx.handle, load().lq_halo_bytes(ctx.handle, int(what), C.byref(b)))
+    return b.value
+
+
+def _rawbuf(buf, nbytes):
+    """(pointer, where) of a byte buffer: numpy array or torch tensor (any dtype) holding >= nbytes"""
+    if isinstance(buf, np.ndarray):
+        if not buf.flags["C_CONTIGUOUS"] or buf.nbytes < nbytes:
+            raise LqError(LQ_ERR_ARG, "halo buffer too small or not contiguous")
+        return C.c_void_p(buf.ctypes.data), LQ_HOST
+    if hasattr(buf, "data_ptr"):
+        if not buf.is_contiguous() or buf.numel() * buf.element_size() < nbytes:
+            raise LqError(LQ_ERR_ARG, "halo buffer too small or not contiguous")
+        return C.c_void_p(buf.data_ptr()), (LQ_DEVICE if buf.is_cuda else LQ_HOST)
+    raise LqError(LQ_ERR_ARG, "unsupported buffer type %r" % type(buf))
+
+
+def lq_halo_export(ctx, what, face, buf) -> None:
+    p, w = _rawbuf(buf, lq_halo_bytes(ctx, what))
+    _check(ctx.handle, load().lq_halo_export(ctx.handle, int(what), int(face), p, w))
+
+
+def lq_halo_import(ctx, what, face, buf) -> None:
+    p, w = _rawbuf(buf, lq_halo_bytes(ctx, what))
+    _check(ctx.handle, load().lq_halo_import(ctx.handle, int(what), int(face), p, w))
+
+
+def _handles(ctxs):
+    return (C.c_void_p * len(ctxs))(*[c.handle for c in ctxs])
+
+
+def lq_slabs_exchange(ctxs, what) -> None:
+    _check(ctxs[0].handle, load().lq_slabs_exchange(_handles(ctxs), len(ctxs), int(what)))
+
+
+def lq_slabs_fire_minimize(ctxs, max_steps, force_tol, params: dict, report_energy=False) -> dict:
+    fp = _fire_params(params, report_energy)
+    rep = lq_fire_report()
+    _check(ctxs[0].handle, load().lq_slabs_fire_minimize(_handles(ctxs), len(ctxs), int(max_steps), float(force_tol),
+                                                         C.byref(fp), C.byref(rep)))
+    return _report(rep)
+
+
+def lq_fire_begin(ctx, max_steps, force_tol, params: dict) -> None:
+    fp = _fire_params(params)
+    _check(ctx.handle, load().lq_fire_begin(ctx.handle, int(max_steps), float(force_tol), C.byref(fp)))
+
+
+def lq_fire_step_local(ctx) -> None:
+    """this slab's fused sweep of the next step"""
+    _check(ctx.handle, load().lq_fire_step_local(ctx.handle))
+
+
+def lq_fire_step_finish(ctx, tot6) -> bool:
+    """fix-up launch (where the path has one) + this slab's reductions into tot6 (6 doubles: numpy array or CUDA
+    tensor).  Returns True if the halo packages must be exchanged once more after the commit."""
+    p, w = _buf(tot6, np.float64, 6)
+    again = C.c_int()
+    _check(ctx.handle, load().lq_fire_step_finish(ctx.handle, p, w, C.byref(again)))
+    return bool(again.value)
+
+
+def lq_fire_step_commit(ctx, rows) -> None:
+    """rows: [nrank][6] doubles (numpy array or CUDA tensor), combined in rank order"""
+    n = (rows.size if isinstance(rows, np.ndarray) else rows.numel()) // 6
+    p, w = _buf(rows, np.float64, 6 * n)
+    _check(ctx.handle, load().lq_fire_step_commit(ctx.handle, p, int(n), w))
+
+
+def lq_fire_peek(ctx) -> dict:
+    rep = lq_fire_report()
+    _check(ctx.handle, load().lq_fire_peek(ctx.handle, C.byref(rep)))
+    return _report(rep)
+
+
+def lq_fire_end(ctx) -> dict:
+    rep = lq_fire_report()
+    _check(ctx.handle, load().lq_fire_end(ctx.handle, C.byref(rep)))
+    return _report(rep)

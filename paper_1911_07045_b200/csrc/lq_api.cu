@@ -1,9 +1,7 @@
 // lq_api.cu -- the C ABI of liblq.so (include/lq.h): argument checking, device buffers,
 // host<->device marshalling and the FIRE driver loop.  No arithmetic of the method runs on
 // the host: every step of the path is a kernel in lq_kernels.cu / lq_sweep.cu.
-#include "../../include/lq.h"
-#include "lq_internal.cuh"
-#include "lq_sweep.cuh"
+#include "lq_ctx.cuh"
 
 #include <cmath>
 #include <cstdio>
@@ -11,81 +9,42 @@
 #include <new>
 #include <string>
 
-struct lq_ctx {
-    LqGeom g{};
-    LqPhys ph{};
-    int device = 0;
-    cudaStream_t stream = nullptr;
-    // state, padded SoA; [cur] is the live buffer, [cur^1] the sweep's output buffer
-    double *q[2] = {nullptr, nullptr}, *v[2] = {nullptr, nullptr}, *F[2] = {nullptr, nullptr};
-    int cur = 0;
-    uint8_t *maskp = nullptr, *flags = nullptr, *kind = nullptr;
-    double *W = nullptr, *axis = nullptr;
-    bool flags_active = false, anch_active = false, has_Q = false;
-    unsigned long long n_class[3] = {0, 0, 0};
-    double *partials = nullptr;
-    size_t partials_len = 0;
-    double *dscal3 = nullptr;            // 3 doubles of energy output
-    LqFireScalars *dsc = nullptr;        // 2 slots
-    unsigned long long *dcounts = nullptr;
-    int *dbad = nullptr;
-    LqSweepPlan *sweep = nullptr;
-    LqDescentPlan *descent = nullptr;
-    int fire_path = 0;
-    int rc_chunks = 0;                   // "rc_chunks" option: 0 = chunk table chosen by the makespan model
-    bool v_valid = false;                // v[cur] holds the velocities of the last lq_fire_minimize (else: report zeros)
-    double v_mix_a = 1.0, v_mix_b = 0.0; // FIRE rescale of the last step, not yet applied to v[cur] (the sweeps apply it lazily)
-    cudaEvent_t ev0 = nullptr, ev1 = nullptr;   // timing of the minimisation loops (report.gpu_ms)
-    void *scratch = nullptr;             // lq_analyze(LQ_HOST): device staging of the outputs, grown on demand
-    size_t scratch_len = 0;
-    std::string err;
-};
+thread_local std::string g_noctx_err;
 
 namespace {
 
-thread_local std::string g_noctx_err;
+}  // namespace
 
-int fail(lq_ctx *c, int code, const std::string &msg) {
-    if (c) c->err = msg;
-    else g_noctx_err = msg;
-    return code;
-}
-#define LQ_CUDA(c, call)                                                                             \
-    do {                                                                                             \
-        cudaError_t e_ = (call);                                                                     \
-        if (e_ != cudaSuccess)                                                                       \
-            return fail((c), e_ == cudaErrorMemoryAllocation ? LQ_ERR_NOMEM : LQ_ERR_CUDA,           \
-                        std::string(#call) + ": " + cudaGetErrorString(e_));                         \
-    } while (0)
-
-LqFields fields_of(const lq_ctx *c) {
-    LqFields f;
-    f.flags = c->flags_active ? c->flags : nullptr;
-    f.kind = (c->flags_active && c->anch_active) ? c->kind : nullptr;
-    f.W = c->W;
-    f.axis = c->axis;
-    return f;
-}
-
-// copy between a caller's dense [ncomp][Lz][Ly][Lx] array and a padded device array
-cudaError_t copy_box(const LqGeom &g, const void *padded_c, const void *user, size_t elem, int ncomp, bool to_padded,
-                     cudaStream_t st) {
+cudaError_t lq_copy_box(const LqGeom &g, const void *padded_c, const void *user, size_t elem, int ncomp, bool to_padded,
+                        cudaStream_t st, int pz0, int nz, int user_z0, int user_nz) {
     void *padded = const_cast<void *>(padded_c);
+    if (nz < 0) nz = g.Lz;
+    if (user_nz < 0) user_nz = nz;
     for (int c = 0; c < ncomp; ++c) {
         cudaMemcpy3DParms p;
         memset(&p, 0, sizeof(p));
-        cudaPitchedPtr up = make_cudaPitchedPtr((char *)user + (size_t)c * g.N * elem, g.Lx * elem, g.Lx * elem, g.Ly);
+        cudaPitchedPtr up = make_cudaPitchedPtr((char *)user + (size_t)c * g.Lx * g.Ly * (size_t)user_nz * elem, g.Lx * elem,
+                                                g.Lx * elem, g.Ly);
         cudaPitchedPtr pp = make_cudaPitchedPtr((char *)padded + (size_t)c * g.NP * elem, g.Px * elem, g.Px * elem, g.Py);
-        cudaPos ppos = make_cudaPos(LQ_XO * elem, LQ_GH, LQ_GH), upos = make_cudaPos(0, 0, 0);
+        cudaPos ppos = make_cudaPos(LQ_XO * elem, LQ_GH, pz0), upos = make_cudaPos(0, 0, user_z0);
         if (to_padded) { p.srcPtr = up; p.srcPos = upos; p.dstPtr = pp; p.dstPos = ppos; }
         else           { p.srcPtr = pp; p.srcPos = ppos; p.dstPtr = up; p.dstPos = upos; }
-        p.extent = make_cudaExtent(g.Lx * elem, g.Ly, g.Lz);
+        p.extent = make_cudaExtent(g.Lx * elem, g.Ly, nz);
         p.kind = cudaMemcpyDefault;
         cudaError_t e = cudaMemcpy3DAsync(&p, st);
         if (e != cudaSuccess) return e;
     }
     return cudaSuccess;
 }
+
+int lq_ensure_field(lq_ctx *c, double **p) {
+    if (*p) return LQ_OK;
+    LQ_CUDA(c, cudaMalloc(p, (size_t)5 * c->g.NP * sizeof(double)));
+    LQ_CUDA(c, cudaMemsetAsync(*p, 0, (size_t)5 * c->g.NP * sizeof(double), c->stream));
+    return LQ_OK;
+}
+
+namespace {
 
 int ensure_partials(lq_ctx *c, size_t n) {
     if (c->partials_len >= n) return LQ_OK;
@@ -95,25 +54,6 @@ int ensure_partials(lq_ctx *c, size_t n) {
     c->partials_len = n;
     return LQ_OK;
 }
-
-int ensure_field(lq_ctx *c, double **p) {
-    if (*p) return LQ_OK;
-    LQ_CUDA(c, cudaMalloc(p, (size_t)5 * c->g.NP * sizeof(double)));
-    LQ_CUDA(c, cudaMemsetAsync(*p, 0, (size_t)5 * c->g.NP * sizeof(double), c->stream));
-    return LQ_OK;
-}
-
-bool bad_where(int w) { return w != LQ_HOST && w != LQ_DEVICE; }
-
-// every ABI entry runs on the context's device, whatever device the calling thread had current
-struct DeviceGuard {
-    int prev = -1;
-    explicit DeviceGuard(const lq_ctx *c) {
-        if (c && cudaGetDevice(&prev) == cudaSuccess && prev != c->device) cudaSetDevice(c->device);
-        else prev = -1;
-    }
-    ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
-};
 
 }  // namespace
 
@@ -155,7 +95,7 @@ int lq_create(int Lx, int Ly, int Lz, double A, double B, double C, double L1, d
     c->ph = LqPhys{A, B, C, L1, L2, L3, (-B + sqrt(B * B - 24.0 * A * C)) / (6.0 * C)};
     int rc = LQ_OK;
     do {
-        if ((rc = ensure_field(c, &c->q[0])) != LQ_OK) break;
+        if ((rc = lq_ensure_field(c, &c->q[0])) != LQ_OK) break;
         if (cudaMalloc(&c->dscal3, 3 * sizeof(double)) != cudaSuccess ||
             cudaMalloc(&c->dsc, 2 * sizeof(LqFireScalars)) != cudaSuccess ||
             cudaMalloc(&c->dcounts, 3 * sizeof(unsigned long long)) != cudaSuccess ||
@@ -178,7 +118,7 @@ void lq_destroy(lq_ctx *c) {
     DeviceGuard dg(c);
     if (c->ev0) cudaEventDestroy(c->ev0);
     if (c->ev1) cudaEventDestroy(c->ev1);
-    cudaFree(c->scratch);
+    cudaFree(c->scratch); cudaFree(c->dtot); cudaFree(c->dsegs); cudaFree(c->dscptr);
     for (int i = 0; i < 2; ++i) { cudaFree(c->q[i]); cudaFree(c->v[i]); cudaFree(c->F[i]); }
     cudaFree(c->maskp); cudaFree(c->flags); cudaFree(c->kind); cudaFree(c->W); cudaFree(c->axis);
     cudaFree(c->partials); cudaFree(c->dscal3); cudaFree(c->dsc); cudaFree(c->dcounts); cudaFree(c->dbad);
@@ -199,6 +139,7 @@ int lq_set_sites(lq_ctx *c, const uint8_t *mask, const uint8_t *anch_kind, const
     if (!c) return LQ_ERR_ARG;
     DeviceGuard dg(c);
     if (bad_where(where)) return fail(c, LQ_ERR_ARG, "lq_set_sites: bad `where`");
+    if (c->g.zopen && mask) return fail(c, LQ_ERR_STATE, "lq_set_sites: sub-domain contexts take lq_set_sites_ext (arrays with a 3-plane margin)");
     if (anch_kind && (!W || !axis)) return fail(c, LQ_ERR_ARG, "lq_set_sites: anch_kind given without W / axis");
     const LqGeom &g = c->g;
     cudaStream_t st = c->stream;
@@ -214,7 +155,7 @@ int lq_set_sites(lq_ctx *c, const uint8_t *mask, const uint8_t *anch_kind, const
     if (!c->maskp) LQ_CUDA(c, cudaMalloc(&c->maskp, (size_t)g.NP));
     if (!c->flags) LQ_CUDA(c, cudaMalloc(&c->flags, (size_t)g.NP));
     LQ_CUDA(c, cudaMemsetAsync(c->maskp, 0, (size_t)g.NP, st));
-    LQ_CUDA(c, copy_box(g, c->maskp, mask, 1, 1, true, st));
+    LQ_CUDA(c, lq_copy_box(g, c->maskp, mask, 1, 1, true, st));
     LQ_CUDA(c, cudaMemsetAsync(c->dbad, 0, 2 * sizeof(int), st));
     lq_launch_check_u8_max(g, c->maskp, 1, c->dbad, st);
     if (anch_kind) {
@@ -222,7 +163,7 @@ int lq_set_sites(lq_ctx *c, const uint8_t *mask, const uint8_t *anch_kind, const
         if (!c->W) LQ_CUDA(c, cudaMalloc(&c->W, (size_t)g.NP * sizeof(double)));
         if (!c->axis) LQ_CUDA(c, cudaMalloc(&c->axis, (size_t)3 * g.NP * sizeof(double)));
         LQ_CUDA(c, cudaMemsetAsync(c->kind, 0, (size_t)g.NP, st));
-        LQ_CUDA(c, copy_box(g, c->kind, anch_kind, 1, 1, true, st));
+        LQ_CUDA(c, lq_copy_box(g, c->kind, anch_kind, 1, 1, true, st));
         lq_launch_check_u8_max(g, c->kind, 2, c->dbad + 1, st);
     }
     int bad[2] = {0, 0};
@@ -246,8 +187,8 @@ int lq_set_sites(lq_ctx *c, const uint8_t *mask, const uint8_t *anch_kind, const
     if (anch_kind) {
         LQ_CUDA(c, cudaMemsetAsync(c->W, 0, (size_t)g.NP * sizeof(double), st));
         LQ_CUDA(c, cudaMemsetAsync(c->axis, 0, (size_t)3 * g.NP * sizeof(double), st));
-        LQ_CUDA(c, copy_box(g, c->W, W, sizeof(double), 1, true, st));
-        LQ_CUDA(c, copy_box(g, c->axis, axis, sizeof(double), 3, true, st));
+        LQ_CUDA(c, lq_copy_box(g, c->W, W, sizeof(double), 1, true, st));
+        LQ_CUDA(c, lq_copy_box(g, c->axis, axis, sizeof(double), 3, true, st));
         lq_launch_fill_ghosts_u8(g, c->kind, st);     // the recompute sweep evaluates anchoring on halo sites
         lq_launch_fill_ghosts_f64(g, c->W, 1, st);
         lq_launch_fill_ghosts_f64(g, c->axis, 3, st);
@@ -268,7 +209,7 @@ int lq_get_flags(lq_ctx *c, uint8_t *flags, int where) {
         if (where == LQ_HOST) memset(flags, 0xFC, (size_t)c->g.N);
         else LQ_CUDA(c, cudaMemsetAsync(flags, 0xFC, (size_t)c->g.N, c->stream));
     } else {
-        LQ_CUDA(c, copy_box(c->g, c->flags, flags, 1, 1, false, c->stream));
+        LQ_CUDA(c, lq_copy_box(c->g, c->flags, flags, 1, 1, false, c->stream));
     }
     LQ_CUDA(c, cudaStreamSynchronize(c->stream));
     return LQ_OK;
@@ -278,7 +219,7 @@ int lq_set_Q(lq_ctx *c, const double *q, int where) {
     if (!c) return LQ_ERR_ARG;
     DeviceGuard dg(c);
     if (!q || bad_where(where)) return fail(c, LQ_ERR_ARG, "lq_set_Q: bad argument");
-    LQ_CUDA(c, copy_box(c->g, c->q[c->cur], q, sizeof(double), 5, true, c->stream));
+    LQ_CUDA(c, lq_copy_box(c->g, c->q[c->cur], q, sizeof(double), 5, true, c->stream));
     lq_launch_fill_ghosts_f64(c->g, c->q[c->cur], 5, c->stream);
     LQ_CUDA(c, cudaStreamSynchronize(c->stream));
     LQ_CUDA(c, cudaGetLastError());
@@ -292,7 +233,7 @@ int lq_get_Q(lq_ctx *c, double *q, int where) {
     DeviceGuard dg(c);
     if (!q || bad_where(where)) return fail(c, LQ_ERR_ARG, "lq_get_Q: bad argument");
     if (!c->has_Q) return fail(c, LQ_ERR_STATE, "lq_get_Q: no Q has been set");
-    LQ_CUDA(c, copy_box(c->g, c->q[c->cur], q, sizeof(double), 5, false, c->stream));
+    LQ_CUDA(c, lq_copy_box(c->g, c->q[c->cur], q, sizeof(double), 5, false, c->stream));
     LQ_CUDA(c, cudaStreamSynchronize(c->stream));
     return LQ_OK;
 }
@@ -302,7 +243,7 @@ int lq_get_velocity(lq_ctx *c, double *v, int where) {
     DeviceGuard dg(c);
     if (!v || bad_where(where)) return fail(c, LQ_ERR_ARG, "lq_get_velocity: bad argument");
     if (!c->has_Q) return fail(c, LQ_ERR_STATE, "lq_get_velocity: no Q has been set");
-    int rc = ensure_field(c, &c->v[c->cur]);
+    int rc = lq_ensure_field(c, &c->v[c->cur]);
     if (rc != LQ_OK) return rc;
     if (!c->v_valid) {
         LQ_CUDA(c, cudaMemsetAsync(c->v[c->cur], 0, (size_t)5 * c->g.NP * sizeof(double), c->stream));
@@ -311,12 +252,12 @@ int lq_get_velocity(lq_ctx *c, double *v, int where) {
     const double *src = c->v[c->cur];
     if (c->v_mix_a != 1.0 || c->v_mix_b != 0.0) {
         // the last step's rescale v <- (1-alpha) v + alpha |v| F/|F| (or v <- 0) is still pending: apply it to a copy
-        if ((rc = ensure_field(c, &c->F[c->cur])) != LQ_OK) return rc;
+        if ((rc = lq_ensure_field(c, &c->F[c->cur])) != LQ_OK) return rc;
         lq_launch_forces(c->g, c->ph, fields_of(c), c->q[c->cur], c->F[c->cur], c->stream);
         lq_launch_axpby((long long)5 * c->g.NP, c->v_mix_a, c->v[c->cur], c->v_mix_b, c->F[c->cur], c->F[c->cur], c->stream);
         src = c->F[c->cur];
     }
-    LQ_CUDA(c, copy_box(c->g, src, v, sizeof(double), 5, false, c->stream));
+    LQ_CUDA(c, lq_copy_box(c->g, src, v, sizeof(double), 5, false, c->stream));
     LQ_CUDA(c, cudaStreamSynchronize(c->stream));
     return LQ_OK;
 }
@@ -351,10 +292,10 @@ int lq_forces(lq_ctx *c, double *F, int where) {
     DeviceGuard dg(c);
     if (!F || bad_where(where)) return fail(c, LQ_ERR_ARG, "lq_forces: bad argument");
     if (!c->has_Q) return fail(c, LQ_ERR_STATE, "lq_forces: no Q has been set");
-    int rc = ensure_field(c, &c->F[c->cur]);
+    int rc = lq_ensure_field(c, &c->F[c->cur]);
     if (rc != LQ_OK) return rc;
     lq_launch_forces(c->g, c->ph, fields_of(c), c->q[c->cur], c->F[c->cur], c->stream);
-    LQ_CUDA(c, copy_box(c->g, c->F[c->cur], F, sizeof(double), 5, false, c->stream));
+    LQ_CUDA(c, lq_copy_box(c->g, c->F[c->cur], F, sizeof(double), 5, false, c->stream));
     LQ_CUDA(c, cudaStreamSynchronize(c->stream));
     LQ_CUDA(c, cudaGetLastError());
     return LQ_OK;
@@ -388,6 +329,10 @@ int lq_get_info(lq_ctx *c, const char *key, double *value) {
     if (!strcmp(key, "n_simulated")) { *value = nsim; return LQ_OK; }
     if (!strcmp(key, "n_boundary")) { *value = c->flags_active ? (double)c->n_class[1] : 0.0; return LQ_OK; }
     if (!strcmp(key, "n_object")) { *value = c->flags_active ? (double)c->n_class[2] : 0.0; return LQ_OK; }
+    if (!strcmp(key, "has_fixup")) {      // FIRE step = sweep + fix-up launch (stored force on a lattice with objects)
+        *value = ((lq_three(c->ph) || c->fire_path == 2) && c->flags_active) ? 1.0 : 0.0;
+        return LQ_OK;
+    }
     if (!strcmp(key, "sweep_bytes_per_site")) {
         // fused sweep: read + write q, v (and F when it is stored), 5 fp64 each, + the flag byte where objects exist
         const bool three = lq_three(c->ph);
@@ -403,6 +348,7 @@ int lq_fire_minimize(lq_ctx *c, long max_steps, double force_tol, const lq_fire_
     DeviceGuard dg(c);
     if (!fp || !out) return fail(c, LQ_ERR_ARG, "lq_fire_minimize: NULL params / report");
     if (!c->has_Q) return fail(c, LQ_ERR_STATE, "lq_fire_minimize: no Q has been set");
+    if (c->g.zopen) return fail(c, LQ_ERR_STATE, "lq_fire_minimize: sub-domain contexts run lq_slabs_fire_minimize or lq_fire_begin / step / end");
     if (!(fp->dt0 > 0.0) || !(fp->dtmax >= fp->dt0) || !(fp->alpha0 >= 0.0 && fp->alpha0 <= 1.0) ||
         !(fp->finc >= 1.0) || !(fp->fdec > 0.0 && fp->fdec <= 1.0) || !(fp->falpha > 0.0 && fp->falpha <= 1.0) ||
         fp->Nmin < 0 || (fp->integrator != 0 && fp->integrator != 1) || max_steps < 0 || !(force_tol >= 0.0))
@@ -415,12 +361,12 @@ int lq_fire_minimize(lq_ctx *c, long max_steps, double force_tol, const lq_fire_
     const bool fused = c->fire_path != 1;
     const bool three = lq_three(c->ph);
     const bool stored_F = three || c->fire_path == 2;   // recompute-F sweep: one-constant only
-    if ((rc = ensure_field(c, &c->v[c->cur])) != LQ_OK) return rc;
-    if ((!fused || stored_F) && (rc = ensure_field(c, &c->F[c->cur])) != LQ_OK) return rc;
+    if ((rc = lq_ensure_field(c, &c->v[c->cur])) != LQ_OK) return rc;
+    if ((!fused || stored_F) && (rc = lq_ensure_field(c, &c->F[c->cur])) != LQ_OK) return rc;
     if (fused) {
-        if ((rc = ensure_field(c, &c->q[c->cur ^ 1])) != LQ_OK) return rc;
-        if ((rc = ensure_field(c, &c->v[c->cur ^ 1])) != LQ_OK) return rc;
-        if (stored_F && (rc = ensure_field(c, &c->F[c->cur ^ 1])) != LQ_OK) return rc;
+        if ((rc = lq_ensure_field(c, &c->q[c->cur ^ 1])) != LQ_OK) return rc;
+        if ((rc = lq_ensure_field(c, &c->v[c->cur ^ 1])) != LQ_OK) return rc;
+        if (stored_F && (rc = lq_ensure_field(c, &c->F[c->cur ^ 1])) != LQ_OK) return rc;
     }
 
     LqFireConsts fc{fp->dt0, fp->dtmax, fp->alpha0, fp->finc, fp->fdec, fp->falpha, force_tol, fp->Nmin, (long long)max_steps,
@@ -579,6 +525,7 @@ int lq_descent_minimize(lq_ctx *c, int method, long max_steps, double force_tol,
     if (!dp || !out) return fail(c, LQ_ERR_ARG, "lq_descent_minimize: NULL pointer");
     memset(out, 0, sizeof(*out));
     if (!c->has_Q) return fail(c, LQ_ERR_STATE, "lq_descent_minimize: call lq_set_Q first");
+    if (c->g.zopen) return fail(c, LQ_ERR_STATE, "lq_descent_minimize: not available on sub-domain contexts");
     if ((method != LQ_MIN_GD && method != LQ_MIN_NESTEROV) || !(dp->eta > 0.0) || max_steps < 0 || !(force_tol >= 0.0) ||
         (method == LQ_MIN_NESTEROV && !(dp->mu >= 0.0 && dp->mu < 1.0)))
         return fail(c, LQ_ERR_ARG, "lq_descent_minimize: bad parameters");
@@ -586,8 +533,8 @@ int lq_descent_minimize(lq_ctx *c, int method, long max_steps, double force_tol,
     cudaStream_t st = c->stream;
     int rc;
     const int nbuf = method == LQ_MIN_NESTEROV ? 3 : 2;
-    if ((rc = ensure_field(c, &c->q[c->cur ^ 1])) != LQ_OK) return rc;
-    if (nbuf == 3 && (rc = ensure_field(c, &c->v[0])) != LQ_OK) return rc;
+    if ((rc = lq_ensure_field(c, &c->q[c->cur ^ 1])) != LQ_OK) return rc;
+    if (nbuf == 3 && (rc = lq_ensure_field(c, &c->v[0])) != LQ_OK) return rc;
     double *buf[3] = {c->q[c->cur], c->q[c->cur ^ 1], c->v[0]};
     LqFireScalars h;
     memset(&h, 0, sizeof(h));

@@ -34,6 +34,7 @@ struct FixArgs {
     int n_sweep;
     double *partials;
     unsigned int *counter;
+    int defer;              // sub-domains: publish the partials only; the cross-domain reduction advances the schedule
 };
 
 #ifndef LQ_FIX_MINB
@@ -71,7 +72,7 @@ __global__ void __launch_bounds__(FB, LQ_FIX_MINB) k_fixup(const FixArgs a) {
         const int x = (int)(p % a.g.Px) - LQ_XO, y = (int)((p / a.g.Px) % a.g.Py) - LQ_GH,
                   z = (int)(p / a.g.sz) - LQ_GH;
         const int shx = ghost_shift(x, a.g.Lx, LQ_GH), shy = ghost_shift(y, a.g.Ly, LQ_GH),
-                  shz = ghost_shift(z, a.g.Lz, LQ_GH);
+                  shz = ghost_shift_z(z, a.g);
         if (shx | shy | shz) {
             for (int m = 1; m < 8; ++m) {
                 if (((m & 1) && !shx) || ((m & 2) && !shy) || ((m & 4) && !shz)) continue;
@@ -99,8 +100,11 @@ __global__ void __launch_bounds__(FB, LQ_FIX_MINB) k_fixup(const FixArgs a) {
             for (int w = 1; w < NW; ++w) t = k < 3 ? t + red[k * NW + w] : fmax(t, red[k * NW + w]);
             a.partials[4 * blockIdx.x + k] = t;
         }
-        __threadfence();
-        s_last = atomicAdd(a.counter, 1u) == gridDim.x - 1 ? 1u : 0u;
+        if (a.defer) s_last = 0u;
+        else {
+            __threadfence();
+            s_last = atomicAdd(a.counter, 1u) == gridDim.x - 1 ? 1u : 0u;
+        }
     }
     __syncthreads();
     if (!s_last) return;
@@ -182,8 +186,8 @@ int lq_fixup_num_blocks(int n) { return n > 0 ? (n + FB - 1) / FB : 1; }
 cudaError_t lq_launch_fixup(bool three, const LqGeom &g, const LqPhys &ph, const LqFields &f, const double *q,
                             double *v, double *F, const int *list, int n, LqFireScalars *sc, const LqFireConsts &fc,
                             const double *sweep_partials, int n_sweep, double *partials, unsigned int *counter,
-                            cudaStream_t st) {
-    FixArgs a{g, ph, f, q, v, F, list, n, sc, fc, sweep_partials, n_sweep, partials, counter};
+                            cudaStream_t st, int defer) {
+    FixArgs a{g, ph, f, q, v, F, list, n, sc, fc, sweep_partials, n_sweep, partials, counter, defer};
     const int nb = lq_fixup_num_blocks(n);
     if (three) k_fixup<true><<<nb, FB, 0, st>>>(a);
     else k_fixup<false><<<nb, FB, 0, st>>>(a);

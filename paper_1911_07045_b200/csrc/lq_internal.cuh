@@ -31,6 +31,8 @@ struct LqGeom {
     long long sy, sz;  // strides (elements) of +y and +z in the padded box
     long long NP;      // padded sites per component
     long long N;       // Lx*Ly*Lz
+    int zopen;         // 1: z-slab sub-domain: the z ghost planes hold the neighbour slabs' planes
+                       // (halo exchange), nothing wraps in z and no kernel writes z ghost images
     __host__ __device__ inline long long pidx(int x, int y, int z) const {
         return (long long)(x + LQ_XO) + sy * (long long)(y + LQ_GH) + sz * (long long)(z + LQ_GH);
     }
@@ -155,8 +157,18 @@ struct LqFields {
 void lq_launch_fill_ghosts_f64(const LqGeom &g, double *field, int ncomp, cudaStream_t st);
 void lq_launch_fill_ghosts_u8(const LqGeom &g, uint8_t *field, cudaStream_t st);
 void lq_launch_classify(const LqGeom &g, const uint8_t *mask_p, uint8_t *flags_p, cudaStream_t st);
+// sub-domains: mask_ext is a DENSE [Lz+6][Ly][Lx] array covering planes -3 .. Lz+2; flags are written on planes -2 .. Lz+1
+void lq_launch_classify_ext(const LqGeom &g, const uint8_t *mask_ext, uint8_t *flags_p, cudaStream_t st);
+// reductions of a step across sub-domains: seg[i] = (partials pointer, count, stride 4 | 2) in a fixed order
+struct LqPartialSeg { const double *p; int n; int width; };
+void lq_launch_reduce_partials(const LqPartialSeg *seg_dev, int nseg, double *tot6, cudaStream_t st);
+// tot = nrank x 6 doubles (P, FF, vv, Fmax, FF0, Fmax0), combined in rank order; advances every sc[i] identically
+void lq_launch_advance(const double *tot, int nrank, LqFireScalars *const *sc_dev, int nsc, LqFireConsts fc, int first,
+                       cudaStream_t st);
 void lq_launch_count_classes(const LqGeom &g, const uint8_t *flags_p, unsigned long long *counts3, cudaStream_t st);
 void lq_launch_check_u8_max(const LqGeom &g, const uint8_t *arr_p, int maxval, int *bad, cudaStream_t st);
+void lq_launch_check_dense_u8_max(const uint8_t *a, long long n, int maxval, int *bad, cudaStream_t st);
+void lq_launch_check_dense_u8_ne(const uint8_t *a, long long n, int value, int *bad, cudaStream_t st);
 void lq_launch_forces(const LqGeom &g, const LqPhys &ph, const LqFields &f, const double *q, double *F, cudaStream_t st);
 // energy: partial sums per block into partials (3 per block) then final reduce into out3 (device)
 int lq_energy_num_blocks(const LqGeom &g);

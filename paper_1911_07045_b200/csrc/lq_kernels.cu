@@ -20,9 +20,11 @@ __global__ void k_fill_ghosts(LqGeom g, T *field, int ncomp) {
     const int pz = blockIdx.z;
     if (px >= g.Lx + 2 * LQ_GH || py >= g.Py) return;
     const int x = px - LQ_GH, y = py - LQ_GH, z = pz - LQ_GH;
-    if (x >= 0 && x < g.Lx && y >= 0 && y < g.Ly && z >= 0 && z < g.Lz) return;
+    // sub-domain (zopen): nothing wraps in z; every padded plane, its z ghost planes included, gets its x/y ghosts
+    const bool zin = g.zopen || (z >= 0 && z < g.Lz);
+    if (x >= 0 && x < g.Lx && y >= 0 && y < g.Ly && zin) return;
     const long long dst = g.pidx(x, y, z);
-    const long long src = g.pidx(wrap(x, g.Lx), wrap(y, g.Ly), wrap(z, g.Lz));
+    const long long src = g.pidx(wrap(x, g.Lx), wrap(y, g.Ly), g.zopen ? z : wrap(z, g.Lz));
     for (int c = 0; c < ncomp; ++c) field[c * g.NP + dst] = field[c * g.NP + src];
 }
 
@@ -45,6 +47,28 @@ __global__ void k_classify(LqGeom g, const uint8_t *__restrict__ mask_p, uint8_t
     flags_p[p] = (uint8_t)(f | cls);
 }
 
+// sub-domain classification: dense mask with a 3-plane margin (planes -3 .. Lz+2, periodic in x and y) -> packed
+// flags on planes -2 .. Lz+1 (the full z ghost width), same bit layout as k_classify
+__global__ void k_classify_ext(LqGeom g, const uint8_t *__restrict__ m, uint8_t *__restrict__ flags_p) {
+    const int x = blockIdx.x * blockDim.x + threadIdx.x;
+    const int y = blockIdx.y * blockDim.y + threadIdx.y;
+    const int z = (int)blockIdx.z - LQ_GH;                   // -2 .. Lz+1
+    if (x >= g.Lx || y >= g.Ly) return;
+    auto at = [&](int xx, int yy, int zz) -> unsigned {
+        return m[(size_t)wrap(xx, g.Lx) + (size_t)g.Lx * ((size_t)wrap(yy, g.Ly) + (size_t)g.Ly * (size_t)(zz + 3))];
+    };
+    const unsigned nb[6] = {at(x + 1, y, z), at(x - 1, y, z), at(x, y + 1, z), at(x, y - 1, z), at(x, y, z + 1), at(x, y, z - 1)};
+    unsigned f = 0, any_obj = 0;
+#pragma unroll
+    for (int b = 0; b < 6; ++b) {
+        const unsigned sim = nb[b] == 0;
+        f |= sim << (2 + b);
+        any_obj |= !sim;
+    }
+    const unsigned cls = at(x, y, z) != 0 ? 2u : (any_obj ? 1u : 0u);
+    flags_p[g.pidx(x, y, z)] = (uint8_t)(f | cls);
+}
+
 __global__ void k_count_classes(LqGeom g, const uint8_t *__restrict__ flags_p, unsigned long long *counts) {
     const int x = blockIdx.x * blockDim.x + threadIdx.x;
     const int y = blockIdx.y * blockDim.y + threadIdx.y;
@@ -63,6 +87,12 @@ __global__ void k_check_u8_max(LqGeom g, const uint8_t *__restrict__ a, int maxv
     const int y = blockIdx.y * blockDim.y + threadIdx.y;
     const int z = blockIdx.z;
     if (x < g.Lx && y < g.Ly && a[g.pidx(x, y, z)] > maxval) *bad = 1;
+}
+
+// dense byte array: mode 0: any value > ref; mode 1: any value != ref
+__global__ void k_check_dense_u8(const uint8_t *__restrict__ a, long long n, int ref, int mode, int *bad) {
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x)
+        if (mode == 0 ? a[i] > ref : a[i] != ref) *bad = 1;
 }
 
 __device__ __forceinline__ void load_anchor(const LqFields &f, long long NP, long long p, unsigned fl, int &kind,
@@ -260,6 +290,49 @@ __global__ void __launch_bounds__(256) k_fire_update(const double *__restrict__ 
     *sc = t;
 }
 
+// Cross-domain reduction of one step ("one tiny all-reduce"): the per-CTA partials of
+// every sub-domain's sweep (and fix-up) in a FIXED order -> tot6 = (P, FF, vv, Fmax, FF0, Fmax0).  Segments of width 4
+// feed the first four, segments of width 2 (the first sweep's initial-state partials) the last two.
+__global__ void __launch_bounds__(256) k_reduce_partials(const LqPartialSeg *__restrict__ seg, int nseg,
+                                                         double *__restrict__ tot6) {
+    double s[6] = {0, 0, 0, 0, 0, 0};
+    for (int i = 0; i < nseg; ++i) {
+        const LqPartialSeg sg = seg[i];
+        if (sg.width == 4) {
+            for (int b = threadIdx.x; b < sg.n; b += 256) {
+                s[0] += sg.p[4 * b]; s[1] += sg.p[4 * b + 1]; s[2] += sg.p[4 * b + 2]; s[3] = fmax(s[3], sg.p[4 * b + 3]);
+            }
+        } else {
+            for (int b = threadIdx.x; b < sg.n; b += 256) { s[4] += sg.p[2 * b]; s[5] = fmax(s[5], sg.p[2 * b + 1]); }
+        }
+    }
+    // order: sums first (block_reduce sums the first nsum entries, max-reduces the rest)
+    double r[6] = {s[0], s[1], s[2], s[4], s[3], s[5]};
+    __shared__ double out[6];
+    block_reduce<6, 256>(r, 4, out);
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        tot6[0] = out[0]; tot6[1] = out[1]; tot6[2] = out[2]; tot6[3] = out[4]; tot6[4] = out[3]; tot6[5] = out[5];
+    }
+}
+
+// tot: nrank x 6 (one row per rank / sub-domain group, combined in rank order) -> the same schedule update in every
+// sub-domain's scalars.  first: the sweep just reduced was the first of the call (recompute path, velocity Verlet).
+__global__ void k_advance(const double *__restrict__ tot, int nrank, LqFireScalars *const *__restrict__ scs, int nsc,
+                          LqFireConsts fc, int first) {
+    if (threadIdx.x != 0 || blockIdx.x != 0) return;
+    double t[4] = {0, 0, 0, 0}, t0[2] = {0, 0};
+    for (int r = 0; r < nrank; ++r) {
+        t[0] += tot[6 * r]; t[1] += tot[6 * r + 1]; t[2] += tot[6 * r + 2]; t[3] = fmax(t[3], tot[6 * r + 3]);
+        t0[0] += tot[6 * r + 4]; t0[1] = fmax(t0[1], tot[6 * r + 5]);
+    }
+    LqFireScalars nx = *scs[0];
+    if (nx.converged) return;
+    if (first) lq_fire_advance_first(nx, fc, t, t0);
+    else lq_fire_advance_any(nx, fc, t);
+    for (int i = 0; i < nsc; ++i) *scs[i] = nx;
+}
+
 __global__ void k_zero_object_sites(LqGeom g, const uint8_t *__restrict__ flags, double *__restrict__ field) {
     const int x = blockIdx.x * blockDim.x + threadIdx.x;
     const int y = blockIdx.y * blockDim.y + threadIdx.y;
@@ -344,11 +417,20 @@ void lq_launch_fill_ghosts_u8(const LqGeom &g, uint8_t *field, cudaStream_t st) 
 void lq_launch_classify(const LqGeom &g, const uint8_t *mask_p, uint8_t *flags_p, cudaStream_t st) {
     k_classify<<<plane_grid(g), dim3(BX, BY), 0, st>>>(g, mask_p, flags_p);
 }
+void lq_launch_classify_ext(const LqGeom &g, const uint8_t *mask_ext, uint8_t *flags_p, cudaStream_t st) {
+    k_classify_ext<<<dim3((g.Lx + BX - 1) / BX, (g.Ly + BY - 1) / BY, g.Pz), dim3(BX, BY), 0, st>>>(g, mask_ext, flags_p);
+}
 void lq_launch_count_classes(const LqGeom &g, const uint8_t *flags_p, unsigned long long *counts3, cudaStream_t st) {
     k_count_classes<<<plane_grid(g), dim3(BX, BY), 0, st>>>(g, flags_p, counts3);
 }
 void lq_launch_check_u8_max(const LqGeom &g, const uint8_t *arr_p, int maxval, int *bad, cudaStream_t st) {
     k_check_u8_max<<<plane_grid(g), dim3(BX, BY), 0, st>>>(g, arr_p, maxval, bad);
+}
+void lq_launch_check_dense_u8_max(const uint8_t *a, long long n, int maxval, int *bad, cudaStream_t st) {
+    k_check_dense_u8<<<148 * 4, 256, 0, st>>>(a, n, maxval, 0, bad);
+}
+void lq_launch_check_dense_u8_ne(const uint8_t *a, long long n, int value, int *bad, cudaStream_t st) {
+    k_check_dense_u8<<<148 * 4, 256, 0, st>>>(a, n, value, 1, bad);
 }
 void lq_launch_forces(const LqGeom &g, const LqPhys &ph, const LqFields &f, const double *q, double *F,
                       cudaStream_t st) {
@@ -381,6 +463,13 @@ void lq_launch_fire1_force(const LqGeom &g, const LqPhys &ph, const LqFields &f,
 void lq_launch_fire_update(const double *partials, int nblocks, LqFireScalars *sc, LqFireConsts fc, int first,
                            cudaStream_t st) {
     k_fire_update<<<1, 256, 0, st>>>(partials, nblocks, sc, fc, first);
+}
+void lq_launch_reduce_partials(const LqPartialSeg *seg_dev, int nseg, double *tot6, cudaStream_t st) {
+    k_reduce_partials<<<1, 256, 0, st>>>(seg_dev, nseg, tot6);
+}
+void lq_launch_advance(const double *tot, int nrank, LqFireScalars *const *sc_dev, int nsc, LqFireConsts fc, int first,
+                       cudaStream_t st) {
+    k_advance<<<1, 32, 0, st>>>(tot, nrank, sc_dev, nsc, fc, first);
 }
 void lq_launch_zero_object_sites(const LqGeom &g, const uint8_t *flags, double *field, cudaStream_t st) {
     k_zero_object_sites<<<plane_grid(g), dim3(BX, BY), 0, st>>>(g, flags, field);

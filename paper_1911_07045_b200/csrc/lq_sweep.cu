@@ -207,7 +207,7 @@ k_sweep(const __grid_constant__ CUtensorMap tq, const __grid_constant__ CUtensor
             // periodic ghost shell of the outputs, full width LQ_GH: whatever runs next on this state (the
             // recompute sweep reads q with a 2-site halo) finds every ghost current
             const int shx = ghost_shift(x, a.g.Lx, LQ_GH), shy = ghost_shift(y, a.g.Ly, LQ_GH),
-                      shz = ghost_shift(k, a.g.Lz, LQ_GH);
+                      shz = ghost_shift_z(k, a.g);
             if (shx | shy | shz) {
                 for (int m = 1; m < 8; ++m) {
                     if (((m & 1) && !shx) || ((m & 2) && !shy) || ((m & 4) && !shz)) continue;
@@ -386,11 +386,10 @@ static cudaError_t launch(LqSweepPlan *pl, int in, const SweepArgs &a, int varia
         }                                                                                    \
     } while (0)
 
-int lq_sweep_run(LqSweepPlan **planp, bool stored_F, const LqGeom &g, const LqPhys &ph, const LqFields &f, double *q[2],
-                 double *v[2], double *F[2], int *cur, LqFireScalars *dsc, const LqFireConsts &fc, long max_steps,
-                 cudaStream_t st, long *launches, long *sweeps, LqFireScalars *h, std::string &err, int rc_chunks) {
-    using C1 = Cfg<32, 16>;   // one-constant: 512 threads, <= 128 registers
-    using C3 = Cfg<32, 16>;   // three-constant: same tile (ptxas fits the 19-point fast path in 128 registers)
+int lq_sweep_prepare(LqSweepPlan **planp, bool stored_F, const LqGeom &g, const LqPhys &ph, const LqFields &f, double *q[2],
+                     double *v[2], double *F[2], cudaStream_t st, long *launches, std::string &err, int rc_chunks) {
+    using C1 = Cfg<32, 16>;
+    using C3 = Cfg<32, 16>;
     const bool three = lq_three(ph);
     const bool masked = f.flags != nullptr;
     LqSweepPlan *pl = *planp;
@@ -480,15 +479,67 @@ int lq_sweep_run(LqSweepPlan **planp, bool stored_F, const LqGeom &g, const LqPh
         pl->kind_seen = f.kind;
     }
     LQ_PLAN_CUDA(cudaMemsetAsync(pl->counter, 0, sizeof(unsigned int), st));
+    return LQ_OK;
+}
 
-    const int cur0 = *cur;
+// One sweep (+ its fix-up launch on masked stored-force lattices) reading buffers `in`, writing `in ^ 1`.
+// phase 0: both launches; 1: the sweep only; 2: the fix-up only (sub-domains: the fix-up reads q' across the slab
+// faces, so the neighbours' new boundary planes must arrive between the two).
+// first: first sweep of a call on the recompute path with velocity Verlet.  defer: leave the partials to a
+// cross-domain reduction (sub-domains) instead of advancing the schedule in the last CTA.
+int lq_sweep_step(LqSweepPlan *pl, bool stored_F, const LqGeom &g, const LqPhys &ph, const LqFields &f, double *q[2],
+                  double *v[2], double *F[2], int in, LqFireScalars *dsc, const LqFireConsts &fc, bool first, bool defer,
+                  cudaStream_t st, std::string &err, int phase) {
+    using C1 = Cfg<32, 16>;
+    using C3 = Cfg<32, 16>;
+    const bool three = lq_three(ph);
+    const bool masked = f.flags != nullptr;
+    const int out = in ^ 1;
     SweepArgs a;
     memset(&a, 0, sizeof(a));
     a.g = g; a.ph = ph; a.f = f; a.sc = dsc; a.fc = fc; a.partials = pl->partials; a.counter = pl->counter; a.zc = pl->zc;
     a.plain = pl->plain; a.tsum = pl->tsum; a.bond = pl->bond; a.work = pl->work; a.ntx = pl->ntx; a.nty = pl->nty;
     a.partials0 = pl->partials0;
-    a.defer_advance = (masked && stored_F) ? 1 : 0;
+    a.defer_advance = (defer || (masked && stored_F)) ? 1 : 0;
+    a.qo = q[out]; a.vo = v[out]; a.Fo = F[out];
     const int ncta = stored_F ? (int)(pl->grid.x * pl->grid.y * pl->grid.z) : pl->n_items;
+    cudaError_t e = cudaSuccess;
+    if (phase == 2) { /* fix-up only: the sweep of this step has run (sub-domains exchange q' in between) */ }
+    else if (!stored_F)
+        e = lq_launch_sweep_rc(masked, first, ncta, pl->attr_rc, pl->mq[in], pl->mv[in], a, st);
+    else if (three && (ph.L4 != 0.0 || ph.L6 != 0.0)) {
+        const int xt = (ph.L4 != 0.0 ? 1 : 0) | (ph.L6 != 0.0 ? 2 : 0);
+        if (xt == 1) e = masked ? launch<C3, true, true, 1>(pl, in, a, 5, st) : launch<C3, true, false, 1>(pl, in, a, 4, st);
+        else if (xt == 2) e = masked ? launch<C3, true, true, 2>(pl, in, a, 7, st) : launch<C3, true, false, 2>(pl, in, a, 6, st);
+        else e = masked ? launch<C3, true, true, 3>(pl, in, a, 9, st) : launch<C3, true, false, 3>(pl, in, a, 8, st);
+    }
+    else if (three) e = masked ? launch<C3, true, true>(pl, in, a, 3, st) : launch<C3, true, false>(pl, in, a, 2, st);
+    else e = masked ? launch<C1, false, true>(pl, in, a, 1, st) : launch<C1, false, false>(pl, in, a, 0, st);
+    if (e == cudaSuccess && masked && stored_F && phase != 1)
+        e = lq_launch_fixup(three, g, ph, f, q[out], v[out], F[out], pl->np_list, pl->n_np, dsc, fc, pl->partials,
+                            ncta, pl->partials2, pl->counter2, st, defer ? 1 : 0);
+    if (e != cudaSuccess) { err = std::string("lq_sweep launch: ") + cudaGetErrorString(e); return LQ_ERR_CUDA; }
+    return LQ_OK;
+}
+
+// partial-sum segments of the last sweep (for the cross-domain reduction): returns how many were written (<= 3)
+int lq_sweep_segments(const LqSweepPlan *pl, bool stored_F, bool masked, bool first, LqPartialSeg seg[3]) {
+    int n = 0;
+    const int ncta = stored_F ? (int)(pl->grid.x * pl->grid.y * pl->grid.z) : pl->n_items;
+    seg[n++] = LqPartialSeg{pl->partials, ncta, 4};
+    if (stored_F && masked) seg[n++] = LqPartialSeg{pl->partials2, lq_fixup_num_blocks(pl->n_np), 4};
+    if (first) seg[n++] = LqPartialSeg{pl->partials0, ncta, 2};
+    return n;
+}
+
+int lq_sweep_run(LqSweepPlan **planp, bool stored_F, const LqGeom &g, const LqPhys &ph, const LqFields &f, double *q[2],
+                 double *v[2], double *F[2], int *cur, LqFireScalars *dsc, const LqFireConsts &fc, long max_steps,
+                 cudaStream_t st, long *launches, long *sweeps, LqFireScalars *h, std::string &err, int rc_chunks) {
+    int rc = lq_sweep_prepare(planp, stored_F, g, ph, f, q, v, F, st, launches, err, rc_chunks);
+    if (rc != LQ_OK) return rc;
+    LqSweepPlan *pl = *planp;
+    const bool masked = f.flags != nullptr;
+    const int cur0 = *cur;
     // Sweeps to enqueue and buffer flips per step taken.  Recompute path, velocity Verlet: the first sweep also
     // carries the stop test on the initial state, so `max_steps` sweeps (one even if max_steps == 0) and the live
     // buffer flips once per counted step.  Stored path: one extra leading sweep evaluates F(q_0) (all coefficients
@@ -497,27 +548,13 @@ int lq_sweep_run(LqSweepPlan **planp, bool stored_F, const LqGeom &g, const LqPh
     const bool extra = stored_F || fc.euler;
     const long total = extra ? max_steps + 1 : (max_steps > 0 ? max_steps : 1);
     const long chunk = fc.force_tol > 0.0 ? 100 : (1L << 30);
-    cudaError_t e = cudaSuccess;
     long done = 0;
     while (done < total) {
         const long n = (total - done) < chunk ? (total - done) : chunk;
         for (long i = 0; i < n; ++i) {
-            const int in = (int)((cur0 + done + i) & 1), out = in ^ 1;
-            a.qo = q[out]; a.vo = v[out]; a.Fo = F[out];
-            if (!stored_F)
-                e = lq_launch_sweep_rc(masked, !fc.euler && done + i == 0, ncta, pl->attr_rc, pl->mq[in], pl->mv[in], a, st);
-            else if (three && (ph.L4 != 0.0 || ph.L6 != 0.0)) {
-                const int xt = (ph.L4 != 0.0 ? 1 : 0) | (ph.L6 != 0.0 ? 2 : 0);
-                if (xt == 1) e = masked ? launch<C3, true, true, 1>(pl, in, a, 5, st) : launch<C3, true, false, 1>(pl, in, a, 4, st);
-                else if (xt == 2) e = masked ? launch<C3, true, true, 2>(pl, in, a, 7, st) : launch<C3, true, false, 2>(pl, in, a, 6, st);
-                else e = masked ? launch<C3, true, true, 3>(pl, in, a, 9, st) : launch<C3, true, false, 3>(pl, in, a, 8, st);
-            }
-            else if (three) e = masked ? launch<C3, true, true>(pl, in, a, 3, st) : launch<C3, true, false>(pl, in, a, 2, st);
-            else e = masked ? launch<C1, false, true>(pl, in, a, 1, st) : launch<C1, false, false>(pl, in, a, 0, st);
-            if (e == cudaSuccess && masked && stored_F)
-                e = lq_launch_fixup(three, g, ph, f, q[out], v[out], F[out], pl->np_list, pl->n_np, dsc, fc, pl->partials,
-                                    ncta, pl->partials2, pl->counter2, st);
-            if (e != cudaSuccess) { err = std::string("lq_sweep launch: ") + cudaGetErrorString(e); return LQ_ERR_CUDA; }
+            const int in = (int)((cur0 + done + i) & 1);
+            rc = lq_sweep_step(pl, stored_F, g, ph, f, q, v, F, in, dsc, fc, !stored_F && !fc.euler && done + i == 0, false, st, err);
+            if (rc != LQ_OK) return rc;
         }
         done += n;
         *launches += (masked && stored_F) ? 2 * n : n; *sweeps += n;

@@ -19,6 +19,15 @@ int lq_sweep_run(LqSweepPlan **plan, bool stored_F, const LqGeom &g, const LqPhy
                  double *v[2], double *F[2], int *cur, LqFireScalars *dsc, const LqFireConsts &fc, long max_steps,
                  cudaStream_t st, long *launches, long *sweeps, LqFireScalars *h, std::string &err, int rc_chunks = 0);
 
+// The same in pieces (sub-domains, lq_slab.cu, drive several contexts step by step): build the plan; one sweep; the
+// partial-sum segments that sweep left behind.
+int lq_sweep_prepare(LqSweepPlan **plan, bool stored_F, const LqGeom &g, const LqPhys &ph, const LqFields &f, double *q[2],
+                     double *v[2], double *F[2], cudaStream_t st, long *launches, std::string &err, int rc_chunks);
+int lq_sweep_step(LqSweepPlan *plan, bool stored_F, const LqGeom &g, const LqPhys &ph, const LqFields &f, double *q[2],
+                  double *v[2], double *F[2], int in, LqFireScalars *dsc, const LqFireConsts &fc, bool first, bool defer,
+                  cudaStream_t st, std::string &err, int phase = 0);
+int lq_sweep_segments(const LqSweepPlan *plan, bool stored_F, bool masked, bool first, LqPartialSeg seg[3]);
+
 // gradient descent / Nesterov (lq_descent.cu): one launch per step; buf[0] holds q_0, nbuf rotating buffers
 struct LqDescentPlan;
 void lq_descent_destroy(LqDescentPlan *plan);
@@ -48,4 +57,4 @@ int lq_fixup_num_blocks(int n);
 cudaError_t lq_launch_fixup(bool three, const LqGeom &g, const LqPhys &ph, const LqFields &f, const double *q,
                             double *v, double *F, const int *list, int n, LqFireScalars *sc, const LqFireConsts &fc,
                             const double *sweep_partials, int n_sweep, double *partials, unsigned int *counter,
-                            cudaStream_t st);
+                            cudaStream_t st, int defer = 0);

@@ -89,6 +89,8 @@ __device__ __forceinline__ void drift(double q, double vc, double F, double ma, 
 
 // ghost-shell shift of coordinate i in a periodic dimension of length L, ghost width gw (0 if interior)
 __device__ __forceinline__ int ghost_shift(int i, int L, int gw) { return i < gw ? L : (i >= L - gw ? -L : 0); }
+// same along z: a sub-domain (g.zopen) has no periodic image in z, its z ghost planes are the neighbours'
+__device__ __forceinline__ int ghost_shift_z(int k, const LqGeom &g) { return g.zopen ? 0 : ghost_shift(k, g.Lz, LQ_GH); }
 
 // End of a sweep: block-reduce r = (P, FF, vv, Fmax) partials, publish them, and let the LAST CTA to finish
 // reduce all CTAs' partials in index order (bitwise reproducible) and advance the FIRE schedule

@@ -284,7 +284,7 @@ k_sweep_rc(const __grid_constant__ CUtensorMap tq, const __grid_constant__ CUten
             }
             // periodic ghost shell of the outputs (width LQ_GH: the next sweep reads q with a 2-site halo)
             const int shx = ghost_shift(x, a.g.Lx, LQ_GH), shy = ghost_shift(y, a.g.Ly, LQ_GH),
-                      shz = ghost_shift(k, a.g.Lz, LQ_GH);
+                      shz = ghost_shift_z(k, a.g);
             if (shx | shy | shz) {
                 for (int m = 1; m < 8; ++m) {
                     if (((m & 1) && !shx) || ((m & 2) && !shy) || ((m & 4) && !shz)) continue;

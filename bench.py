@@ -221,6 +221,9 @@ def main():
     ap.add_argument("--fire-path", type=int, default=0)
     ap.add_argument("--method", default="fire", choices=["fire", "gd", "nesterov", "analyze"],
                     help="minimiser whose step is timed (default: FIRE, the headline metric; gd / nesterov: SURVEY 8(f1))")
+    ap.add_argument("--slabs", type=int, default=0,
+                    help="FIRE only: cut the lattice into this many z-slab sub-domains ON THIS GPU (SURVEY 8(f4): sweeps per "
+                         "slab + device-to-device halo copies + cross-domain reduction per step); 0 = undivided")
     ap.add_argument("--eta", type=float, default=0.004)
     ap.add_argument("--mu", type=float, default=0.8)
     args = ap.parse_args()
@@ -260,7 +263,17 @@ def main():
     hout = torch.empty((5, N), dtype=torch.float64, pin_memory=True)
     lq.lq_set_Q(ctx, hq)
 
-    if args.method == "fire":
+    slabs = None
+    if args.method == "fire" and args.slabs > 0:
+        from paper_1911_07045_b200 import parallel
+        slabs = parallel.make_slabs(lq, c, args.slabs)
+        for s_ in slabs:
+            lq.lq_set_stream(s_, stream.cuda_stream)
+            lq.lq_set_option(s_, "fire_path", args.fire_path)
+
+        def minimize(steps):
+            return lq.lq_slabs_fire_minimize(slabs, steps, 0.0, c["fire"])
+    elif args.method == "fire":
         def minimize(steps):
             return lq.lq_fire_minimize(ctx, steps, 0.0, c["fire"])
     elif args.method == "analyze":
@@ -303,7 +316,7 @@ def main():
 
     # e2e: host buffers in, K steps, host buffers out -- all inside the timed region
     e2e = None
-    if not args.no_e2e:
+    if not args.no_e2e and slabs is None:
         torch.cuda.synchronize()
         if dist is not None:
             dist.barrier()
@@ -334,7 +347,10 @@ def main():
     # initialisation rides on the first sweep there is nothing else inside those events (masked three-constant
     # lattices: the sweep plus its fix-up launch).  Units per launch = simulated sites.
     loop_ms = rep.get("gpu_ms") or ms
-    launch_ms = loop_ms / max(rep["sweep_launches"], 1)
+    nlaunch = max(rep["sweep_launches"], 1)
+    if slabs is not None:
+        nlaunch = max(rep["sweep_launches"] // len(slabs), 1)    # one "launch" = the sweeps of all slabs of one step
+    launch_ms = loop_ms / nlaunch
     achieved = alg_bytes_site * nsim / (launch_ms * 1e-3) / 1e9
     design_bytes_site = lq.lq_get_info(ctx, "sweep_bytes_per_site") if args.method == "fire" else alg_bytes_site
     three = c["L2"] != 0 or c["L3"] != 0
@@ -369,7 +385,8 @@ def main():
             "config": {"workload": c["name"], "lattice": [c["Lx"], c["Ly"], c["Lz"]], "n_simulated": nsim,
                        "elastic": "L1" if c["L2"] == 0 and c["L3"] == 0 else "L1+L2+L3",
                        "l2": "inputs_larger_than_L2" if 120.0 * N > 126e6 * 4 else "L2_resident_no_flush",
-                       "multi_gpu": "replicas only", "fire_path": args.fire_path, "method": args.method},
+                       "multi_gpu": "replicas only", "fire_path": args.fire_path, "method": args.method,
+                       "z_slabs_on_this_gpu": args.slabs},
             "clocks": clocks, "e2e": e2e, "gpu_launches": rep["launches"], "roofline": roofline,
             "cpu_baseline": cpu}
     print(json.dumps(line), flush=True)

@@ -71,8 +71,9 @@ k_sweep(const __grid_constant__ CUtensorMap tq, const __grid_constant__ CUtensor
     double *red = reinterpret_cast<double *>(smem + C::OFF_RED);
     const int tid = threadIdx.x;
     const int tx = tid % C::TX, ty = tid / C::TX;
-    const int x0 = blockIdx.x * C::TX, y0 = blockIdx.y * C::TY;
-    const int zb = blockIdx.z * a.zc, ze = min(a.g.Lz, zb + a.zc);
+    const int4 wk = a.work[blockIdx.x];          // (tile x, tile y, first plane, end plane), longest items first
+    const int x0 = wk.x * C::TX, y0 = wk.y * C::TY;
+    const int zb = wk.z, ze = wk.w;
     const int x = x0 + tx, y = y0 + ty;
     const bool active = x < a.g.Lx && y < a.g.Ly;
     const int nplanes = ze - zb + 2;             // planes zb-1 .. ze
@@ -85,7 +86,7 @@ k_sweep(const __grid_constant__ CUtensorMap tq, const __grid_constant__ CUtensor
     }
     uint8_t *ts = smem + C::OFF_TS;               // ts[i] = summary of plane zb+i
     if (MASKED && tid < ze - zb)
-        ts[tid] = a.tsum[((size_t)(zb + tid + 1) * gridDim.y + blockIdx.y) * gridDim.x + blockIdx.x];
+        ts[tid] = a.tsum[((size_t)(zb + tid + 1) * a.nty + wk.y) * a.ntx + wk.x];
     __syncthreads();
 
     auto issue = [&](int j) {
@@ -274,9 +275,7 @@ struct LqSweepPlan {
     unsigned int *counter2 = nullptr;
     const uint8_t *flags_seen = nullptr, *kind_seen = nullptr;
     bool sites_dirty = true;
-    dim3 grid;                                   // stored path: (tiles x, tiles y, z-chunks)
-    int zc = 0;
-    int4 *work = nullptr;                        // recompute path: work items, longest first
+    int4 *work = nullptr;                        // work items (tile, z-range), longest first
     int n_items = 0, ntx = 0, nty = 0, chunks_forced = 0;
     bool attr_set[12] = {}, attr_rc[4] = {};
 };
@@ -373,7 +372,7 @@ static cudaError_t launch(LqSweepPlan *pl, int in, const SweepArgs &a, int varia
         if (e != cudaSuccess) return e;
         pl->attr_set[variant] = true;
     }
-    k_sweep<C, THREE, MASKED, XT><<<pl->grid, C::NT, C::SMEM_BYTES, st>>>(pl->mq[in], pl->mv[in], pl->mF[in], a);
+    k_sweep<C, THREE, MASKED, XT><<<pl->n_items, C::NT, C::SMEM_BYTES, st>>>(pl->mq[in], pl->mv[in], pl->mF[in], a);
     return cudaGetLastError();
 }
 
@@ -419,34 +418,20 @@ int lq_sweep_prepare(LqSweepPlan **planp, bool stored_F, const LqGeom &g, const 
         pl->stored = stored_F;
         const int ntx = (g.Lx + TX - 1) / TX, nty = (g.Ly + TY - 1) / TY;
         pl->ntx = ntx; pl->nty = nty;
-        size_t ncta;
-        if (stored_F) {
-            // equal z-chunks of <= 64 planes; the chunk count minimises the modelled makespan
-            //   waves(ntiles * nzc / 148 SMs, 1 CTA/SM) * (planes per chunk + halo planes + pipeline fill)
-            long long best = -1;
-            int zc = g.Lz;
-            for (int nzc = 1; nzc <= (g.Lz + 3) / 4; ++nzc) {
-                const int c = (g.Lz + nzc - 1) / nzc;
-                if (c > 64 && nzc < (g.Lz + 63) / 64) continue;
-                const long long n = (long long)ntx * nty * ((g.Lz + c - 1) / c);
-                const long long cost = ((n + 147) / 148) * (c + 2 + 3);
-                if (best < 0 || cost < best) { best = cost; zc = c; }
-            }
-            pl->zc = zc;
-            pl->grid = dim3(ntx, nty, (g.Lz + zc - 1) / zc);
-            ncta = (size_t)pl->grid.x * pl->grid.y * pl->grid.z;
-        } else {
-            int nsm = 148;
-            int dev = 0;
-            if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
-            const std::vector<int4> items = lq_build_chunk_table(ntx, nty, g.Lz, lq_sweep_rc_max_chunk(), 7, nsm, rc_chunks);
-            cudaFree(pl->work); pl->work = nullptr;
-            LQ_PLAN_CUDA(cudaMalloc(&pl->work, items.size() * sizeof(int4)));
-            // pageable host source: the copy is staged before the call returns, `items` may go out of scope
-            LQ_PLAN_CUDA(cudaMemcpyAsync(pl->work, items.data(), items.size() * sizeof(int4), cudaMemcpyHostToDevice, st));
-            pl->n_items = (int)items.size();
-            ncta = items.size();
-        }
+        // z-chunks per tile column: the work table of lq_build_chunk_table (both sweeps; a chunk costs its planes
+        // plus the halo planes and the pipeline fill: 4 + 3 for the recompute sweep, 2 + 3 for the stored-force one,
+        // whose tile-summary array caps a chunk at 128 planes)
+        int nsm = 148;
+        int dev = 0;
+        if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
+        const std::vector<int4> items = stored_F ? lq_build_chunk_table(ntx, nty, g.Lz, 126, 5, nsm, rc_chunks)
+                                                 : lq_build_chunk_table(ntx, nty, g.Lz, lq_sweep_rc_max_chunk(), 7, nsm, rc_chunks);
+        cudaFree(pl->work); pl->work = nullptr;
+        LQ_PLAN_CUDA(cudaMalloc(&pl->work, items.size() * sizeof(int4)));
+        // pageable host source: the copy is staged before the call returns, `items` may go out of scope
+        LQ_PLAN_CUDA(cudaMemcpyAsync(pl->work, items.data(), items.size() * sizeof(int4), cudaMemcpyHostToDevice, st));
+        pl->n_items = (int)items.size();
+        const size_t ncta = items.size();
         cudaFree(pl->partials); cudaFree(pl->partials0); cudaFree(pl->counter);
         pl->partials = pl->partials0 = nullptr; pl->counter = nullptr;
         LQ_PLAN_CUDA(cudaMalloc(&pl->partials, ncta * 4 * sizeof(double)));
@@ -497,12 +482,12 @@ int lq_sweep_step(LqSweepPlan *pl, bool stored_F, const LqGeom &g, const LqPhys 
     const int out = in ^ 1;
     SweepArgs a;
     memset(&a, 0, sizeof(a));
-    a.g = g; a.ph = ph; a.f = f; a.sc = dsc; a.fc = fc; a.partials = pl->partials; a.counter = pl->counter; a.zc = pl->zc;
+    a.g = g; a.ph = ph; a.f = f; a.sc = dsc; a.fc = fc; a.partials = pl->partials; a.counter = pl->counter;
     a.plain = pl->plain; a.tsum = pl->tsum; a.bond = pl->bond; a.work = pl->work; a.ntx = pl->ntx; a.nty = pl->nty;
     a.partials0 = pl->partials0;
     a.defer_advance = (defer || (masked && stored_F)) ? 1 : 0;
     a.qo = q[out]; a.vo = v[out]; a.Fo = F[out];
-    const int ncta = stored_F ? (int)(pl->grid.x * pl->grid.y * pl->grid.z) : pl->n_items;
+    const int ncta = pl->n_items;
     cudaError_t e = cudaSuccess;
     if (phase == 2) { /* fix-up only: the sweep of this step has run (sub-domains exchange q' in between) */ }
     else if (!stored_F)
@@ -525,7 +510,7 @@ int lq_sweep_step(LqSweepPlan *pl, bool stored_F, const LqGeom &g, const LqPhys 
 // partial-sum segments of the last sweep (for the cross-domain reduction): returns how many were written (<= 3)
 int lq_sweep_segments(const LqSweepPlan *pl, bool stored_F, bool masked, bool first, LqPartialSeg seg[3]) {
     int n = 0;
-    const int ncta = stored_F ? (int)(pl->grid.x * pl->grid.y * pl->grid.z) : pl->n_items;
+    const int ncta = pl->n_items;
     seg[n++] = LqPartialSeg{pl->partials, ncta, 4};
     if (stored_F && masked) seg[n++] = LqPartialSeg{pl->partials2, lq_fixup_num_blocks(pl->n_np), 4};
     if (first) seg[n++] = LqPartialSeg{pl->partials0, ncta, 2};

@@ -15,14 +15,13 @@ struct SweepArgs {
     LqFireConsts fc;
     double *partials;
     unsigned int *counter;
-    int zc;
     const uint8_t *plain;   // stored-force sweep, masked lattices: per-site 'constant stencil weights' byte
     const uint8_t *tsum;    // per (plane, tile): tile + halo all plain
     int defer_advance;      // stored-force sweep on masked lattices: the fix-up kernel (lq_fixup.cu) finishes the step
-    // recompute sweep (lq_sweep_rc.cu)
-    const uint32_t *bond;   // masked lattices: per-site bond code (LQ_BOND_*), ghost margin of 1 filled
     const int4 *work;       // work items (tile x, tile y, first plane, end plane), longest first; one per CTA
     int ntx, nty;           // tiles per row / column (indexing of tsum)
+    // recompute sweep (lq_sweep_rc.cu)
+    const uint32_t *bond;   // masked lattices: per-site bond code (LQ_BOND_*), ghost margin of 1 filled
     double *partials0;      // first sweep: per-CTA (|F(q_0)|^2, max|F_a(q_0)|) of the initial state
 };
 

@@ -124,14 +124,22 @@ k_sweep_rc(const __grid_constant__ CUtensorMap tq, const __grid_constant__ CUten
     double r[4] = {0.0, 0.0, 0.0, 0.0};
     double r0[2] = {0.0, 0.0};
 
-    // halo share: perimeter cell (hx, hy) of the 34 x 18 q' box; own cell is (tx+1, ty+1)
+    // halo share: perimeter cell (hx, hy) of the 34 x 18 q' box; own cell is (tx+1, ty+1).  The 100 perimeter cells
+    // go to the first four warps, 25 lanes each: 8 side cells (4 consecutive rows, left and right) + 17 cells of the
+    // top / bottom rows.  A column of the 36-wide TMA box strides 72 banks = 8 (mod 32), so rows 4 apart collide:
+    // with at most one row of each residue per warp the side cells' shared-memory accesses are conflict-free among
+    // themselves (all 32 side cells in one warp, as before, made every one of its accesses 4-way conflicted).
     int hx = -1, hy = -1;
-    if (tid < RC::NHALO) {
-        int h = tid;
-        if (h < RC::BXW) { hx = h; hy = 0; }
-        else if (h < 2 * RC::BXW) { hx = h - RC::BXW; hy = RC::BYH - 1; }
-        else { h -= 2 * RC::BXW; hy = 1 + (h >> 1); hx = (h & 1) ? RC::BXW - 1 : 0; }
+    if (tid < 128) {
+        const int w = tid >> 5, l = tid & 31;
+        if (l < 8) { hy = 1 + 4 * w + (l >> 1); hx = (l & 1) ? RC::BXW - 1 : 0; }
+        else if (l < 25) {
+            const int t = 17 * w + (l - 8);                  // 0 .. 67: top row, then bottom row
+            if (t < RC::BXW) { hx = t; hy = 0; }
+            else { hx = t - RC::BXW; hy = RC::BYH - 1; }
+        }
     }
+    static_assert(RC::TY == 16 && 4 * 17 == 2 * RC::BXW, "halo mapping assumes a 32 x 16 tile");
 
     // Bond codes (masked lattices) of the own cell and the halo cell: cp.async'd into shared memory one plane ahead,
     // and only for planes whose tile + halo holds a non-plain site, so that (i) no dependent global load gates a

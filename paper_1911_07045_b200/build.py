@@ -12,7 +12,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(CSRC, "liblq.so")
-SOURCES = ["lq_api.cu", "lq_kernels.cu", "lq_sweep.cu", "lq_sweep_rc.cu", "lq_fixup.cu", "lq_descent.cu", "lq_analyze.cu", "lq_slab.cu"]
+SOURCES = ["lq_api.cu", "lq_kernels.cu", "lq_sweep.cu", "lq_sweep_rc.cu", "lq_fixup.cu", "lq_descent.cu", "lq_analyze.cu", "lq_slab.cu", "lq_resident.cu"]
 HEADERS = ["lq_internal.cuh", "lq_site.cuh", "lq_sweep.cuh", "lq_sweep_dev.cuh", "lq_ctx.cuh", os.path.join("..", "..", "include", "lq.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC",

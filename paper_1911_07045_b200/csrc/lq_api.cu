@@ -118,6 +118,7 @@ void lq_destroy(lq_ctx *c) {
     DeviceGuard dg(c);
     if (c->ev0) cudaEventDestroy(c->ev0);
     if (c->ev1) cudaEventDestroy(c->ev1);
+    cudaFree(c->res_bond);
     cudaFree(c->scratch); cudaFree(c->dtot); cudaFree(c->dsegs); cudaFree(c->dscptr);
     for (int i = 0; i < 2; ++i) { cudaFree(c->q[i]); cudaFree(c->v[i]); cudaFree(c->F[i]); }
     cudaFree(c->maskp); cudaFree(c->flags); cudaFree(c->kind); cudaFree(c->W); cudaFree(c->axis);
@@ -146,6 +147,7 @@ int lq_set_sites(lq_ctx *c, const uint8_t *mask, const uint8_t *anch_kind, const
     if (!mask) {
         lq_sweep_invalidate(c->sweep);
         lq_descent_invalidate(c->descent);
+        c->res_bond_dirty = true;
         c->flags_active = false; c->anch_active = false;
         c->n_class[0] = (unsigned long long)g.N; c->n_class[1] = c->n_class[2] = 0;
         return LQ_OK;
@@ -171,6 +173,7 @@ int lq_set_sites(lq_ctx *c, const uint8_t *mask, const uint8_t *anch_kind, const
     LQ_CUDA(c, cudaStreamSynchronize(st));
     lq_sweep_invalidate(c->sweep);
     lq_descent_invalidate(c->descent);
+    c->res_bond_dirty = true;
     if (bad[0] || (anch_kind && bad[1])) {
         c->flags_active = false; c->anch_active = false;
         c->n_class[0] = (unsigned long long)g.N; c->n_class[1] = c->n_class[2] = 0;
@@ -315,6 +318,11 @@ int lq_set_option(lq_ctx *c, const char *key, double value) {
         c->fire_path = (int)value;
         return LQ_OK;
     }
+    if (!strcmp(key, "resident")) {
+        if (value != 0.0 && value != 1.0) return fail(c, LQ_ERR_ARG, "resident must be 0 or 1");
+        c->resident = (int)value;
+        return LQ_OK;
+    }
     if (!strcmp(key, "rc_chunks")) {
         if (!(value >= 0.0 && value <= 4096.0)) return fail(c, LQ_ERR_ARG, "rc_chunks must be in [0, 4096]");
         c->rc_chunks = (int)value;
@@ -377,7 +385,41 @@ int lq_fire_minimize(lq_ctx *c, long max_steps, double force_tol, const lq_fire_
     long launches = 0, sweeps = 0;
     LQ_CUDA(c, cudaEventRecord(c->ev0, st));
 
-    if (fused) {
+    bool done_resident = false;
+    int rdims[6];
+    int nsm = 148;
+    cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, c->device);
+    if (fused && !stored_F && !euler && c->resident && lq_resident_plan(g, nsm, rdims)) {
+        // small lattice: the whole call is ONE cooperative launch with the state resident on chip (lq_resident.cu)
+        const int ncta = rdims[0] * rdims[1] * rdims[2];
+        if ((rc = ensure_partials(c, (size_t)6 * ncta)) != LQ_OK) return rc;
+        if (f.flags && c->res_bond_dirty) {
+            if (!c->res_bond) LQ_CUDA(c, cudaMalloc(&c->res_bond, (size_t)g.NP * sizeof(uint32_t)));
+            LQ_CUDA(c, cudaMemsetAsync(c->res_bond, 0, (size_t)g.NP * sizeof(uint32_t), st));
+            lq_launch_bond_map(g, f.flags, f.kind, c->res_bond, st);
+            c->res_bond_dirty = false;
+            launches += 1;
+        }
+        h.dt = fp->dt0; h.alpha = fp->alpha0;
+        LQ_CUDA(c, cudaMemcpyAsync(&c->dsc[0], &h, sizeof(h), cudaMemcpyHostToDevice, st));
+        cudaError_t e = lq_launch_fire_resident(g, c->ph, f, c->q[c->cur], c->v[c->cur], f.flags ? c->res_bond : nullptr,
+                                                c->dsc, fc, c->partials, rdims, st);
+        if (e == cudaSuccess) {
+            // the kernel rewrote the interior of q and v: refresh their periodic ghost shells for whatever runs next
+            lq_launch_fill_ghosts_f64(g, c->q[c->cur], 5, st);
+            lq_launch_fill_ghosts_f64(g, c->v[c->cur], 5, st);
+            LQ_CUDA(c, cudaMemcpyAsync(&h, &c->dsc[0], sizeof(h), cudaMemcpyDeviceToHost, st));
+            launches += 3; sweeps += 1;
+            done_resident = true;
+        } else if (e != cudaErrorCooperativeLaunchTooLarge) {
+            return fail(c, LQ_ERR_CUDA, std::string("lq_fire_minimize (resident kernel): ") + cudaGetErrorString(e));
+        } else {
+            cudaGetLastError();          // not co-resident on this device: the streaming sweeps take over
+            memset(&h, 0, sizeof(h));
+        }
+    }
+    if (done_resident) {
+    } else if (fused) {
         // Algorithm 1's initialisation (v = 0, dt0, alpha0, force of the initial state and the stop test on it) is
         // part of the first sweep: mix_a = mix_b = 0 makes it ignore whatever the velocity buffer holds, the
         // recompute sweep reduces max|F(q_0)| in its first phase, the stored-force path starts with one sweep whose

@@ -38,6 +38,9 @@ struct lq_ctx {
     int fire_cur0 = 0, fire_buf = 0;     // live buffer when the run began / buffer the last sweep wrote
     bool fire_sweep_pending = false;     // lq_fire_step_local ran, lq_fire_step_finish not yet
     bool fire_last_first = false;        // the last sweep was the FIRST instantiation (its stop test is on q_0)
+    int resident = 1;                    // "resident" option: small one-constant lattices run the on-chip kernel
+    uint32_t *res_bond = nullptr;        // bond codes for the resident kernel (masked lattices)
+    bool res_bond_dirty = true;
     int fire_path = 0;
     int rc_chunks = 0;                   // "rc_chunks" option: 0 = chunk table chosen by the makespan model
     bool v_valid = false;                // v[cur] holds the velocities of the last lq_fire_minimize (else: report zeros)

@@ -58,3 +58,9 @@ cudaError_t lq_launch_fixup(bool three, const LqGeom &g, const LqPhys &ph, const
                             double *v, double *F, const int *list, int n, LqFireScalars *sc, const LqFireConsts &fc,
                             const double *sweep_partials, int n_sweep, double *partials, unsigned int *counter,
                             cudaStream_t st, int defer = 0);
+
+// FIRE with the state resident on chip: one cooperative launch per lq_fire_minimize call (lq_resident.cu)
+bool lq_resident_plan(const LqGeom &g, int nsm, int dims[6]);
+cudaError_t lq_launch_fire_resident(const LqGeom &g, const LqPhys &ph, const LqFields &f, double *q, double *v,
+                                    const uint32_t *bond, LqFireScalars *sc, const LqFireConsts &fc, double *partials,
+                                    const int dims[6], cudaStream_t st);

@@ -312,3 +312,35 @@ def test_device_buffers_and_stream(lq):
     assert np.array_equal(fl.cpu().numpy(), lq.lq_get_flags(ctx))
     lq.lq_destroy(ctx)
     lq.lq_destroy(ctx2)
+
+
+@pytest.mark.parametrize("name", ["cfg1", "masked_70x35x9_L1only", "masked_5x4x6_L1"])
+def test_resident_kernel_matches_streaming_sweeps_and_oracle(lq, oracle_mod, name):
+    """Small one-constant lattices run lq_fire_minimize as ONE cooperative launch with the state on chip
+    (lq_resident.cu); "resident" = 0 forces the streaming sweep on the same context.  Both against the oracle
+    (100 steps, 1e-8) and against each other; the resident run reports a single launch of the fused kernel."""
+    if name == "masked_5x4x6_L1":
+        c = wl.random_masked_problem(106, 5, 4, 6, obj_frac=0.25, L2=0.0, L3=0.0)
+    else:
+        c = SMALL_CASES[name]()
+    ctx = lq.create_from_config(c)
+    o = make_oracle(oracle_mod, c)
+    qref, rref, vref = o.fire(c["q"], 100, 0.0, c["fire"], variant=1, return_v=True)
+    out = {}
+    for resident in (1, 0):
+        lq.lq_set_option(ctx, "resident", resident)
+        lq.lq_set_Q(ctx, c["q"])
+        rep = lq.lq_fire_minimize(ctx, 100, 0.0, c["fire"], report_energy=True)
+        q, v = lq.lq_get_Q(ctx), lq.lq_get_velocity(ctx)
+        assert rep["steps"] == 100 and rep["converged"] == 0
+        assert rep["sweep_launches"] == (1 if resident else 100)
+        assert np.abs(q - qref).max() <= TOL_Q100
+        assert np.abs(v - vref).max() <= 1e-7 * max(np.abs(vref).max(), 1e-3)
+        assert abs(rep["energy"] - rref["energy"]) <= TOL_E * abs(rref["energy"])
+        assert abs(rep["dt"] - rref["dt"]) <= 1e-15 and abs(rep["alpha"] - rref["alpha"]) <= 1e-15
+        # ghost shell left current: the generic force kernel (reads neighbours through the ghosts) agrees with the oracle
+        Fref = o.forces(qref, 1)
+        assert np.abs(lq.lq_forces(ctx) - Fref).max() <= 1e-7 * np.abs(Fref).max()
+        out[resident] = q
+    assert np.abs(out[0] - out[1]).max() <= 1e-11
+    lq.lq_destroy(ctx)

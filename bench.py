@@ -351,7 +351,10 @@ def main():
     if slabs is not None:
         nlaunch = max(rep["sweep_launches"] // len(slabs), 1)    # one "launch" = the sweeps of all slabs of one step
     launch_ms = loop_ms / nlaunch
-    achieved = alg_bytes_site * nsim / (launch_ms * 1e-3) / 1e9
+    # on-chip resident kernel (small lattices): ONE launch runs all K steps
+    resident = args.method == "fire" and slabs is None and rep["sweep_launches"] == 1 and K > 1
+    sites_per_launch = nsim * (K if resident else 1)
+    achieved = alg_bytes_site * sites_per_launch / (launch_ms * 1e-3) / 1e9
     design_bytes_site = lq.lq_get_info(ctx, "sweep_bytes_per_site") if args.method == "fire" else alg_bytes_site
     three = c["L2"] != 0 or c["L3"] != 0
     if args.method == "analyze":
@@ -370,8 +373,12 @@ def main():
     roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                 "traffic": traffic, "peak_kind": peak_kind, "kernel": kernel_name,
                 "algorithmic_bytes_per_site": alg_bytes_site, "design_bytes_per_site": design_bytes_site,
-                "achieved_design_GBs": design_bytes_site * nsim / (launch_ms * 1e-3) / 1e9,
-                "launch_ms": launch_ms, "launches_timed": rep["sweep_launches"], "sites_per_launch": nsim}
+                "achieved_design_GBs": design_bytes_site * sites_per_launch / (launch_ms * 1e-3) / 1e9,
+                "launch_ms": launch_ms, "launches_timed": rep["sweep_launches"], "sites_per_launch": sites_per_launch}
+    if resident:
+        roofline["kernel"] = "k_fire_resident"
+        roofline["note"] = ("state resident on chip: the algorithmic bytes never touch HBM, the step is bound by two grid "
+                            "barriers; no roofline claim (SURVEY 8(d): configs 1-2 are latency-bound)")
 
     cpu = None
     if not args.no_cpu_baseline:

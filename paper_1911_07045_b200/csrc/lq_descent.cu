@@ -203,9 +203,9 @@ __device__ __forceinline__ void force1(const LqPhys &ph, const double q[5], cons
 // 4-D TMA boxes (36 x 18 x 1 x 5: tile + 1 halo; the innermost start coordinate must be 16-byte aligned, hence
 // x0-2) into an NS-slot mbarrier ring.  A thread keeps the look-ahead column y(z-1), y(z), y(z+1) of its site in
 // registers and reads the four in-plane neighbours from the landed boxes; y is formed on the fly.
-template <bool NEST, int NS_>
+template <bool NEST, int NS_, int TY_ = 16>
 struct DS {
-    static constexpr int TX = 32, TY = 16, NT = TX * TY, NS = NS_;
+    static constexpr int TX = 32, TY = TY_, NT = TX * TY, NS = NS_;
     static constexpr int SW = TX + 4, SH = TY + 2, SPLANE = SW * SH;
     static constexpr int BOX_BYTES = 5 * SPLANE * 8, BOX_STRIDE = (BOX_BYTES + 127) / 128 * 128;
     static constexpr int NF = NEST ? 2 : 1;
@@ -218,11 +218,13 @@ struct DS {
 // THREE: L2/L3 != 0 -- the 19-point constant-weight stencil (lqs::bulk_force_threeconst) reads planes k-1, k, k+1
 // from the ring (three live slots instead of two).
 // XT: extra distortion terms in the 19-point stencil (bit 0 chiral L4, bit 1 cubic L6)
+// The cubic-term (L6) instantiations run 32 x 8 tiles of 256 threads: their 19-point cubic stencil needs the
+// 255-register budget (at 128 registers it spilled ~800 B per thread).
 template <bool NEST, bool MASKED, bool THREE, int XT, int NS>
-__global__ void __launch_bounds__(512, 1)
+__global__ void __launch_bounds__(((XT & 2) ? 8 : 16) * 32, 1)
 k_descent_sweep(const __grid_constant__ CUtensorMap tq, const __grid_constant__ CUtensorMap tp, const DescArgs a,
                 const uint8_t *__restrict__ plain, int zc) {
-    using C = DS<NEST, NS>;
+    using C = DS<NEST, NS, (XT & 2) ? 8 : 16>;
     extern __shared__ __align__(1024) unsigned char smem[];
     __shared__ unsigned s_last;
     if (a.sc->converged) return;
@@ -328,6 +330,7 @@ struct LqDescentPlan {
     // one-constant fast path
     CUtensorMap map[3];
     double *mapped[3] = {nullptr, nullptr, nullptr};
+    int map_ty = 0;                   // tile rows the maps' boxes were made for
     uint8_t *plain = nullptr;         // per-site plain byte (masked lattices)
     int *list = nullptr;              // index-ordered non-plain simulated sites
     int n_list = 0;
@@ -356,7 +359,7 @@ template <bool NEST, bool MASKED, bool THREE, int XT = 0>
 cudaError_t launch_sweep_t(LqDescentPlan *pl, dim3 grid, const CUtensorMap &mq, const CUtensorMap &mp, const DescArgs &a,
                            int zc, cudaStream_t st) {
     constexpr int NS = NEST ? NS_NEST : NS_GD;
-    using C = DS<NEST, NS>;
+    using C = DS<NEST, NS, (XT & 2) ? 8 : 16>;
     const int v = 8 * XT + (THREE ? 4 : 0) + (NEST ? 2 : 0) + (MASKED ? 1 : 0);
     if (!pl->attr_set[v]) {
         cudaError_t e = cudaFuncSetAttribute(k_descent_sweep<NEST, MASKED, THREE, XT, NS>,
@@ -400,12 +403,14 @@ int lq_descent_run(LqDescentPlan **planp, int method, int path, const LqGeom &g,
     dim3 grid(1, 1, 1);
     int zc = g.Lz;
     if (fast) {
+        const int TY = (three && ph.L6 != 0.0) ? 8 : 16;       // tile rows: see k_descent_sweep
         for (int i = 0; i < nbuf; ++i)
-            if (pl->mapped[i] != buf[i]) {
-                if (!lq_make_box_map(&pl->map[i], g, buf[i], 36, 18)) { err = "lq_descent: cuTensorMapEncodeTiled failed"; return LQ_ERR_CUDA; }
+            if (pl->mapped[i] != buf[i] || pl->map_ty != TY) {
+                if (!lq_make_box_map(&pl->map[i], g, buf[i], 36, TY + 2)) { err = "lq_descent: cuTensorMapEncodeTiled failed"; return LQ_ERR_CUDA; }
                 pl->mapped[i] = buf[i];
             }
-        const int ntx = (g.Lx + 31) / 32, nty = (g.Ly + 15) / 16;
+        pl->map_ty = TY;
+        const int ntx = (g.Lx + 31) / 32, nty = (g.Ly + TY - 1) / TY;
         long long best = -1;
         for (int nzc = 1; nzc <= (g.Lz + 3) / 4; ++nzc) {          // equal chunks, modelled makespan on 148 SMs
             const int c = (g.Lz + nzc - 1) / nzc;

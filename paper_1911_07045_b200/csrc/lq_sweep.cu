@@ -276,7 +276,7 @@ struct LqSweepPlan {
     const uint8_t *flags_seen = nullptr, *kind_seen = nullptr;
     bool sites_dirty = true;
     int4 *work = nullptr;                        // work items (tile, z-range), longest first
-    int n_items = 0, ntx = 0, nty = 0, chunks_forced = 0;
+    int n_items = 0, ntx = 0, nty = 0, chunks_forced = 0, ty = 0;
     bool attr_set[12] = {}, attr_rc[4] = {};
 };
 
@@ -387,8 +387,6 @@ static cudaError_t launch(LqSweepPlan *pl, int in, const SweepArgs &a, int varia
 
 int lq_sweep_prepare(LqSweepPlan **planp, bool stored_F, const LqGeom &g, const LqPhys &ph, const LqFields &f, double *q[2],
                      double *v[2], double *F[2], cudaStream_t st, long *launches, std::string &err, int rc_chunks) {
-    using C1 = Cfg<32, 16>;
-    using C3 = Cfg<32, 16>;
     const bool three = lq_three(ph);
     const bool masked = f.flags != nullptr;
     LqSweepPlan *pl = *planp;
@@ -397,9 +395,13 @@ int lq_sweep_prepare(LqSweepPlan **planp, bool stored_F, const LqGeom &g, const 
         *planp = pl;
     }
     if (three && !stored_F) { err = "lq_sweep: the recompute path is one-constant only"; return LQ_ERR_ARG; }
-    const int TX = 32, TY = !stored_F ? lq_sweep_rc_tile(1) : (three ? C3::TY : C1::TY);
-    bool rebuild = pl->three != three || pl->stored != stored_F || pl->partials == nullptr || pl->chunks_forced != rc_chunks;
+    // stored-force sweep: 32 x 16 tiles; with the cubic term (L6) 32 x 8 tiles of 256 threads, whose 255-register
+    // budget holds the 19-point cubic stencil without spills
+    const int TX = 32, TY = !stored_F ? lq_sweep_rc_tile(1) : (ph.L6 != 0.0 ? 8 : 16);
+    bool rebuild = pl->three != three || pl->stored != stored_F || pl->partials == nullptr || pl->chunks_forced != rc_chunks ||
+                   pl->ty != TY;
     pl->chunks_forced = rc_chunks;
+    pl->ty = TY;
     for (int i = 0; i < 2; ++i) rebuild |= pl->bq[i] != q[i] || pl->bv[i] != v[i] || (stored_F && pl->bF[i] != F[i]);
     if (rebuild) {
         for (int i = 0; i < 2; ++i) {
@@ -477,6 +479,7 @@ int lq_sweep_step(LqSweepPlan *pl, bool stored_F, const LqGeom &g, const LqPhys 
                   cudaStream_t st, std::string &err, int phase) {
     using C1 = Cfg<32, 16>;
     using C3 = Cfg<32, 16>;
+    using C6 = Cfg<32, 8>;      // cubic term: see lq_sweep_prepare
     const bool three = lq_three(ph);
     const bool masked = f.flags != nullptr;
     const int out = in ^ 1;
@@ -495,8 +498,8 @@ int lq_sweep_step(LqSweepPlan *pl, bool stored_F, const LqGeom &g, const LqPhys 
     else if (three && (ph.L4 != 0.0 || ph.L6 != 0.0)) {
         const int xt = (ph.L4 != 0.0 ? 1 : 0) | (ph.L6 != 0.0 ? 2 : 0);
         if (xt == 1) e = masked ? launch<C3, true, true, 1>(pl, in, a, 5, st) : launch<C3, true, false, 1>(pl, in, a, 4, st);
-        else if (xt == 2) e = masked ? launch<C3, true, true, 2>(pl, in, a, 7, st) : launch<C3, true, false, 2>(pl, in, a, 6, st);
-        else e = masked ? launch<C3, true, true, 3>(pl, in, a, 9, st) : launch<C3, true, false, 3>(pl, in, a, 8, st);
+        else if (xt == 2) e = masked ? launch<C6, true, true, 2>(pl, in, a, 7, st) : launch<C6, true, false, 2>(pl, in, a, 6, st);
+        else e = masked ? launch<C6, true, true, 3>(pl, in, a, 9, st) : launch<C6, true, false, 3>(pl, in, a, 8, st);
     }
     else if (three) e = masked ? launch<C3, true, true>(pl, in, a, 3, st) : launch<C3, true, false>(pl, in, a, 2, st);
     else e = masked ? launch<C1, false, true>(pl, in, a, 1, st) : launch<C1, false, false>(pl, in, a, 0, st);

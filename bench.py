@@ -377,8 +377,8 @@ def main():
                 "launch_ms": launch_ms, "launches_timed": rep["sweep_launches"], "sites_per_launch": sites_per_launch}
     if resident:
         roofline["kernel"] = "k_fire_resident"
-        roofline["note"] = ("state resident on chip: the algorithmic bytes never touch HBM, the step is bound by two grid "
-                            "barriers; no roofline claim (SURVEY 8(d): configs 1-2 are latency-bound)")
+        roofline["note"] = ("state resident on chip: the algorithmic bytes never touch HBM, the step is bound by its grid "
+                            "barrier; no roofline claim (SURVEY 8(d): configs 1-2 are latency-bound)")
 
     cpu = None
     if not args.no_cpu_baseline:

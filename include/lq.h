@@ -277,8 +277,8 @@ int lq_get_S0(lq_ctx *ctx, double *S0);
  *                      rest, 1 = general kernel on every site
  *   "resident" (set):  1 (default) = one-constant lattices small enough to live on chip (bricks of <= 512 sites on
  *                      <= one CTA per SM, about 75 000 sites on a B200) run lq_fire_minimize (integrator 0,
- *                      fire_path 0) as ONE cooperative launch with q, v, F in registers / shared memory and two grid
- *                      barriers per step; report.sweep_launches is then 1.  0 = always the streaming sweeps
+ *                      fire_path 0) as ONE cooperative launch with q, v, F in registers / shared memory and one grid
+ *                      barrier per step; report.sweep_launches is then 1.  0 = always the streaming sweeps
  *   "rc_chunks" (set): recompute sweep: 0 = z-chunks per tile column chosen by the makespan model (default),
  *                      n > 0 = n equal chunks per column (clamped to chunks of 4 .. 126 planes)
  *   "sweep_bytes_per_site" (get): algorithmic HBM bytes one sweep moves per site

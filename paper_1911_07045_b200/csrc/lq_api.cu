@@ -392,7 +392,9 @@ int lq_fire_minimize(lq_ctx *c, long max_steps, double force_tol, const lq_fire_
     if (fused && !stored_F && !euler && c->resident && lq_resident_plan(g, nsm, rdims)) {
         // small lattice: the whole call is ONE cooperative launch with the state resident on chip (lq_resident.cu)
         const int ncta = rdims[0] * rdims[1] * rdims[2];
-        if ((rc = ensure_partials(c, (size_t)6 * ncta)) != LQ_OK) return rc;
+        if ((rc = ensure_partials(c, (size_t)10 * ncta)) != LQ_OK) return rc;
+        for (int i = 0; i < 2; ++i)
+            if ((rc = lq_ensure_field(c, &c->F[i])) != LQ_OK) return rc;
         if (f.flags && c->res_bond_dirty) {
             if (!c->res_bond) LQ_CUDA(c, cudaMalloc(&c->res_bond, (size_t)g.NP * sizeof(uint32_t)));
             LQ_CUDA(c, cudaMemsetAsync(c->res_bond, 0, (size_t)g.NP * sizeof(uint32_t), st));
@@ -402,13 +404,16 @@ int lq_fire_minimize(lq_ctx *c, long max_steps, double force_tol, const lq_fire_
         }
         h.dt = fp->dt0; h.alpha = fp->alpha0;
         LQ_CUDA(c, cudaMemcpyAsync(&c->dsc[0], &h, sizeof(h), cudaMemcpyHostToDevice, st));
-        cudaError_t e = lq_launch_fire_resident(g, c->ph, f, c->q[c->cur], c->v[c->cur], f.flags ? c->res_bond : nullptr,
+        cudaError_t e = lq_launch_fire_resident(g, c->ph, f, c->q, c->v, c->F, c->cur, f.flags ? c->res_bond : nullptr,
                                                 c->dsc, fc, c->partials, rdims, st);
         if (e == cudaSuccess) {
-            // the kernel rewrote the interior of q and v: refresh their periodic ghost shells for whatever runs next
+            LQ_CUDA(c, cudaMemcpyAsync(&h, &c->dsc[0], sizeof(h), cudaMemcpyDeviceToHost, st));
+            LQ_CUDA(c, cudaStreamSynchronize(st));
+            // the final state sits in the buffer the last step wrote; the kernel writes interiors only: refresh the
+            // periodic ghost shells of q and v for whatever runs next
+            c->cur = (int)((c->cur + h.step) & 1);
             lq_launch_fill_ghosts_f64(g, c->q[c->cur], 5, st);
             lq_launch_fill_ghosts_f64(g, c->v[c->cur], 5, st);
-            LQ_CUDA(c, cudaMemcpyAsync(&h, &c->dsc[0], sizeof(h), cudaMemcpyDeviceToHost, st));
             launches += 3; sweeps += 1;
             done_resident = true;
         } else if (e != cudaErrorCooperativeLaunchTooLarge) {

@@ -4,13 +4,15 @@
 // (BASELINE.json config 1: 32^3 = 2.6 MB of state) one step of them is pure latency: a launch, a TMA pipeline fill
 // per z-chunk, a tail.  Here ONE cooperative launch runs the whole lq_fire_minimize call: every CTA owns one brick of
 // the lattice for the entire run, keeps q, v and the force of its sites in registers and the brick's q' (+ a one-site
-// halo) in shared memory, and the only traffic per step is the brick surfaces through L2 and two grid barriers
-// (Algorithm 1):
-//     v_k = mix_a v + (mix_b + dt/2) F ;  q' = q + dt v_k       own sites; q' also goes to the global array
-//     -- grid barrier --                                          neighbours' q' visible
-//     halo of q' from the global array (periodic index wrap) ;  F' = force(q') ;  v' = v_k + dt/2 F'
+// halo) in shared memory, and the only traffic per step is the brick surfaces through L2 and ONE grid barrier
+// (Algorithm 1).  As in the streaming sweeps, q' of a site is a pointwise
+// function of that site's (q, vc, F) and the step's global scalars, so a CTA recomputes the q' of its halo cells
+// from its neighbours' state instead of waiting for them to publish it:
+//     v_k = mix_a vc + (mix_b + dt/2) F ;  q' = q + dt v_k       own sites (registers) and halo cells (state of the
+//                                                                 neighbour bricks, read from global buffer `in`)
+//     F' = force(q') ;  vc' = v_k + dt/2 F'                      own sites; (q', vc', F') -> global buffer `out`
 //     per-CTA (P, |F|^2, |v|^2, max|F|) -> global               block reduction in a fixed order
-//     -- grid barrier --
+//     -- grid barrier --                                          (state and partials ping-pong by step parity)
 //     every CTA reduces all CTAs' partials in index order and advances dt, alpha, N_pos (same bits everywhere)
 // The stop test, the step cap and the initial-state test of Algorithm 1 are evaluated on the device; the host launches
 // once and reads the scalars back.  Masked lattices: the per-site bond code (weighted 7-point stencil) and the
@@ -32,12 +34,12 @@ struct ResArgs {
     LqGeom g;
     LqPhys ph;
     LqFields f;
-    double *q;              // padded global Q: read at the start, its interior rewritten every step (halo exchange)
-    double *v;              // padded global velocity: written once at the end (the un-rescaled v of the last step)
+    double *q[2], *v[2], *F[2];   // padded global state, ping-pong: step s reads buffer (cur + s) & 1, writes the other
+    int cur;                // buffer that holds the initial q
     const uint32_t *bond;   // bond codes (masked lattices) or null
     LqFireScalars *sc;      // in: initial scalars; out: final scalars
     LqFireConsts fc;
-    double *partials;       // [ncta][4] (+ [ncta][2] for the initial state)
+    double *partials;       // [2][ncta][4] by step parity, then [ncta][2] for the initial state
     int nbx, nby, nbz;      // bricks per direction
     int bx, by, bz;         // brick size (the last brick of a direction may be ragged)
 };
@@ -79,21 +81,64 @@ __global__ void __launch_bounds__(NT, 1) k_fire_resident(const ResArgs a) {
 
     double q5[5], v5[5] = {0, 0, 0, 0, 0}, F5[5];
 #pragma unroll
-    for (int c = 0; c < 5; ++c) q5[c] = active ? a.q[c * NP + p] : 0.0;
+    for (int c = 0; c < 5; ++c) q5[c] = active ? a.q[a.cur][c * NP + p] : 0.0;
 
-    // halo of the brick from the global array (L2; periodic index wrap): the six faces, 5 components
+    // halo of the brick (the six faces; periodic index wrap): cell h -> global index pg and shared-box index si
     const int nf_xy = ex * ey, nf_xz = ex * ez, nf_yz = ey * ez, nhalo = 2 * (nf_xy + nf_xz + nf_yz);
+    auto halo_cell = [&](int h, long long &pg, int &si) {
+        int hx, hy, hz, t = h;
+        if (t < 2 * nf_xy) { const int s = t >= nf_xy; t -= s * nf_xy; hx = t % ex; hy = t / ex; hz = s ? ez : -1; }
+        else if ((t -= 2 * nf_xy) < 2 * nf_xz) { const int s = t >= nf_xz; t -= s * nf_xz; hx = t % ex; hz = t / ex; hy = s ? ey : -1; }
+        else { t -= 2 * nf_xz; const int s = t >= nf_yz; t -= s * nf_yz; hy = t % ey; hz = t / ey; hx = s ? ex : -1; }
+        pg = a.g.pidx(wrapi(x0 + hx, a.g.Lx), wrapi(y0 + hy, a.g.Ly), wrapi(z0 + hz, a.g.Lz));
+        si = ((hz + 1) * SY + (hy + 1)) * SX + hx + 1;
+    };
+    // initial state: q of the halo cells as it stands (object cells keep this value for the whole run)
     auto load_halo = [&]() {
         for (int h = tid; h < nhalo; h += NT) {
-            int gx, gy, gz, hx, hy, hz, t = h;
-            if (t < 2 * nf_xy) { const int s = t >= nf_xy; t -= s * nf_xy; hx = t % ex; hy = t / ex; hz = s ? ez : -1; }
-            else if ((t -= 2 * nf_xy) < 2 * nf_xz) { const int s = t >= nf_xz; t -= s * nf_xz; hx = t % ex; hz = t / ex; hy = s ? ey : -1; }
-            else { t -= 2 * nf_xz; const int s = t >= nf_yz; t -= s * nf_yz; hy = t % ey; hz = t / ey; hx = s ? ex : -1; }
-            gx = wrapi(x0 + hx, a.g.Lx); gy = wrapi(y0 + hy, a.g.Ly); gz = wrapi(z0 + hz, a.g.Lz);
-            const long long pg = a.g.pidx(gx, gy, gz);
-            const int si = ((hz + 1) * SY + (hy + 1)) * SX + hx + 1;
+            long long pg; int si;
+            halo_cell(h, pg, si);
 #pragma unroll
-            for (int c = 0; c < 5; ++c) qs[c * SP + si] = __ldcg(a.q + c * NP + pg);
+            for (int c = 0; c < 5; ++c) qs[c * SP + si] = __ldcg(a.q[a.cur] + c * NP + pg);
+        }
+    };
+    // a step's q' of the halo cells, recomputed from the neighbours' (q, vc, F) in buffer `in` with the very
+    // instruction sequence their owners use (lqsw::drift): no CTA waits for another one's q'.  The thread's first
+    // halo cell (all of them when nhalo <= NT) is fetched into registers right after the grid barrier, so that its
+    // L2 round trip overlaps the reduction of the partials.
+    long long hp0 = -1; int hs0 = 0;                  // first halo cell: global index (-1: none or an object), box index
+    if (tid < nhalo) {
+        halo_cell(tid, hp0, hs0);
+        if (a.bond && (a.bond[hp0] & LQ_BOND_OBJECT)) hp0 = -1;
+    }
+    double hq[5], hv[5], hF[5];
+    auto fetch_halo0 = [&](int in) {
+        if (hp0 < 0) return;
+#pragma unroll
+        for (int c = 0; c < 5; ++c) {
+            hq[c] = __ldcg(a.q[in] + c * NP + hp0); hv[c] = __ldcg(a.v[in] + c * NP + hp0); hF[c] = __ldcg(a.F[in] + c * NP + hp0);
+        }
+    };
+    auto drift_halo = [&](int in, const LqStepCoef &kc) {
+        if (hp0 >= 0) {
+#pragma unroll
+            for (int c = 0; c < 5; ++c) {
+                double vk, qn;
+                drift(hq[c], hv[c], hF[c], kc.ma, kc.cF, kc.dt, vk, qn);
+                qs[c * SP + hs0] = qn;
+            }
+        }
+        for (int h = tid + NT; h < nhalo; h += NT) {
+            long long pg; int si;
+            halo_cell(h, pg, si);
+            if (a.bond && (__ldg(a.bond + pg) & LQ_BOND_OBJECT)) continue;
+#pragma unroll
+            for (int c = 0; c < 5; ++c) {
+                double vk, qn;
+                drift(__ldcg(a.q[in] + c * NP + pg), __ldcg(a.v[in] + c * NP + pg), __ldcg(a.F[in] + c * NP + pg), kc.ma, kc.cF,
+                      kc.dt, vk, qn);
+                qs[c * SP + si] = qn;
+            }
         }
     };
     // force on the own site from the shared box (weighted 7-point stencil + bulk + anchoring), same arithmetic as
@@ -173,14 +218,19 @@ __global__ void __launch_bounds__(NT, 1) k_fire_resident(const ResArgs a) {
 #pragma unroll
     for (int c = 0; c < 5; ++c) F5[c] = 0.0;
     if (sim) force(q5, F5);
+    if (active) {                                     // (vc = 0, F(q_0)) for the neighbours' first drift
+#pragma unroll
+        for (int c = 0; c < 5; ++c) { __stcg(a.v[a.cur] + c * NP + p, 0.0); __stcg(a.F[a.cur] + c * NP + p, F5[c]); }
+    }
     {
         double r0[2] = {0.0, 0.0};
 #pragma unroll
         for (int c = 0; c < 5; ++c) { r0[0] = __fma_rn(F5[c], F5[c], r0[0]); r0[1] = fmax(r0[1], fabs(F5[c])); }
-        publish(r0, 2, 1, a.partials + 4 * ncta + 2 * cta);
+        publish(r0, 2, 1, a.partials + 8 * ncta + 2 * cta);
         grid.sync();
+        fetch_halo0(a.cur);
         double t0[4];
-        gather(a.partials + 4 * ncta, 2, 1, t0);
+        gather(a.partials + 8 * ncta, 2, 1, t0);
         if (tid == 0) {
             LqFireScalars nx = s_sc;
             nx.P = 0.0; nx.FF = t0[0]; nx.vv = 0.0; nx.Fmax = t0[1];
@@ -190,10 +240,12 @@ __global__ void __launch_bounds__(NT, 1) k_fire_resident(const ResArgs a) {
         __syncthreads();
     }
 
-    // ---- the FIRE loop, entirely on the device
+    // ---- the FIRE loop, entirely on the device: one grid barrier per step
+    int in = a.cur;
     while (!s_sc.converged && s_sc.step < a.fc.max_steps) {
         const LqFireScalars sc = s_sc;
         const LqStepCoef kc = lq_step_coef(sc, a.fc);
+        const int out = in ^ 1;
         double vk[5], qn[5], Fn[5] = {0.0, 0.0, 0.0, 0.0, 0.0}, vn[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
 #pragma unroll
         for (int c = 0; c < 5; ++c) {
@@ -203,13 +255,9 @@ __global__ void __launch_bounds__(NT, 1) k_fire_resident(const ResArgs a) {
         __syncthreads();                              // everyone is done reading the box of the previous step
         if (active) {
 #pragma unroll
-            for (int c = 0; c < 5; ++c) {
-                qs[c * SP + sidx] = qn[c];
-                if (sim) __stcg(a.q + c * NP + p, qn[c]);
-            }
+            for (int c = 0; c < 5; ++c) qs[c * SP + sidx] = qn[c];
         }
-        grid.sync();
-        load_halo();
+        drift_halo(in, kc);
         __syncthreads();
         double r[4] = {0.0, 0.0, 0.0, 0.0};
         if (sim) {
@@ -223,10 +271,18 @@ __global__ void __launch_bounds__(NT, 1) k_fire_resident(const ResArgs a) {
                 r[3] = fmax(r[3], fabs(Fn[c]));
             }
         }
-        publish(r, 4, 3, a.partials + 4 * cta);
+        if (active) {                                 // the new state, for the neighbours' next drift and the caller
+#pragma unroll
+            for (int c = 0; c < 5; ++c) {
+                __stcg(a.q[out] + c * NP + p, qn[c]); __stcg(a.v[out] + c * NP + p, vn[c]); __stcg(a.F[out] + c * NP + p, Fn[c]);
+            }
+        }
+        double *part = a.partials + (size_t)out * 4 * ncta;   // by parity: a fast CTA may publish step s+1 while a slow one gathers s
+        publish(r, 4, 3, part + 4 * cta);
         grid.sync();
+        fetch_halo0(out);
         double tot[4];
-        gather(a.partials, 4, 3, tot);
+        gather(part, 4, 3, tot);
         if (tid == 0) {
             LqFireScalars nx = sc;
             lq_fire_advance(nx, a.fc, tot, 0);
@@ -234,14 +290,11 @@ __global__ void __launch_bounds__(NT, 1) k_fire_resident(const ResArgs a) {
         }
 #pragma unroll
         for (int c = 0; c < 5; ++c) { q5[c] = qn[c]; v5[c] = vn[c]; F5[c] = Fn[c]; }
+        in = out;
         __syncthreads();
     }
 
-    // ---- results: velocities (q is already in the global array), scalars
-    if (active) {
-#pragma unroll
-        for (int c = 0; c < 5; ++c) a.v[c * NP + p] = v5[c];
-    }
+    // ---- results: q, vc of the final state sit in buffer (cur + steps) & 1; scalars
     if (cta == 0 && tid == 0) *a.sc = s_sc;
 }
 
@@ -273,11 +326,13 @@ bool lq_resident_plan(const LqGeom &g, int nsm, int dims[6]) {
 
 // One cooperative launch = the whole minimisation.  Returns cudaErrorCooperativeLaunchTooLarge (or another error) if
 // the grid cannot be co-resident; the caller then falls back to the streaming sweeps.
-cudaError_t lq_launch_fire_resident(const LqGeom &g, const LqPhys &ph, const LqFields &f, double *q, double *v,
-                                    const uint32_t *bond, LqFireScalars *sc, const LqFireConsts &fc, double *partials,
-                                    const int dims[6], cudaStream_t st) {
+cudaError_t lq_launch_fire_resident(const LqGeom &g, const LqPhys &ph, const LqFields &f, double *const q[2],
+                                    double *const v[2], double *const F[2], int cur, const uint32_t *bond,
+                                    LqFireScalars *sc, const LqFireConsts &fc, double *partials, const int dims[6],
+                                    cudaStream_t st) {
     ResArgs a;
-    a.g = g; a.ph = ph; a.f = f; a.q = q; a.v = v; a.bond = bond; a.sc = sc; a.fc = fc; a.partials = partials;
+    a.g = g; a.ph = ph; a.f = f; a.bond = bond; a.sc = sc; a.fc = fc; a.partials = partials; a.cur = cur;
+    for (int i = 0; i < 2; ++i) { a.q[i] = q[i]; a.v[i] = v[i]; a.F[i] = F[i]; }
     a.nbx = dims[0]; a.nby = dims[1]; a.nbz = dims[2]; a.bx = dims[3]; a.by = dims[4]; a.bz = dims[5];
     const int vol = a.bx * a.by * a.bz;
     const int nt = vol <= 128 ? 128 : (vol <= 256 ? 256 : 512);

@@ -61,6 +61,9 @@ cudaError_t lq_launch_fixup(bool three, const LqGeom &g, const LqPhys &ph, const
 
 // FIRE with the state resident on chip: one cooperative launch per lq_fire_minimize call (lq_resident.cu)
 bool lq_resident_plan(const LqGeom &g, int nsm, int dims[6]);
-cudaError_t lq_launch_fire_resident(const LqGeom &g, const LqPhys &ph, const LqFields &f, double *q, double *v,
-                                    const uint32_t *bond, LqFireScalars *sc, const LqFireConsts &fc, double *partials,
-                                    const int dims[6], cudaStream_t st);
+// q, v, F: ping-pong state buffers; step s reads buffer (cur + s) & 1 and writes the other, so the final state sits
+// in buffer (cur + steps taken) & 1.  partials: 10 doubles per CTA.
+cudaError_t lq_launch_fire_resident(const LqGeom &g, const LqPhys &ph, const LqFields &f, double *const q[2],
+                                    double *const v[2], double *const F[2], int cur, const uint32_t *bond,
+                                    LqFireScalars *sc, const LqFireConsts &fc, double *partials, const int dims[6],
+                                    cudaStream_t st);

@@ -375,6 +375,20 @@ def main():
                 "algorithmic_bytes_per_site": alg_bytes_site, "design_bytes_per_site": design_bytes_site,
                 "achieved_design_GBs": design_bytes_site * sites_per_launch / (launch_ms * 1e-3) / 1e9,
                 "launch_ms": launch_ms, "launches_timed": rep["sweep_launches"], "sites_per_launch": sites_per_launch}
+    # the secondary roof: fp64 FMA rate of this device, measured now by the library's register-only
+    # microbenchmark (outside the timed region), and the fp64 work the timed kernel did against it
+    if slabs is None:
+        try:
+            alu = lq.lq_get_info(ctx, "fp64_fma_tflops")
+            # ~190 flop per one-constant force + update, ~340 with L2/L3; the recompute sweep
+            # evaluates the one-constant force ~2.2 times per site-update (~340); GD / Nesterov drop FIRE's update
+            flop_site = {"fire": 340.0, "gd": 300.0 if three else 150.0, "nesterov": 310.0 if three else 160.0,
+                         "analyze": 250.0}[args.method]
+            roofline["fp64_fma_peak_tflops"] = alu
+            roofline["fp64_flop_per_site_estimate"] = flop_site
+            roofline["fp64_frac_estimate"] = flop_site * sites_per_launch / (launch_ms * 1e-3) / 1e12 / alu
+        except Exception:
+            pass
     if resident:
         roofline["kernel"] = "k_fire_resident"
         roofline["note"] = ("state resident on chip: the algorithmic bytes never touch HBM, the step is bound by its grid "

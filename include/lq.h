@@ -284,6 +284,8 @@ int lq_get_S0(lq_ctx *ctx, double *S0);
  *   "sweep_bytes_per_site" (get): algorithmic HBM bytes one sweep moves per site
  *   "n_simulated" (get), "n_boundary" (get), "n_object" (get)
  *   "has_fixup" (get): 1 if a FIRE step on this context is a sweep plus a fix-up launch (stored force + objects)
+ *   "fp64_fma_tflops" (get): runs a register-only fp64 FMA microbenchmark on the context's device and stream (a few
+ *                      milliseconds) and returns the measured TFLOP/s: the ALU roof next to the HBM one
  * Unknown key: LQ_ERR_ARG. */
 int lq_set_option(lq_ctx *ctx, const char *key, double value);
 int lq_get_info(lq_ctx *ctx, const char *key, double *value);

@@ -341,6 +341,13 @@ int lq_get_info(lq_ctx *c, const char *key, double *value) {
         *value = ((lq_three(c->ph) || c->fire_path == 2) && c->flags_active) ? 1.0 : 0.0;
         return LQ_OK;
     }
+    if (!strcmp(key, "fp64_fma_tflops")) {       // measured now: the fp64 ALU roof of this device (a few ms of FMAs)
+        DeviceGuard dg(c);
+        const double t = lq_measure_fp64_fma(c->device, c->stream);
+        if (t < 0.0) return fail(c, LQ_ERR_CUDA, "lq_get_info: the fp64 FMA microbenchmark failed");
+        *value = t;
+        return LQ_OK;
+    }
     if (!strcmp(key, "sweep_bytes_per_site")) {
         // fused sweep: read + write q, v (and F when it is stored), 5 fp64 each, + the flag byte where objects exist
         const bool three = lq_three(c->ph);

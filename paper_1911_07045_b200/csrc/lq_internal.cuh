@@ -154,6 +154,7 @@ struct LqFields {
 };
 
 // ---- generic kernels (lq_kernels.cu) ----------------------------------------------------
+double lq_measure_fp64_fma(int device, cudaStream_t st);   // fp64 FMA microbenchmark, TFLOP/s (< 0: error)
 void lq_launch_fill_ghosts_f64(const LqGeom &g, double *field, int ncomp, cudaStream_t st);
 void lq_launch_fill_ghosts_u8(const LqGeom &g, uint8_t *field, cudaStream_t st);
 void lq_launch_classify(const LqGeom &g, const uint8_t *mask_p, uint8_t *flags_p, cudaStream_t st);

@@ -406,6 +406,48 @@ inline dim3 plane_grid(const LqGeom &g) { return dim3((g.Lx + BX - 1) / BX, (g.L
 
 }  // namespace
 
+// fp64 FMA microbenchmark (the secondary roof of SURVEY 8(d)): 16 independent dependent-FMA chains per thread, no
+// memory traffic; returns measured TFLOP/s (2 flop per FMA), < 0 on error.  Behind lq_get_info("fp64_fma_tflops").
+namespace {
+__global__ void __launch_bounds__(512) k_fp64_fma(double *out, int iters, double b, double c) {
+    double a[16];
+#pragma unroll
+    for (int j = 0; j < 16; ++j) a[j] = 1.0 + 1e-3 * (double)(threadIdx.x + j);
+    for (int i = 0; i < iters; ++i) {
+#pragma unroll
+        for (int j = 0; j < 16; ++j) a[j] = __fma_rn(a[j], b, c);
+    }
+    double s = 0.0;
+#pragma unroll
+    for (int j = 0; j < 16; ++j) s += a[j];
+    out[(size_t)blockIdx.x * blockDim.x + threadIdx.x] = s;
+}
+}  // namespace
+double lq_measure_fp64_fma(int device, cudaStream_t st) {
+    int nsm = 148;
+    cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, device);
+    const int nblk = 4 * nsm, nt = 512, iters = 1 << 14;
+    double *out = nullptr;
+    cudaEvent_t e0, e1;
+    if (cudaMalloc(&out, (size_t)nblk * nt * sizeof(double)) != cudaSuccess) return -1.0;
+    cudaEventCreate(&e0); cudaEventCreate(&e1);
+    k_fp64_fma<<<nblk, nt, 0, st>>>(out, 256, 0.999999, 1e-7);          // warm-up
+    float best = 0.f;
+    for (int rep = 0; rep < 3; ++rep) {
+        cudaEventRecord(e0, st);
+        k_fp64_fma<<<nblk, nt, 0, st>>>(out, iters, 0.999999, 1e-7);
+        cudaEventRecord(e1, st);
+        cudaEventSynchronize(e1);
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, e0, e1);
+        if (best == 0.f || ms < best) best = ms;
+    }
+    const cudaError_t err = cudaGetLastError();
+    cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(out);
+    if (err != cudaSuccess || best <= 0.f) return -1.0;
+    return 2.0 * 16.0 * (double)iters * (double)nblk * nt / (best * 1e-3) / 1e12;
+}
+
 void lq_launch_fill_ghosts_f64(const LqGeom &g, double *field, int ncomp, cudaStream_t st) {
     dim3 b(64, 4), gr((g.Lx + 2 * LQ_GH + 63) / 64, (g.Py + 3) / 4, g.Pz);
     k_fill_ghosts<double><<<gr, b, 0, st>>>(g, field, ncomp);

@@ -223,7 +223,12 @@ struct DS {
 template <bool NEST, bool MASKED, bool THREE, int XT, int NS>
 __global__ void __launch_bounds__(((XT & 2) ? 8 : 16) * 32, 1)
 k_descent_sweep(const __grid_constant__ CUtensorMap tq, const __grid_constant__ CUtensorMap tp, const DescArgs a,
-                const uint8_t *__restrict__ plain, int zc) {
+                const uint8_t *__restrict__ plain, const uint32_t *__restrict__ bond, int zc) {
+    // masked lattices: with one elastic constant every simulated site is handled here from its bond code
+    // (lq_internal.cuh LQ_BOND_*: six weights of the boundary-aware 7-point stencil, + object / anchoring
+    // bits; the same codes the FIRE recompute sweep uses); with three constants `plain` marks the sites of the
+    // constant-weight 19-point stencil and the rest goes to k_descent on the non-plain list
+    constexpr bool BOND = MASKED && !THREE;
     using C = DS<NEST, NS, (XT & 2) ? 8 : 16>;
     extern __shared__ __align__(1024) unsigned char smem[];
     __shared__ unsigned s_last;
@@ -263,13 +268,13 @@ k_descent_sweep(const __grid_constant__ CUtensorMap tq, const __grid_constant__ 
 #pragma unroll
     for (int c = 0; c < 5; ++c) ym[c] = yc[c] = 0.0;
     long long p = a.g.pidx(x, y, zb - 1);          // padded index of the plane handled now (k = zb + j - 2)
-    unsigned pb_next = 1u;
+    unsigned pb_next = BOND ? LQ_BOND_PLAIN : 1u;
     int s0 = 0, s1 = NS - 1, s2 = NS - 2;        // ring slots of planes j, j-1, j-2
     uint32_t par = 0;
     for (int j = 0; j < nplanes; ++j) {
         const unsigned pb = pb_next;
-        pb_next = 1u;
-        if (MASKED && active && j >= 1 && j + 1 < nplanes) pb_next = plain[p + a.g.sz];
+        pb_next = BOND ? LQ_BOND_PLAIN : 1u;
+        if (MASKED && active && j >= 1 && j + 1 < nplanes) pb_next = BOND ? bond[p + a.g.sz] : (unsigned)plain[p + a.g.sz];
         mbar_wait(&full[s0], par);
         const double *sj = reinterpret_cast<const double *>(smem + s0 * C::SLOT);
         double yn[5];
@@ -278,7 +283,42 @@ k_descent_sweep(const __grid_constant__ CUtensorMap tq, const __grid_constant__ 
         if (j >= 2 && active) {
             const int k = zb + j - 2;
             const double *sb = reinterpret_cast<const double *>(smem + s1 * C::SLOT);
-            if (!MASKED || pb == 1u) {
+            if (BOND && pb != LQ_BOND_PLAIN) {
+                if (pb & LQ_BOND_OBJECT) store_site(a.g, a.qo, p, x, y, k, yc);     // object site: y == q, never moves
+                else {
+                    const double w0 = lq_bond_weight(pb, 0), w1 = lq_bond_weight(pb, 1), w2 = lq_bond_weight(pb, 2),
+                                 w3 = lq_bond_weight(pb, 3), w4 = lq_bond_weight(pb, 4), w5 = lq_bond_weight(pb, 5);
+                    double lap[5], F[5], o[5];
+#pragma unroll
+                    for (int c = 0; c < 5; ++c) {
+                        const double qx = yc[c];
+                        lap[c] = (w0 * (Y(sb, c, 1) - qx) + w1 * (Y(sb, c, -1) - qx)) +
+                                 (w2 * (Y(sb, c, C::SW) - qx) + w3 * (Y(sb, c, -C::SW) - qx)) +
+                                 (w4 * (yn[c] - qx) + w5 * (ym[c] - qx));
+                    }
+                    force1(a.ph, yc, lap, F);
+                    if (pb & LQ_BOND_ANCH) {          // Eq. 14 / 15 at a boundary site with an anchoring record
+                        const int kind = a.f.kind[p];
+                        if (kind != 0) {
+                            const long long NP = a.g.NP;
+                            const double n[3] = {a.f.axis[p], a.f.axis[NP + p], a.f.axis[2 * NP + p]};
+                            const double Q[6] = {yc[0], yc[1], yc[2], yc[3], yc[4], -yc[0] - yc[3]};
+                            double G[3][3] = {{0.0, 0.0, 0.0}, {0.0, 0.0, 0.0}, {0.0, 0.0, 0.0}}, Fa[5];
+                            lqs::anchoring(a.ph, kind, a.f.W[p], n, Q, G);
+                            lqs::G_to_F(G, Fa);
+#pragma unroll
+                            for (int c = 0; c < 5; ++c) F[c] += Fa[c];
+                        }
+                    }
+#pragma unroll
+                    for (int c = 0; c < 5; ++c) {
+                        o[c] = __fma_rn(eta, F[c], yc[c]);
+                        r[0] = __fma_rn(F[c], F[c], r[0]);
+                        r[1] = fmax(r[1], fabs(F[c]));
+                    }
+                    store_site(a.g, a.qo, p, x, y, k, o);
+                }
+            } else if (!MASKED || BOND || pb == 1u) {
                 double F[5], o[5];
                 if (!THREE) {
                     double lap[5];
@@ -331,7 +371,9 @@ struct LqDescentPlan {
     CUtensorMap map[3];
     double *mapped[3] = {nullptr, nullptr, nullptr};
     int map_ty = 0;                   // tile rows the maps' boxes were made for
-    uint8_t *plain = nullptr;         // per-site plain byte (masked lattices)
+    uint8_t *plain = nullptr;         // per-site plain byte (masked lattices, three constants)
+    uint32_t *bond = nullptr;         // per-site bond code (masked lattices, one constant)
+    bool bond_built = false, list_built = false;
     int *list = nullptr;              // index-ordered non-plain simulated sites
     int n_list = 0;
     const uint8_t *flags_seen = nullptr;
@@ -345,6 +387,7 @@ void lq_descent_destroy(LqDescentPlan *p) {
     cudaFree(p->sweep_partials);
     cudaFree(p->counter);
     cudaFree(p->plain);
+    cudaFree(p->bond);
     cudaFree(p->list);
     delete p;
 }
@@ -367,7 +410,7 @@ cudaError_t launch_sweep_t(LqDescentPlan *pl, dim3 grid, const CUtensorMap &mq, 
         if (e != cudaSuccess) return e;
         pl->attr_set[v] = true;
     }
-    k_descent_sweep<NEST, MASKED, THREE, XT, NS><<<grid, C::NT, C::SMEM_BYTES, st>>>(mq, mp, a, pl->plain, zc);
+    k_descent_sweep<NEST, MASKED, THREE, XT, NS><<<grid, C::NT, C::SMEM_BYTES, st>>>(mq, mp, a, pl->plain, pl->bond, zc);
     return cudaGetLastError();
 }
 template <bool NEST, bool MASKED>
@@ -425,17 +468,26 @@ int lq_descent_run(LqDescentPlan **planp, int method, int path, const LqGeom &g,
             if (cudaMalloc(&pl->sweep_partials, 2 * ncta * sizeof(double)) != cudaSuccess) { err = "lq_descent: cudaMalloc failed"; return LQ_ERR_NOMEM; }
             pl->sweep_cap = 2 * ncta;
         }
-        if (masked && (pl->sites_dirty || pl->flags_seen != f.flags || !pl->plain)) {
+        if (masked && (pl->sites_dirty || pl->flags_seen != f.flags)) { pl->bond_built = pl->list_built = false; }
+        if (masked && !three && !pl->bond_built) {
+            // one constant: bond codes, every simulated site in the sweep (no second kernel)
+            if (!pl->bond && cudaMalloc(&pl->bond, (size_t)g.NP * sizeof(uint32_t)) != cudaSuccess) { err = "lq_descent: cudaMalloc failed"; return LQ_ERR_NOMEM; }
+            DESC_CUDA(cudaMemsetAsync(pl->bond, 0, (size_t)g.NP * sizeof(uint32_t), st));
+            lq_launch_bond_map(g, f.flags, f.kind, pl->bond, st);
+            *launches += 1;
+            pl->bond_built = true;
+        }
+        if (masked && three && !pl->list_built) {
             if (!pl->plain && cudaMalloc(&pl->plain, (size_t)g.NP) != cudaSuccess) { err = "lq_descent: cudaMalloc failed"; return LQ_ERR_NOMEM; }
             DESC_CUDA(cudaMemsetAsync(pl->plain, 0, (size_t)g.NP, st));
             lq_launch_plain_map(g, f.flags, pl->plain, st);
             *launches += 1;
             if (lq_fixup_build_list(g, f.flags, pl->plain, &pl->list, &pl->n_list, st) != 0) { err = "lq_descent: building the non-plain site list failed"; return LQ_ERR_NOMEM; }
-            pl->sites_dirty = false;
-            pl->flags_seen = f.flags;
+            pl->list_built = true;
         }
+        if (masked) { pl->sites_dirty = false; pl->flags_seen = f.flags; }
     }
-    const long long nsites = fast ? (masked ? pl->n_list : 0) : g.N;
+    const long long nsites = fast ? ((masked && three) ? pl->n_list : 0) : g.N;
     const unsigned nblk = (unsigned)((nsites + DB - 1) / DB);
     if (pl->cap < (size_t)2 * nblk) {
         cudaFree(pl->partials); pl->partials = nullptr; pl->cap = 0;

@@ -344,3 +344,14 @@ def test_resident_kernel_matches_streaming_sweeps_and_oracle(lq, oracle_mod, nam
         out[resident] = q
     assert np.abs(out[0] - out[1]).max() <= 1e-11
     lq.lq_destroy(ctx)
+
+
+def test_fp64_fma_microbenchmark_reports_a_plausible_roof(lq):
+    """lq_get_info("fp64_fma_tflops") runs the register-only FMA microbenchmark (SURVEY 8(d)'s secondary roof):
+    a B200 has 148 SMs x 64 fp64 FMA per clock, 37 TFLOP/s at 1.965 GHz; anything between a third of that and
+    a little above it is a believable measurement, anything else a broken timer or kernel."""
+    c = wl.make_replica("4")
+    ctx = lq.create_from_config(c)
+    t = lq.lq_get_info(ctx, "fp64_fma_tflops")
+    assert 12.0 < t < 42.0, t
+    lq.lq_destroy(ctx)

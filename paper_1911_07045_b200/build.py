@@ -48,7 +48,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
         if p.wait() != 0:
             raise RuntimeError("nvcc failed")
     tmp = LIB + ".tmp%d" % os.getpid()
-    subprocess.run([nvcc, "-shared", "-cudart", "static", "-o", tmp] + objs, check=True)
+    subprocess.run([nvcc, "-shared", "-cudart", "static", "-Wno-deprecated-gpu-targets", "-o", tmp] + objs, check=True)
     os.replace(tmp, LIB)
     return LIB
 

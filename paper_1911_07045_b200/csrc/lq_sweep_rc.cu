@@ -49,7 +49,6 @@ struct RC {
     static constexpr int MAXZC = 126;                              // ts[] holds ze - zb + 2 <= 128 entries
     static constexpr int OFF_CODE = OFF_TS + 128;                  // bond codes: 4 slots x (NT own + 128 halo) x u32
     static constexpr int SMEM_BYTES = OFF_CODE + 4 * (NT + 128) * 4;
-    static constexpr int NHALO = 2 * BXW + 2 * (BYH - 2);
 };
 static_assert(RC::SMEM_BYTES <= 232448, "shared memory budget");
 

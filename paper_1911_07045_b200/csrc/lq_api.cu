@@ -91,6 +91,7 @@ int lq_create(int Lx, int Ly, int Lz, double A, double B, double C, double L1, d
     g.Py = Ly + 2 * LQ_GH; g.Pz = Lz + 2 * LQ_GH;
     g.sy = g.Px; g.sz = (long long)g.Px * g.Py;
     g.NP = g.sz * g.Pz; g.N = (long long)Lx * Ly * Lz;
+    g.gwx = (Lx % 4 == 0 && Lx >= 8 && g.Px - LQ_XO - Lx >= 4) ? 4 : LQ_GH;
     if (g.NP > 2147483647LL) { delete c; return fail(nullptr, LQ_ERR_ARG, "lq_create: lattice too large (padded sites > 2^31-1)"); }
     c->ph = LqPhys{A, B, C, L1, L2, L3, (-B + sqrt(B * B - 24.0 * A * C)) / (6.0 * C)};
     int rc = LQ_OK;

@@ -71,7 +71,7 @@ __device__ __forceinline__ void store_site(const LqGeom &g, double *qo, long lon
     const long long NP = g.NP;
 #pragma unroll
     for (int c = 0; c < 5; ++c) qo[c * NP + p] = o[c];
-    const int shx = ghost_shift(x, g.Lx, LQ_GH), shy = ghost_shift(y, g.Ly, LQ_GH), shz = ghost_shift(z, g.Lz, LQ_GH);
+    const int shx = ghost_shift(x, g.Lx, g.gwx), shy = ghost_shift(y, g.Ly, LQ_GH), shz = ghost_shift(z, g.Lz, LQ_GH);
     if (shx | shy | shz) {
         for (int m = 1; m < 8; ++m) {
             if (((m & 1) && !shx) || ((m & 2) && !shy) || ((m & 4) && !shz)) continue;

@@ -71,7 +71,7 @@ __global__ void __launch_bounds__(FB, LQ_FIX_MINB) k_fixup(const FixArgs a) {
         }
         const int x = (int)(p % a.g.Px) - LQ_XO, y = (int)((p / a.g.Px) % a.g.Py) - LQ_GH,
                   z = (int)(p / a.g.sz) - LQ_GH;
-        const int shx = ghost_shift(x, a.g.Lx, LQ_GH), shy = ghost_shift(y, a.g.Ly, LQ_GH),
+        const int shx = ghost_shift(x, a.g.Lx, a.g.gwx), shy = ghost_shift(y, a.g.Ly, LQ_GH),
                   shz = ghost_shift_z(z, a.g);
         if (shx | shy | shz) {
             for (int m = 1; m < 8; ++m) {

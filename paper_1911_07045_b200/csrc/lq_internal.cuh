@@ -31,6 +31,9 @@ struct LqGeom {
     long long sy, sz;  // strides (elements) of +y and +z in the padded box
     long long NP;      // padded sites per component
     long long N;       // Lx*Ly*Lz
+    int gwx;           // width of the x ghost images the sweeps write: LQ_GH, or 4 where Lx % 4 == 0 and the row padding
+                       // has room -- the images of x = 0..3 / Lx-4..Lx-1 then fill whole 32-byte sectors (a 16-byte
+                       // store into a sector costs the ECC'd HBM a read-modify-write); cells beyond LQ_GH are never read
     int zopen;         // 1: z-slab sub-domain: the z ghost planes hold the neighbour slabs' planes
                        // (halo exchange), nothing wraps in z and no kernel writes z ghost images
     __host__ __device__ inline long long pidx(int x, int y, int z) const {

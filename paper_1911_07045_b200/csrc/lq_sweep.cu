@@ -207,7 +207,7 @@ k_sweep(const __grid_constant__ CUtensorMap tq, const __grid_constant__ CUtensor
             }
             // periodic ghost shell of the outputs, full width LQ_GH: whatever runs next on this state (the
             // recompute sweep reads q with a 2-site halo) finds every ghost current
-            const int shx = ghost_shift(x, a.g.Lx, LQ_GH), shy = ghost_shift(y, a.g.Ly, LQ_GH),
+            const int shx = ghost_shift(x, a.g.Lx, a.g.gwx), shy = ghost_shift(y, a.g.Ly, LQ_GH),
                       shz = ghost_shift_z(k, a.g);
             if (shx | shy | shz) {
                 for (int m = 1; m < 8; ++m) {

@@ -290,7 +290,7 @@ k_sweep_rc(const __grid_constant__ CUtensorMap tq, const __grid_constant__ CUten
                 a.vo[c * NP + p] = vn[c];
             }
             // periodic ghost shell of the outputs (width LQ_GH: the next sweep reads q with a 2-site halo)
-            const int shx = ghost_shift(x, a.g.Lx, LQ_GH), shy = ghost_shift(y, a.g.Ly, LQ_GH),
+            const int shx = ghost_shift(x, a.g.Lx, a.g.gwx), shy = ghost_shift(y, a.g.Ly, LQ_GH),
                       shz = ghost_shift_z(k, a.g);
             if (shx | shy | shz) {
                 for (int m = 1; m < 8; ++m) {

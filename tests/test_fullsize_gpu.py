@@ -194,3 +194,26 @@ def test_replica_converged_energy(lq, oracle_mod, name):
     assert abs(rep["energy"] - rref["energy"]) <= TOL_ECONV * abs(rref["energy"])
     assert rep["energy"] < e0
     lq.lq_destroy(ctx)
+
+
+@pytest.mark.parametrize("name", ["5", "3"])
+def test_full_size_descent(lq, oracle_mod, name):
+    """Gradient descent and Nesterov at full size, in the launch configuration bench.py --method times:
+    20 steps of each against the oracle's lqo_descent, every site.  Config 5 runs the one-constant sweep with bond
+    codes (every simulated site in the one kernel), config 3 the 19-point sweep + the list kernel."""
+    c = wl.make_config(name)
+    ctx = lq.create_from_config(c)
+    o = make_oracle(oracle_mod, c)
+    K, eta, mu = 20, 0.004, 0.8
+    for method in (0, 1):
+        lq.lq_set_Q(ctx, np.ascontiguousarray(c["q"]))
+        rep = lq.lq_descent_minimize(ctx, method, K, 0.0, eta, mu)
+        qref, rref = o.descent(c["q"], method, K, 0.0, eta, mu)
+        q = lq.lq_get_Q(ctx)
+        assert rep["steps"] == K
+        assert np.abs(q - qref).max() <= TOL_Q
+        assert abs(rep["Fmax"] - rref["Fmax"]) <= 1e-9 * rref["Fmax"]
+        obj = c["mask"] == 1
+        assert np.array_equal(q[:, obj], c["q"][:, obj])
+        del q, qref
+    lq.lq_destroy(ctx)

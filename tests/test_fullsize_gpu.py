@@ -217,3 +217,37 @@ def test_full_size_descent(lq, oracle_mod, name):
         assert np.array_equal(q[:, obj], c["q"][:, obj])
         del q, qref
     lq.lq_destroy(ctx)
+
+
+def test_full_size_analysis_sampled(lq, oracle_mod):
+    """lq_analyze at 512^3 in the configuration bench.py --method analyze times, after 60 FIRE steps of
+    the quench (melted cores exist): S, director and defect flag on 400 000 sampled sites against numpy.linalg.eigh
+    (the oracle computes them one by one), and the device-side defect count against the returned mask."""
+    c = wl.make_config("4")
+    ctx = lq.create_from_config(c)
+    lq.lq_fire_minimize(ctx, 60, 0.0, c["fire"])
+    q = lq.lq_get_Q(ctx)
+    rng = np.random.default_rng(20)
+    idx = np.sort(rng.choice(c["N"], size=400_000, replace=False))
+    # the caller's threshold: the median order of the sample, so that both outcomes of the defect rule occur
+    thr = float(np.median(oracle_mod.analyze(np.ascontiguousarray(q[:, idx]), None, 0.0)[0]))
+    r = lq.lq_analyze(ctx, thr)
+    lq.lq_destroy(ctx)
+    S, n, d = oracle_mod.analyze(np.ascontiguousarray(q[:, idx]), None, thr)
+    assert np.abs(r["S"][idx] - S).max() <= 1e-12
+    g = r["director"][:, idx]
+    assert np.abs(np.linalg.norm(g, axis=0) - 1.0).max() <= 1e-12
+    Q = np.empty((idx.size, 3, 3))
+    qs = q[:, idx]
+    Q[:, 0, 0], Q[:, 0, 1], Q[:, 0, 2] = qs[0], qs[1], qs[2]
+    Q[:, 1, 0], Q[:, 1, 1], Q[:, 1, 2] = qs[1], qs[3], qs[4]
+    Q[:, 2, 0], Q[:, 2, 1], Q[:, 2, 2] = qs[2], qs[4], -qs[0] - qs[3]
+    assert np.abs(np.einsum("nij,jn->in", Q, g) - S * g).max() <= 1e-10          # eigen-equation residual
+    w = np.linalg.eigvalsh(Q)
+    well = (w[:, 2] - w[:, 1]) > 1e-6
+    assert well.sum() > 0.9 * idx.size
+    assert np.abs(np.abs((g * n).sum(0))[well] - 1.0).max() <= 1e-9
+    clear = np.abs(S - thr) > 1e-12
+    assert np.array_equal(r["defect"][idx][clear], d[clear])
+    assert r["n_defect"] == int(r["defect"].sum())
+    assert 0.4 * c["N"] < r["n_defect"] < 0.6 * c["N"]

@@ -9,7 +9,9 @@ the full 100 steps against the oracle in the SAME launch configuration as the 51
 waves of CTAs).  north_star's converged-energy gate (rel 1e-6): config 2 at full size against the oracle and the
 closed form 980000 f0; configs 3, 5, 5' on their declared replicas (the full-size runs need 5000 /
 30000 steps of a 16M-site oracle).  The oracle leg of the config-2 convergence run (7.3 min) is opt-in:
-LQ_FULL_PARITY=1; its passing log is kept in profiles/r02_parity_fullsize.txt.
+LQ_FULL_PARITY=1; its passing log is kept in profiles/r02_parity_fullsize.txt.  Also at full size: gradient descent and
+Nesterov on configs 5 and 3, the analysis kernel at 512^3 on sampled sites, and config 3's lattice with every energy
+term switched on (chiral, cubic, both fields).
 """
 import os
 
@@ -251,3 +253,29 @@ def test_full_size_analysis_sampled(lq, oracle_mod):
     assert np.array_equal(r["defect"][idx][clear], d[clear])
     assert r["n_defect"] == int(r["defect"].sum())
     assert 0.4 * c["N"] < r["n_defect"] < 0.6 * c["N"]
+
+
+def test_full_size_every_term_on(lq, oracle_mod):
+    """Config 3's lattice (256^3, walls + colloid, L1 L2 L3) with the chiral (L4) and cubic (L6) distortion terms of
+    Eq. 10 and both external fields of Eq. 13 switched on: 10 FIRE steps and 5 steps each of GD and Nesterov against the
+    oracle, every site.  This is the size at which the cubic-term sweeps (32 x 8 tiles of 256 threads) run many CTAs
+    over several z-chunks."""
+    c = wl.make_config("3")
+    Hf, chi, Ef, eps, L4, L6 = (0.3, -0.5, 0.8), 0.7, (0.6, 0.2, -0.4), -0.9, 0.35, -0.4
+    o = oracle_mod.Oracle(c["Lx"], c["Ly"], c["Lz"], c["A"], c["B"], c["C"], c["L1"], c["L2"], c["L3"], mask=c["mask"],
+                          kind=c["kind"], W=c["W"], axis=c["axis"], H=Hf, chi=chi, E=Ef, eps=eps, L4=L4, L6=L6)
+    ctx = lq.create_from_config(c)
+    lq.lq_set_field(ctx, Hf, chi, Ef, eps)
+    lq.lq_set_chiral(ctx, L4)
+    lq.lq_set_cubic(ctx, L6)
+    lq.lq_fire_minimize(ctx, 10, 0.0, c["fire"])
+    qref, _ = o.fire(c["q"], 10, 0.0, c["fire"], variant=1)
+    assert np.abs(lq.lq_get_Q(ctx) - qref).max() <= TOL_Q
+    del qref
+    for method in (0, 1):
+        lq.lq_set_Q(ctx, np.ascontiguousarray(c["q"]))
+        lq.lq_descent_minimize(ctx, method, 5, 0.0, 0.003, 0.8)
+        qd, _ = o.descent(c["q"], method, 5, 0.0, 0.003, 0.8)
+        assert np.abs(lq.lq_get_Q(ctx) - qd).max() <= TOL_Q
+        del qd
+    lq.lq_destroy(ctx)

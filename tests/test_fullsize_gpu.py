@@ -201,12 +201,16 @@ def test_replica_converged_energy(lq, oracle_mod, name):
 @pytest.mark.parametrize("name", ["5", "3"])
 def test_full_size_descent(lq, oracle_mod, name):
     """Gradient descent and Nesterov at full size, in the launch configuration bench.py --method times:
-    20 steps of each against the oracle's lqo_descent, every site.  Config 5 runs the one-constant sweep with bond
-    codes (every simulated site in the one kernel), config 3 the 19-point sweep + the list kernel."""
+    10 steps of each (20 with LQ_FULL_PARITY=1) against the oracle's lqo_descent, every site.  Config 5 runs the
+    one-constant sweep with bond codes (every simulated site in the one kernel), config 3 the 19-point sweep + the list
+    kernel (opt-in, LQ_FULL_PARITY=1: 72 s of oracle; test_full_size_every_term_on runs the same kernels on the same
+    lattice by default)."""
+    if name == "3" and not FULL:
+        pytest.skip("config 3 leg is opt-in (LQ_FULL_PARITY=1); passing log: profiles/r02_parity_fullsize.txt")
     c = wl.make_config(name)
     ctx = lq.create_from_config(c)
     o = make_oracle(oracle_mod, c)
-    K, eta, mu = 20, 0.004, 0.8
+    K, eta, mu = (20 if FULL else 10), 0.004, 0.8
     for method in (0, 1):
         lq.lq_set_Q(ctx, np.ascontiguousarray(c["q"]))
         rep = lq.lq_descent_minimize(ctx, method, K, 0.0, eta, mu)

@@ -103,6 +103,29 @@ int lq_get_velocity(lq_ctx *ctx, double *v, int where);
 int lq_energy(lq_ctx *ctx, double *E);
 int lq_energy_terms(lq_ctx *ctx, double *terms);
 
+/* lq_energy_terms for callers that must not allocate device memory.  lq_energy_terms keeps its per-block partial
+ * sums in a buffer it cudaMalloc's on first use (and again when a larger lattice needs more).  That is a problem for a
+ * host that has handed the whole GPU to a memory pool of its own (a framework's caching allocator, a service with a
+ * fixed memory budget: a driver allocation may fail there or is simply forbidden), and for a latency-critical loop that
+ * cannot take the device-wide synchronisation and the driver lock that cudaMalloc / cudaFree imply while other streams
+ * are busy.  This entry point computes the same three numbers (bulk, distortion, anchoring; bit-identical to
+ * lq_energy_terms: same kernels, same summation order) and calls no cudaMalloc, cudaFree or allocating library routine:
+ * the partial sums live in a static array inside liblq.so, 1.5 MiB of every GPU that loads the library, held until the
+ * process exits.
+ *   - Input: the context's current Q and geometry.  Output: terms[3], caller-owned; where = LQ_DEVICE writes the three
+ *     doubles on the context's stream and returns without synchronising; LQ_HOST copies them to the host and
+ *     synchronises the stream before returning.
+ *   - Limit: lattices of at most 65536 reduction blocks, ceil(Lx/64) * ceil(Ly/4) * ceil(Lz/8) (512^3 is exactly at the
+ *     limit).  Larger: LQ_ERR_ARG, and lq_last_error names both numbers; nothing is launched.
+ *   - The first call on each device looks up the array's device address (one runtime query, no allocation); make that
+ *     first call before any stream capture begins.
+ *   - All contexts, streams and threads share the one array per GPU.  It keeps the previous call's contents; nothing in
+ *     it needs clearing, because each call overwrites every slot it later reads.  Two calls whose kernels can overlap on
+ *     the GPU (different streams, or different contexts on different streams) race on it and return garbage: order them
+ *     on one stream or with events.  lq_energy_terms, with its per-context buffer, has no such restriction.
+ * Errors: LQ_ERR_ARG (NULL terms, bad where, lattice over the limit), LQ_ERR_STATE before lq_set_Q, LQ_ERR_CUDA. */
+int lq_energy_terms_noalloc(lq_ctx *ctx, double *terms, int where);
+
 /* Force F_a(x) = -dF/dq_a(x) in the five stored variables, [5][N], exactly 0 at
  * object sites. */
 int lq_forces(lq_ctx *ctx, double *F, int where);

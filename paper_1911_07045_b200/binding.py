@@ -23,7 +23,7 @@ _lib = None
 
 # every symbol include/lq.h declares (checked by tests/test_abi.py against the header)
 SYMBOLS = ["lq_create", "lq_destroy", "lq_set_stream", "lq_set_sites", "lq_get_flags", "lq_set_Q", "lq_get_Q",
-           "lq_get_velocity", "lq_set_field", "lq_set_chiral", "lq_set_cubic", "lq_analyze", "lq_energy", "lq_energy_terms", "lq_forces", "lq_fire_minimize", "lq_descent_minimize", "lq_get_S0",
+           "lq_get_velocity", "lq_set_field", "lq_set_chiral", "lq_set_cubic", "lq_analyze", "lq_energy", "lq_energy_terms", "lq_energy_terms_noalloc", "lq_forces", "lq_fire_minimize", "lq_descent_minimize", "lq_get_S0",
            "lq_set_option", "lq_get_info", "lq_last_error", "lq_version",
            "lq_create_slab", "lq_set_sites_ext", "lq_halo_bytes", "lq_halo_export", "lq_halo_import", "lq_slabs_exchange",
            "lq_slabs_fire_minimize", "lq_fire_begin", "lq_fire_step_local", "lq_fire_step_finish", "lq_fire_step_commit", "lq_fire_peek",
@@ -81,6 +81,7 @@ def load():
     L.lq_get_velocity.argtypes = [vp, vp, ip]
     L.lq_energy.argtypes = [vp, dp]
     L.lq_energy_terms.argtypes = [vp, dp]
+    L.lq_energy_terms_noalloc.argtypes = [vp, vp, ip]
     L.lq_forces.argtypes = [vp, vp, ip]
     L.lq_fire_minimize.argtypes = [vp, C.c_long, C.c_double, C.POINTER(lq_fire_params), C.POINTER(lq_fire_report)]
     L.lq_analyze.argtypes = [vp, C.c_double, vp, vp, vp, C.POINTER(C.c_long), ip]
@@ -232,6 +233,18 @@ def lq_energy_terms(ctx):
     t = (C.c_double * 3)()
     _check(ctx.handle, load().lq_energy_terms(ctx.handle, t))
     return np.array(t[:])
+
+
+def lq_energy_terms_noalloc(ctx, out=None):
+    """lq_energy_terms without any device allocation (static scratch inside the library; see include/lq.h for who
+    needs that, the 65536-block size limit and the sharing rules).  ``out``: a 3-element fp64 numpy array (filled
+    when the call returns) or CUDA torch tensor (filled in stream order, no synchronisation); None = a new numpy
+    array.  Returns ``out``."""
+    if out is None:
+        out = np.empty(3, dtype=np.float64)
+    ptr, where = _buf(out, np.float64, 3)
+    _check(ctx.handle, load().lq_energy_terms_noalloc(ctx.handle, ptr, where))
+    return out
 
 
 def lq_get_S0(ctx) -> float:

@@ -2,8 +2,11 @@
 // energy, and the unfused FIRE path (fire_path = 1).  One thread per lattice site, global
 // loads through L1/L2.  These serve lq_set_sites / lq_forces / lq_energy and are the
 // cross-check for the fused sweep (lq_sweep.cu), which is the product's hot path.
+#include "lq_ctx.cuh"
 #include "lq_internal.cuh"
 #include "lq_site.cuh"
+
+#include <mutex>
 
 namespace {
 
@@ -543,4 +546,65 @@ void lq_launch_bond_map(const LqGeom &g, const uint8_t *flags, const uint8_t *ki
 void lq_launch_tile_summary_bond(const LqGeom &g, const uint32_t *bond, uint8_t *tsum, int TX, int TY, int ntx, int nty,
                                  cudaStream_t st) {
     k_tile_summary<uint32_t><<<dim3(ntx, nty, g.Lz + 2), 128, 0, st>>>(g, bond, LQ_BOND_PLAIN, tsum, TX, TY);
+}
+
+// ---- lq_energy_terms_noalloc (include/lq.h): the energy pass of lq_energy_terms with its per-block partial sums in a
+// static device array instead of a cudaMalloc'ed buffer.  Same two kernels, same launch shape, same summation order,
+// so the three numbers are bit-identical to lq_energy_terms'.
+namespace {
+
+constexpr int LQ_NOALLOC_MAX_BLOCKS = 65536;   // k_energy blocks (64 x 4 x 8 sites each): 512^3 needs exactly this many
+
+// 3 partial sums per block, then 3 doubles that stage the result for a host caller: 1.5 MiB of every GPU that loads
+// liblq.so, held until the process exits.  Shared by all contexts and all calls.
+static __device__ __align__(256) double g_noalloc_scratch[3 * LQ_NOALLOC_MAX_BLOCKS + 3];
+
+constexpr int LQ_NOALLOC_MAX_DEVICES = 64;
+double *g_noalloc_ptr[LQ_NOALLOC_MAX_DEVICES];  // device address of g_noalloc_scratch, by device ordinal (0 = not asked yet)
+std::mutex g_noalloc_mu;
+
+// In host code `g_noalloc_scratch` is only a handle for the runtime, not an address a kernel may dereference, and each
+// device has its own copy of the array: ask the runtime for the address on the device that is current (the caller's
+// DeviceGuard made that the context's device), once per device, and hand that pointer to the kernels.
+cudaError_t noalloc_scratch(int device, double **out) {
+    if (device < 0 || device >= LQ_NOALLOC_MAX_DEVICES) return cudaErrorInvalidDevice;
+    std::lock_guard<std::mutex> lock(g_noalloc_mu);
+    if (!g_noalloc_ptr[device]) {
+        void *addr = nullptr;
+        const cudaError_t e = cudaGetSymbolAddress(&addr, g_noalloc_scratch);
+        if (e != cudaSuccess) return e;
+        g_noalloc_ptr[device] = static_cast<double *>(addr);
+    }
+    *out = g_noalloc_ptr[device];
+    return cudaSuccess;
+}
+
+}  // namespace
+
+extern "C" int lq_energy_terms_noalloc(lq_ctx *c, double *terms, int where) {
+    if (!c) return LQ_ERR_ARG;
+    DeviceGuard dg(c);
+    if (!terms || bad_where(where)) return fail(c, LQ_ERR_ARG, "lq_energy_terms_noalloc: bad argument");
+    const long long nblk = lq_energy_num_blocks(c->g);
+    if (nblk > LQ_NOALLOC_MAX_BLOCKS)
+        return fail(c, LQ_ERR_ARG, "lq_energy_terms_noalloc: this lattice needs " + std::to_string(nblk) +
+                                       " reduction blocks (ceil(Lx/64) * ceil(Ly/4) * ceil(Lz/8)) but the static scratch "
+                                       "array holds " + std::to_string(LQ_NOALLOC_MAX_BLOCKS) +
+                                       "; use lq_energy_terms, which allocates");
+    if (!c->has_Q) return fail(c, LQ_ERR_STATE, "lq_energy_terms_noalloc: no Q has been set");
+    double *scratch = nullptr;
+    LQ_CUDA(c, noalloc_scratch(c->device, &scratch));
+    // nothing has to be cleared between calls: every block overwrites its own three slots and the final sum reads
+    // exactly the nblk slots this launch wrote
+    double *out3 = where == LQ_DEVICE ? terms : scratch + 3 * LQ_NOALLOC_MAX_BLOCKS;
+    const LqFields f = fields_of(c);
+    if (lq_three(c->ph)) k_energy<true><<<site_grid(c->g), dim3(BX, BY), 0, c->stream>>>(c->g, c->ph, f, c->q[c->cur], scratch);
+    else k_energy<false><<<site_grid(c->g), dim3(BX, BY), 0, c->stream>>>(c->g, c->ph, f, c->q[c->cur], scratch);
+    k_final_sum<3><<<1, 256, 0, c->stream>>>(scratch, nblk, out3);
+    LQ_CUDA(c, cudaGetLastError());
+    if (where == LQ_HOST) {
+        LQ_CUDA(c, cudaMemcpyAsync(terms, out3, 3 * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+        LQ_CUDA(c, cudaStreamSynchronize(c->stream));
+    }
+    return LQ_OK;
 }

@@ -189,7 +189,7 @@ int lq_set_chiral(lq_ctx *ctx, double L4);
  * limit L6 = (4 / 27 S^3)(K3 - K1): it separates bend from splay).  Discretised like L1..L3: same-axis
  * products average to the mean of the squared one-sided differences, different-axis products to products of the
  * mean differences; the weight Q_lk is the site's own tensor.  Routed like lq_set_chiral (19-point sweeps with the
- * term compiled in; those instantiations spill registers, so expect about a third of the L6 = 0 rate).  Errors as
+ * term compiled in, on 32 x 8 tiles so that they fit the register budget without spilling).  Errors as
  * lq_set_chiral. */
 int lq_set_cubic(lq_ctx *ctx, double L6);
 
@@ -226,10 +226,12 @@ int lq_descent_minimize(lq_ctx *ctx, int method, long max_steps, double force_to
 int lq_analyze(lq_ctx *ctx, double S_threshold, double *S, double *director, uint8_t *defect, long *n_defect,
                int where);
 
-/* ---- Domain decomposition into z-slabs.  "The simulation domain is divided into rectilinear
- * sub-domains, each handled by one rank; after every minimisation step the sites on the faces between sub-domains are
- * communicated, and the scalar quantities the minimiser needs are reduced over all ranks" (the
- * weak-scaling workload of Fig. 4).  Here: slabs along z.
+/* ---- Domain decomposition into z-slabs.  The paper uses "a standard spatial decomposition of the total
+ * number of lattice sites into rectilinear sub-regions"; "each processing unit is assigned to one of these subregions"
+ * and also keeps the state of the halo sites, which are communicated every simulation step (sec.
+ * III.B; the weak-scaling workload of Fig. 4).  The paper does not spell out the reduction of the
+ * minimiser's scalars over the units; FIRE needs one (P, |F|^2, |v|^2, max|F| are global), so it is part of the
+ * protocol here.  Here: slabs along z.
  *
  * lq_create_slab makes a sub-domain context for the planes [z0, z0 + nz) of a global Lx x Ly x Lz lattice (nz >= 4).
  * It behaves like any context on LOCAL arrays of nz planes (lq_set_Q, lq_get_Q, lq_get_flags, lq_forces, lq_energy,
@@ -281,7 +283,15 @@ int lq_slabs_fire_minimize(lq_ctx **slabs, int n, long max_steps, double force_t
  *             every so often lq_fire_peek(ctx, report) (synchronises) to test `converged`
  *     lq_fire_end(ctx, report)                   fixes the live buffer; Frms uses the slab's own site count
  * The number of sweeps to enqueue is max(max_steps, 1), or max_steps + 1 on the stored-force path or with
- * integrator = 1.  Either every slab of a lattice gets geometry (lq_set_sites_ext) or none does. */
+ * integrator = 1; lq_get_info(ctx, "fire_sweeps_total") returns it after lq_fire_begin.  Either every slab of a lattice
+ * gets geometry (lq_set_sites_ext) or none does.
+ * Stream order.  With where = LQ_DEVICE, lq_halo_export, lq_halo_import, lq_fire_step_finish and lq_fire_step_commit
+ * only ENQUEUE work on the context's stream (lq_set_stream) and return: the caller's device buffer is written / read
+ * when the stream gets there, not when the call returns.  Anything that touches such a buffer on another stream (a
+ * communication library, the caller's own kernels) must be ordered against the context's stream with events or by
+ * running on that stream, and the buffer must stay allocated until the enqueued work has run.  With where = LQ_HOST the
+ * same calls synchronise the context's stream before returning, so the host buffer is complete (or free to reuse) on
+ * return.  lq_fire_step_local and lq_fire_begin always only enqueue; lq_fire_peek and lq_fire_end synchronise. */
 int lq_fire_begin(lq_ctx *ctx, long max_steps, double force_tol, const lq_fire_params *params);
 int lq_fire_step_local(lq_ctx *ctx);
 int lq_fire_step_finish(lq_ctx *ctx, double *tot6, int where, int *exchange_again);
@@ -307,6 +317,10 @@ int lq_get_S0(lq_ctx *ctx, double *S0);
  *   "sweep_bytes_per_site" (get): algorithmic HBM bytes one sweep moves per site
  *   "n_simulated" (get), "n_boundary" (get), "n_object" (get)
  *   "has_fixup" (get): 1 if a FIRE step on this context is a sweep plus a fix-up launch (stored force + objects)
+ *   "stored_force" (get): 1 if the fused FIRE sweep of this context keeps the force in memory (state (q, v, F): three
+ *                      constants, L4 / L6, or fire_path 2), 0 if it recomputes it (state (q, v))
+ *   "fire_sweeps_total" (get): between lq_fire_begin and lq_fire_end: the number of lq_fire_step_local rounds a full run
+ *                      of max_steps steps takes (see the step-wise protocol above); LQ_ERR_STATE otherwise
  *   "fp64_fma_tflops" (get): runs a register-only fp64 FMA microbenchmark on the context's device and stream (a few
  *                      milliseconds) and returns the measured TFLOP/s: the ALU roof next to the HBM one
  * Unknown key: LQ_ERR_ARG. */

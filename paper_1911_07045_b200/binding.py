@@ -147,6 +147,7 @@ class lq_ctx:
         self.handle = handle
         self.Lx, self.Ly, self.Lz = dims
         self.N = dims[0] * dims[1] * dims[2]
+        self.stream = 0                      # cudaStream_t handle last given to lq_set_stream (0 = legacy default)
 
     def __del__(self):
         try:
@@ -175,6 +176,7 @@ def lq_destroy(ctx: lq_ctx) -> None:
 def lq_set_stream(ctx, cuda_stream) -> None:
     """cuda_stream: integer handle (e.g. torch.cuda.current_stream().cuda_stream) or None."""
     _check(ctx.handle, load().lq_set_stream(ctx.handle, C.c_void_p(cuda_stream or 0)))
+    ctx.stream = int(cuda_stream or 0)
 
 
 def lq_set_sites(ctx, mask, anch_kind=None, W=None, axis=None) -> None:

@@ -342,6 +342,14 @@ int lq_get_info(lq_ctx *c, const char *key, double *value) {
         *value = ((lq_three(c->ph) || c->fire_path == 2) && c->flags_active) ? 1.0 : 0.0;
         return LQ_OK;
     }
+    if (!strcmp(key, "stored_force")) { *value = (lq_three(c->ph) || c->fire_path == 2) ? 1.0 : 0.0; return LQ_OK; }
+    if (!strcmp(key, "fire_sweeps_total")) {     // step-wise FIRE of a sub-domain: rounds a full run takes (lq.h)
+        if (!c->fire_open) return fail(c, LQ_ERR_STATE, "lq_get_info: fire_sweeps_total is defined between lq_fire_begin and lq_fire_end");
+        const bool extra = lq_three(c->ph) || c->fire_path == 2 || c->fire_fc.euler;
+        const long long m = c->fire_fc.max_steps;
+        *value = (double)(extra ? m + 1 : (m > 0 ? m : 1));
+        return LQ_OK;
+    }
     if (!strcmp(key, "fp64_fma_tflops")) {       // measured now: the fp64 ALU roof of this device (a few ms of FMAs)
         DeviceGuard dg(c);
         const double t = lq_measure_fp64_fma(c->device, c->stream);
@@ -440,6 +448,11 @@ int lq_fire_minimize(lq_ctx *c, long max_steps, double force_tol, const lq_fire_
         h.dt = fp->dt0; h.alpha = fp->alpha0; h.mix_a = 0.0; h.mix_b = 0.0; h.dt_prev = 0.0;
         h.init = (stored_F && !euler) ? 1 : 0;
         LQ_CUDA(c, cudaMemcpyAsync(&c->dsc[0], &h, sizeof(h), cudaMemcpyHostToDevice, st));
+        // build the plan first (tensor maps, the host-side search of the chunk table, set-up kernels: all on the first
+        // call only) and restart the clock, so that report.gpu_ms is the device time of the sweeps alone
+        if ((rc = lq_sweep_prepare(&c->sweep, stored_F, g, c->ph, f, c->q, c->v, c->F, st, &launches, c->err, c->rc_chunks)) != LQ_OK)
+            return rc;
+        LQ_CUDA(c, cudaEventRecord(c->ev0, st));
         rc = lq_sweep_run(&c->sweep, stored_F, g, c->ph, f, c->q, c->v, c->F, &c->cur, c->dsc, fc, max_steps, st, &launches,
                           &sweeps, &h, c->err, c->rc_chunks);
         if (rc != LQ_OK) return rc;

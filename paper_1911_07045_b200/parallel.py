@@ -9,8 +9,9 @@ Three drivers over the same pieces:
   * ``lq_slabs_fire_minimize`` (binding): N slabs of one process on one GPU, everything in C -- the measured path;
   * ``fire_minimize_emulated``: the per-rank pieces driven rank by rank in ONE process through a ``LocalComm``
     (how the transport-agnostic ABI is checked on the one B200 a lease has: no kernel ever waits on another);
-  * ``fire_minimize_rank``: one rank per GPU over ``torch.distributed`` (NCCL device buffers; gloo for the CPU test
-    of the comm layer).  Unmeasured on hardware: a lease has one GPU.
+  * ``fire_minimize_rank``: one rank per process over ``torch.distributed``: NCCL with device buffers (one rank per
+    GPU; unmeasured on hardware: a lease has one GPU) or gloo with host-staged packages (several processes sharing
+    the one GPU: tests/test_ranks_gpu.py runs it against the oracle).
 """
 from __future__ import annotations
 
@@ -133,87 +134,121 @@ class DistComm:
 
 # ------------------------------------------------------------------ step loops over the C-ABI pieces
 
-def _total_sweeps(max_steps, stored, euler):
-    return max_steps + 1 if (stored or euler) else max(max_steps, 1)
+def ctx_torch_stream(ctx):
+    """the context's CUDA stream as a torch stream.  The LQ_DEVICE halo / finish / commit calls only enqueue on that
+    stream (include/lq.h, "Stream order"), so every torch op and every NCCL call that touches their buffers has to
+    run with it as torch's current stream: NCCL orders its own stream against the current one on both sides."""
+    import torch
+    return torch.cuda.ExternalStream(ctx.stream) if ctx.stream else torch.cuda.default_stream()
 
 
-def fire_minimize_emulated(lq, ctxs, max_steps, force_tol, params, stored=False, poll=100):
+class _HaloBuffers:
+    """the four halo packages of one context (to / from the rank below and above), allocated ONCE at the size of the
+    larger package (LQ_HALO_STATE) and handed out as views: nothing the enqueued copies or the transport still read
+    can be recycled by torch's allocator between rounds.  host=True: pinned CPU tensors for a host-staged transport."""
+
+    def __init__(self, lq, ctx, host):
+        import torch
+        self.k = {w: lq.lq_halo_bytes(ctx, w) // 8 for w in (lq.LQ_HALO_Q, lq.LQ_HALO_STATE)}
+        kmax = max(self.k.values())
+        kw = dict(dtype=torch.float64, device="cpu", pin_memory=True) if host else \
+            dict(dtype=torch.float64, device=torch.device("cuda", torch.cuda.current_device()))
+        self.bufs = [torch.empty(kmax, **kw) for _ in range(4)]
+
+    def views(self, what):
+        return [b[:self.k[what]] for b in self.bufs]          # to_lo, to_hi, from_lo, from_hi
+
+
+def fire_minimize_emulated(lq, ctxs, max_steps, force_tol, params, poll=100):
     """the rank protocol, all ranks in this process, one after the other (no kernel waits on another):
-    step_local on every rank, all-gather of the rows, halo packages to both neighbours, commit on every rank"""
+    step_local on every rank, halo packages to both neighbours, all-gather of the rows, commit on every rank.
+    All contexts must use one stream (as lq_slabs_fire_minimize demands): packages change hands between them."""
     import torch
     n = len(ctxs)
+    if any(c.stream != ctxs[0].stream for c in ctxs):
+        raise ValueError("fire_minimize_emulated: all contexts must use the same stream")
     comm = LocalComm(n)
-    dev = torch.device("cuda")
+    with torch.cuda.stream(ctx_torch_stream(ctxs[0])):
+        hb = [_HaloBuffers(lq, c, host=False) for c in ctxs]
 
-    def halo_round(what):
-        nb = [lq.lq_halo_bytes(c, what) // 8 for c in ctxs]
-        sends = []
-        for c, k in zip(ctxs, nb):
-            lo, hi = torch.empty(k, dtype=torch.float64, device=dev), torch.empty(k, dtype=torch.float64, device=dev)
-            lq.lq_halo_export(c, what, 0, lo)
-            lq.lq_halo_export(c, what, 1, hi)
-            sends.append((lo, hi))
-        for c, (frm_lo, frm_hi) in zip(ctxs, comm.exchange(sends)):
-            lq.lq_halo_import(c, what, 0, frm_lo)
-            lq.lq_halo_import(c, what, 1, frm_hi)
+        def halo_round(what):
+            sends = []
+            for c, b in zip(ctxs, hb):
+                to_lo, to_hi, _, _ = b.views(what)
+                lq.lq_halo_export(c, what, 0, to_lo)
+                lq.lq_halo_export(c, what, 1, to_hi)
+                sends.append((to_lo, to_hi))
+            for c, (frm_lo, frm_hi) in zip(ctxs, comm.exchange(sends)):
+                lq.lq_halo_import(c, what, 0, frm_lo)
+                lq.lq_halo_import(c, what, 1, frm_hi)
 
-    halo_round(lq.LQ_HALO_Q)
-    for c in ctxs:
-        lq.lq_fire_begin(c, max_steps, force_tol, params)
-    euler = int(params.get("integrator", 0)) == 1
-    rows = torch.zeros((n, 6), dtype=torch.float64, device=dev)
-    total = _total_sweeps(max_steps, stored, euler)
-    for s in range(total):
+        halo_round(lq.LQ_HALO_Q)
         for c in ctxs:
-            lq.lq_fire_step_local(c)
-        halo_round(lq.LQ_HALO_STATE)
-        again = [lq.lq_fire_step_finish(c, rows[r]) for r, c in enumerate(ctxs)]
-        for c in ctxs:
-            lq.lq_fire_step_commit(c, rows)
-        if any(again):
+            lq.lq_fire_begin(c, max_steps, force_tol, params)
+        rows = torch.zeros((n, 6), dtype=torch.float64, device=torch.device("cuda", torch.cuda.current_device()))
+        total = int(lq.lq_get_info(ctxs[0], "fire_sweeps_total"))
+        for s in range(total):
+            for c in ctxs:
+                lq.lq_fire_step_local(c)
             halo_round(lq.LQ_HALO_STATE)
-        if force_tol > 0.0 and (s + 1) % poll == 0 and lq.lq_fire_peek(ctxs[0])["converged"]:
-            break
-    reps = [lq.lq_fire_end(c) for c in ctxs]
-    halo_round(lq.LQ_HALO_Q)
+            again = [lq.lq_fire_step_finish(c, rows[r]) for r, c in enumerate(ctxs)]
+            for c in ctxs:
+                lq.lq_fire_step_commit(c, rows)
+            if any(again):
+                halo_round(lq.LQ_HALO_STATE)
+            if force_tol > 0.0 and (s + 1) % poll == 0 and lq.lq_fire_peek(ctxs[0])["converged"]:
+                break
+        reps = [lq.lq_fire_end(c) for c in ctxs]
+        halo_round(lq.LQ_HALO_Q)
+        torch.cuda.current_stream().synchronize()
     return reps[0]
 
 
-def fire_minimize_rank(lq, ctx, comm: DistComm, max_steps, force_tol, params, stored=False, poll=100):
-    """one rank of the decomposed run (call on every rank): NCCL moves the halo packages and the 6-double rows.
-    Unmeasured on hardware (one GPU per lease); the comm layer is covered by the gloo test."""
+def fire_minimize_rank(lq, ctx, comm: DistComm, max_steps, force_tol, params, poll=100, staging="device"):
+    """one rank of the decomposed run (call on every rank).
+
+    staging="device": NCCL moves the halo packages and the 6-double rows between device buffers.  Everything -- the
+    library's enqueue-only LQ_DEVICE calls, torch's ops, NCCL -- runs with the context's stream as torch's current
+    stream, so the run is stream-ordered end to end with no host synchronisation inside a step (only lq_fire_peek
+    every `poll` steps when there is a force tolerance).
+    staging="host": packages and rows go through pinned host buffers (the LQ_HOST calls synchronise the stream), for
+    a transport without device support (gloo): how the protocol is run rank-per-process on the one GPU a lease has.
+    Buffers are allocated once, before the step loop.  Returns this rank's report (Frms: lq_fire_end's note)."""
     import torch
-    dev = torch.device("cuda", torch.cuda.current_device())
+    if staging not in ("device", "host"):
+        raise ValueError("staging must be 'device' or 'host'")
+    host = staging == "host"
+    with torch.cuda.stream(ctx_torch_stream(ctx)):
+        where = torch.device("cpu") if host else torch.device("cuda", torch.cuda.current_device())
+        hb = _HaloBuffers(lq, ctx, host)
+        row = torch.zeros(6, dtype=torch.float64, device=where)
+        rows = torch.zeros((comm.world, 6), dtype=torch.float64, device=where)
 
-    def halo_round(what):
-        k = lq.lq_halo_bytes(ctx, what) // 8
-        to_lo, to_hi, from_lo, from_hi = (torch.empty(k, dtype=torch.float64, device=dev) for _ in range(4))
-        lq.lq_halo_export(ctx, what, 0, to_lo)
-        lq.lq_halo_export(ctx, what, 1, to_hi)
-        torch.cuda.current_stream().synchronize()
-        comm.exchange(to_lo, to_hi, from_lo, from_hi)
-        lq.lq_halo_import(ctx, what, 0, from_lo)
-        lq.lq_halo_import(ctx, what, 1, from_hi)
+        def halo_round(what):
+            to_lo, to_hi, from_lo, from_hi = hb.views(what)
+            lq.lq_halo_export(ctx, what, 0, to_lo)
+            lq.lq_halo_export(ctx, what, 1, to_hi)
+            comm.exchange(to_lo, to_hi, from_lo, from_hi)
+            lq.lq_halo_import(ctx, what, 0, from_lo)
+            lq.lq_halo_import(ctx, what, 1, from_hi)
 
-    halo_round(lq.LQ_HALO_Q)
-    lq.lq_fire_begin(ctx, max_steps, force_tol, params)
-    euler = int(params.get("integrator", 0)) == 1
-    row = torch.zeros(6, dtype=torch.float64, device=dev)
-    rows = torch.zeros((comm.world, 6), dtype=torch.float64, device=dev)
-    # a second halo round per step is needed as soon as ANY rank's step has a fix-up launch: agree on it once
-    row[0] = lq.lq_get_info(ctx, "has_fixup")
-    comm.allgather(row, rows)
-    again = bool(rows[:, 0].max().item() > 0)
-    for s in range(_total_sweeps(max_steps, stored, euler)):
-        lq.lq_fire_step_local(ctx)
-        halo_round(lq.LQ_HALO_STATE)
-        lq.lq_fire_step_finish(ctx, row)
+        halo_round(lq.LQ_HALO_Q)
+        lq.lq_fire_begin(ctx, max_steps, force_tol, params)
+        # a second halo round per step is needed as soon as ANY rank's step has a fix-up launch: agree on it once
+        row[0] = lq.lq_get_info(ctx, "has_fixup")
         comm.allgather(row, rows)
-        lq.lq_fire_step_commit(ctx, rows)
-        if again:
+        again = bool(rows[:, 0].max().item() > 0)
+        for s in range(int(lq.lq_get_info(ctx, "fire_sweeps_total"))):
+            lq.lq_fire_step_local(ctx)
             halo_round(lq.LQ_HALO_STATE)
-        if force_tol > 0.0 and (s + 1) % poll == 0 and lq.lq_fire_peek(ctx)["converged"]:
-            break
-    rep = lq.lq_fire_end(ctx)
-    halo_round(lq.LQ_HALO_Q)
+            lq.lq_fire_step_finish(ctx, row)
+            comm.allgather(row, rows)
+            lq.lq_fire_step_commit(ctx, rows)
+            if again:
+                halo_round(lq.LQ_HALO_STATE)
+            if force_tol > 0.0 and (s + 1) % poll == 0 and lq.lq_fire_peek(ctx)["converged"]:
+                break
+        rep = lq.lq_fire_end(ctx)
+        halo_round(lq.LQ_HALO_Q)
+        torch.cuda.current_stream().synchronize()
     return rep

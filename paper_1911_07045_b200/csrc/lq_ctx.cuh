@@ -34,6 +34,8 @@ struct lq_ctx {
     long fire_sweeps = 0, fire_launches = 0;
     double *dtot = nullptr;              // 6 doubles: this sub-domain's reductions of the last lq_fire_step_local
     LqPartialSeg *dsegs = nullptr;       // device copy of the last sweep's partial-sum segments
+    LqPartialSeg hsegs[3] = {};          // what dsegs holds (uploaded again only when a step's segments differ)
+    int hnseg = -1;
     LqFireScalars **dscptr = nullptr;    // device array {&dsc[0]} for the advance kernel
     int fire_cur0 = 0, fire_buf = 0;     // live buffer when the run began / buffer the last sweep wrote
     bool fire_sweep_pending = false;     // lq_fire_step_local ran, lq_fire_step_finish not yet

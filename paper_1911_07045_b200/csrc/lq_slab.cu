@@ -144,6 +144,27 @@ int fire_finish(lq_ctx *c, LqPartialSeg seg[3], int *nseg) {
     return LQ_OK;
 }
 
+// the segment table of a step on the device: it changes only between the first sweep and the rest of a run, so it is
+// uploaded when it differs from what the device copy already holds, not every step
+cudaError_t upload_segments(lq_ctx *c, const LqPartialSeg *seg, int nseg) {
+    if (nseg == c->hnseg && memcmp(seg, c->hsegs, nseg * sizeof(LqPartialSeg)) == 0) return cudaSuccess;
+    // pageable source: staged before the call returns, so hsegs may change right after
+    const cudaError_t e = cudaMemcpyAsync(c->dsegs, seg, nseg * sizeof(LqPartialSeg), cudaMemcpyHostToDevice, c->stream);
+    if (e != cudaSuccess) { c->hnseg = -1; return e; }
+    memset(c->hsegs, 0, sizeof(c->hsegs));
+    memcpy(c->hsegs, seg, nseg * sizeof(LqPartialSeg));
+    c->hnseg = nseg;
+    return cudaSuccess;
+}
+
+// a step-wise run given up half way: leave the context as it was before lq_fire_begin (live buffer, no open run)
+void fire_abort(lq_ctx *c) {
+    if (!c->fire_open) return;
+    c->fire_open = false;
+    c->fire_sweep_pending = false;
+    c->cur = c->fire_cur0;
+}
+
 int fire_end(lq_ctx *c, lq_fire_report *out) {
     if (!c->fire_open) return fail(c, LQ_ERR_STATE, "lq_fire_end: no step-wise FIRE run is open");
     LqFireScalars h;
@@ -230,6 +251,7 @@ int lq_set_sites_ext(lq_ctx *c, const uint8_t *mask_ext, const uint8_t *kind_ext
     lq_descent_invalidate(c->descent);
     // the dense mask with its 3-plane margin on the device
     uint8_t *dmask = nullptr, *dkind = nullptr;
+    struct FreeOnExit { uint8_t *&p; ~FreeOnExit() { cudaFree(p); p = nullptr; } } free_dmask{dmask};   // every return path
     LQ_CUDA(c, cudaMalloc(&dmask, next));
     cudaError_t e = cudaMemcpyAsync(dmask, mask_ext, next, cudaMemcpyDefault, st);
     int bad[2] = {0, 0};
@@ -243,7 +265,7 @@ int lq_set_sites_ext(lq_ctx *c, const uint8_t *mask_ext, const uint8_t *kind_ext
     if (e == cudaSuccess) e = cudaMemcpyAsync(bad, c->dbad, 2 * sizeof(int), cudaMemcpyDeviceToHost, st);
     if (e == cudaSuccess) e = cudaStreamSynchronize(st);
     if (e != cudaSuccess || bad[0] || bad[1]) {
-        cudaFree(dmask); cudaFree(dkind);
+        cudaFree(dkind);
         c->flags_active = false; c->anch_active = false;
         c->n_class[0] = (unsigned long long)g.N; c->n_class[1] = c->n_class[2] = 0;
         if (e != cudaSuccess) return fail(c, LQ_ERR_CUDA, std::string("lq_set_sites_ext: ") + cudaGetErrorString(e));
@@ -280,7 +302,6 @@ int lq_set_sites_ext(lq_ctx *c, const uint8_t *mask_ext, const uint8_t *kind_ext
     LQ_CUDA(c, cudaMemcpyAsync(&any, c->dbad, sizeof(int), cudaMemcpyDeviceToHost, st));
     LQ_CUDA(c, cudaMemcpyAsync(c->n_class, c->dcounts, 3 * sizeof(unsigned long long), cudaMemcpyDeviceToHost, st));
     LQ_CUDA(c, cudaStreamSynchronize(st));
-    cudaFree(dmask);
     LQ_CUDA(c, cudaGetLastError());
     c->flags_active = any != 0;
     c->anch_active = kind_ext != nullptr && any != 0;
@@ -344,7 +365,7 @@ int lq_fire_step_finish(lq_ctx *c, double *tot6, int where, int *exchange_again)
     int nseg = 0;
     int rc = fire_finish(c, seg, &nseg);
     if (rc != LQ_OK) return rc;
-    LQ_CUDA(c, cudaMemcpyAsync(c->dsegs, seg, nseg * sizeof(LqPartialSeg), cudaMemcpyHostToDevice, c->stream));
+    LQ_CUDA(c, upload_segments(c, seg, nseg));
     lq_launch_reduce_partials(c->dsegs, nseg, c->dtot, c->stream);
     LQ_CUDA(c, cudaMemcpyAsync(tot6, c->dtot, 6 * sizeof(double), cudaMemcpyDefault, c->stream));
     if (where == LQ_HOST) LQ_CUDA(c, cudaStreamSynchronize(c->stream));
@@ -365,6 +386,7 @@ int lq_fire_step_commit(lq_ctx *c, const double *tot, int nrank, int where) {
             c->scratch_len = (size_t)nrank * 6 * sizeof(double);
         }
         LQ_CUDA(c, cudaMemcpyAsync(c->scratch, tot, (size_t)nrank * 6 * sizeof(double), cudaMemcpyHostToDevice, c->stream));
+        LQ_CUDA(c, cudaStreamSynchronize(c->stream));    // pinned host rows are read asynchronously: free to reuse on return
         dt = (const double *)c->scratch;
     }
     lq_launch_advance(dt, nrank, c->dscptr, 1, c->fire_fc, c->fire_last_first ? 1 : 0, c->stream);
@@ -421,23 +443,26 @@ int lq_slabs_fire_minimize(lq_ctx **slabs, int n, long max_steps, double force_t
     }
     int rc;
     if ((rc = slabs_exchange(slabs, n, LQ_HALO_Q, st)) != LQ_OK) return rc;       // ghosts of the initial state
+    LqFireScalars **dscs = nullptr;
+    double *drows = nullptr;
+    // every exit below goes through one of these two: device tables freed; on failure every slab's run closed too
+    auto cleanup = [&]() { cudaFree(dscs); cudaFree(drows); dscs = nullptr; drows = nullptr; };
+    auto give_up = [&](int code, lq_ctx *who) {
+        if (who && who != c0) c0->err = who->err;
+        for (int i = 0; i < n; ++i) fire_abort(slabs[i]);
+        cleanup();
+        return code;
+    };
     for (int i = 0; i < n; ++i)
-        if ((rc = fire_begin(slabs[i], max_steps, force_tol, fp)) != LQ_OK) {
-            if (slabs[i] != c0) c0->err = slabs[i]->err;
-            return rc;
-        }
+        if ((rc = fire_begin(slabs[i], max_steps, force_tol, fp)) != LQ_OK) return give_up(rc, slabs[i]);
     // device tables: every slab's scalars; one row of reductions per slab (combined in slab order by the advance
     // kernel: the same arithmetic as the one-rank-per-GPU protocol, so both give bit-identical trajectories)
     std::vector<LqFireScalars *> scs(n);
     for (int i = 0; i < n; ++i) scs[i] = &slabs[i]->dsc[0];
-    LqFireScalars **dscs = nullptr;
-    double *drows = nullptr;
-    auto cleanup = [&]() { cudaFree(dscs); cudaFree(drows); };
-    if (cudaMalloc(&dscs, n * sizeof(LqFireScalars *)) != cudaSuccess || cudaMalloc(&drows, (size_t)6 * n * sizeof(double)) != cudaSuccess) {
-        cleanup();
-        return fail(c0, LQ_ERR_NOMEM, "lq_slabs_fire_minimize: cudaMalloc failed");
-    }
-    cudaMemcpyAsync(dscs, scs.data(), n * sizeof(LqFireScalars *), cudaMemcpyHostToDevice, st);
+    if (cudaMalloc(&dscs, n * sizeof(LqFireScalars *)) != cudaSuccess || cudaMalloc(&drows, (size_t)6 * n * sizeof(double)) != cudaSuccess)
+        return give_up(fail(c0, LQ_ERR_NOMEM, "lq_slabs_fire_minimize: cudaMalloc failed"), nullptr);
+    if (cudaMemcpyAsync(dscs, scs.data(), n * sizeof(LqFireScalars *), cudaMemcpyHostToDevice, st) != cudaSuccess)
+        return give_up(fail(c0, LQ_ERR_CUDA, "lq_slabs_fire_minimize: upload of the scalar table failed"), nullptr);
     bool any_fixup = false;
     for (int i = 0; i < n; ++i) any_fixup |= has_fixup(slabs[i]);
     const long total = fire_total_sweeps(c0);
@@ -449,33 +474,33 @@ int lq_slabs_fire_minimize(lq_ctx **slabs, int n, long max_steps, double force_t
         const long m = (total - done) < chunk ? (total - done) : chunk;
         for (long s = 0; s < m; ++s) {
             for (int i = 0; i < n; ++i)
-                if ((rc = fire_sweep(slabs[i])) != LQ_OK) { if (slabs[i] != c0) c0->err = slabs[i]->err; cleanup(); return rc; }
+                if ((rc = fire_sweep(slabs[i])) != LQ_OK) return give_up(rc, slabs[i]);
             // the new state's boundary planes to the neighbours; where a fix-up launch follows (it evaluates the force
             // of the sites next to objects on q', across the slab faces too) it changes v and F there: exchange again
-            if ((rc = slabs_exchange(slabs, n, LQ_HALO_STATE, st)) != LQ_OK) { cleanup(); return rc; }
+            if ((rc = slabs_exchange(slabs, n, LQ_HALO_STATE, st)) != LQ_OK) return give_up(rc, nullptr);
             for (int i = 0; i < n; ++i) {
                 lq_ctx *c = slabs[i];
                 LqPartialSeg sg[3];
                 int ns = 0;
-                if ((rc = fire_finish(c, sg, &ns)) != LQ_OK) { if (c != c0) c0->err = c->err; cleanup(); return rc; }
-                // (a pageable-source copy is staged before it returns, so reusing sg next iteration is safe)
-                cudaMemcpyAsync(c->dsegs, sg, ns * sizeof(LqPartialSeg), cudaMemcpyHostToDevice, st);
+                if ((rc = fire_finish(c, sg, &ns)) != LQ_OK) return give_up(rc, c);
+                if (upload_segments(c, sg, ns) != cudaSuccess)
+                    return give_up(fail(c0, LQ_ERR_CUDA, "lq_slabs_fire_minimize: upload of the segment table failed"), nullptr);
                 lq_launch_reduce_partials(c->dsegs, ns, drows + 6 * i, st);
             }
             lq_launch_advance(drows, n, dscs, n, c0->fire_fc, c0->fire_last_first ? 1 : 0, st);
-            if (any_fixup && (rc = slabs_exchange(slabs, n, LQ_HALO_STATE, st)) != LQ_OK) { cleanup(); return rc; }
+            if (any_fixup && (rc = slabs_exchange(slabs, n, LQ_HALO_STATE, st)) != LQ_OK) return give_up(rc, nullptr);
         }
         done += m;
         if (force_tol > 0.0) {
-            cudaMemcpyAsync(&h, &c0->dsc[0], sizeof(h), cudaMemcpyDeviceToHost, st);
-            if (cudaStreamSynchronize(st) != cudaSuccess) { cleanup(); return fail(c0, LQ_ERR_CUDA, "lq_slabs_fire_minimize: stream error"); }
+            if (cudaMemcpyAsync(&h, &c0->dsc[0], sizeof(h), cudaMemcpyDeviceToHost, st) != cudaSuccess || cudaStreamSynchronize(st) != cudaSuccess)
+                return give_up(fail(c0, LQ_ERR_CUDA, "lq_slabs_fire_minimize: stream error"), nullptr);
             if (h.converged) break;
         }
     }
     double nsim = 0.0;
     lq_fire_report rep;
     for (int i = 0; i < n; ++i) {
-        if ((rc = fire_end(slabs[i], i == 0 ? out : &rep)) != LQ_OK) { cleanup(); return rc; }
+        if ((rc = fire_end(slabs[i], i == 0 ? out : &rep)) != LQ_OK) return give_up(rc, slabs[i]);
         nsim += (double)(slabs[i]->flags_active ? slabs[i]->n_class[0] + slabs[i]->n_class[1] : (unsigned long long)slabs[i]->g.N);
         if (i > 0) { out->launches += rep.launches; out->sweep_launches += rep.sweep_launches; }
     }

@@ -90,9 +90,9 @@ def test_rank_protocol_pieces_vs_oracle(lq, oracle_mod, name):
     c = CASES[name]()
     o = make_oracle(oracle_mod, c)
     qref, _ = o.fire(c["q"], 60, 0.0, c["fire"], variant=1)
-    stored = c["L2"] != 0 or c["L3"] != 0
     ctxs = parallel.make_slabs(lq, c, 3)
-    rep = parallel.fire_minimize_emulated(lq, ctxs, 60, 0.0, c["fire"], stored=stored)
+    assert lq.lq_get_info(ctxs[0], "stored_force") == (1.0 if (c["L2"] != 0 or c["L3"] != 0) else 0.0)
+    rep = parallel.fire_minimize_emulated(lq, ctxs, 60, 0.0, c["fire"])
     q = parallel.gather(lq.lq_get_Q, ctxs)
     assert rep["steps"] == 60
     assert np.abs(q - qref).max() <= TOL_Q100
@@ -101,6 +101,31 @@ def test_rank_protocol_pieces_vs_oracle(lq, oracle_mod, name):
     assert np.array_equal(parallel.gather(lq.lq_get_Q, ctxs2), q)
     for x in ctxs + ctxs2:
         lq.lq_destroy(x)
+
+
+@pytest.mark.parametrize("name", ["replica4", "replica3"])
+def test_slabs_semi_implicit_euler_and_velocity(lq, oracle_mod, name):
+    """integrator = 1 through the group driver (extra sweep, dt_prev, no FIRST instantiation) against the oracle, and
+    lq_get_velocity on sub-domain contexts (pending lazy rescale + a force pass that needs the final ghost planes)
+    against the oracle and the undivided context, for both integrators"""
+    c = CASES[name]()
+    o = make_oracle(oracle_mod, c)
+    for integrator in (1, 0):
+        fire = dict(c["fire"], integrator=integrator)
+        qref, rref, vref = o.fire(c["q"], 60, 0.0, fire, variant=1, return_v=True)
+        ctxs = parallel.make_slabs(lq, c, 2)
+        rep = lq.lq_slabs_fire_minimize(ctxs, 60, 0.0, fire)
+        q, v = parallel.gather(lq.lq_get_Q, ctxs), parallel.gather(lq.lq_get_velocity, ctxs)
+        assert rep["steps"] == 60 == rref["steps"]
+        assert np.abs(q - qref).max() <= TOL_Q100, "%s integrator %d: Q err %.3e" % (name, integrator, np.abs(q - qref).max())
+        assert abs(rep["dt"] - rref["dt"]) <= 1e-15 and abs(rep["alpha"] - rref["alpha"]) <= 1e-15
+        vscale = max(np.abs(vref).max(), 1e-3)
+        assert np.abs(v - vref).max() <= 1e-7 * vscale
+        whole = lq.create_from_config(c)
+        lq.lq_fire_minimize(whole, 60, 0.0, fire)
+        assert np.abs(v - lq.lq_get_velocity(whole)).max() <= 1e-7 * vscale
+        for x in ctxs + [whole]:
+            lq.lq_destroy(x)
 
 
 def test_slabs_converge_and_stop(lq, oracle_mod):

@@ -319,19 +319,34 @@ std::vector<int4> lq_build_chunk_table(int ntx, int nty, int Lz, int max_chunk, 
     } else if ((long long)T * best_na < 10LL * nsm) {
         double best = -1.0;
         std::vector<long long> load(nsm);
-        auto makespan = [&](int Ta, int na, int nb) -> double {
-            // items: Ta*na of cost ~Lz/na + ovh, (T-Ta)*nb of cost ~Lz/nb + ovh; greedy on the least-loaded SM
-            std::vector<int> cost;
-            cost.reserve((size_t)Ta * na + (size_t)(T - Ta) * nb);
-            for (int t = 0; t < T; ++t) {
-                const int n = t < Ta ? na : nb;
-                for (int i = 0; i < n; ++i) { int zb, ze; chunks(n, i, zb, ze); cost.push_back(ze - zb + ovh); }
+        // a candidate's cost multiset depends only on the chunk lengths: histogram them (no sort), and skip the
+        // candidate when its lower bound max(ceil(sum / nsm), longest item) cannot beat the best makespan so far
+        // (only a strictly smaller makespan replaces the best, so the table chosen is the same as an exhaustive
+        // search's).  This is host time of the first call on a context.
+        std::vector<int> hist((size_t)Lz + ovh + 2);
+        auto add_lengths = [&](int n, long long tiles, int &longest) {
+            if (tiles <= 0) return;
+            for (int i = 0; i < n; ++i) {
+                int zb, ze;
+                chunks(n, i, zb, ze);
+                hist[ze - zb + ovh] += (int)tiles;
+                if (ze - zb + ovh > longest) longest = ze - zb + ovh;
             }
-            std::sort(cost.begin(), cost.end(), std::greater<int>());
-            std::priority_queue<long long, std::vector<long long>, std::greater<long long>> pq;
-            for (int i = 0; i < nsm; ++i) pq.push(0);
+        };
+        auto makespan = [&](int Ta, int na, int nb) -> double {
+            // items: Ta*na of cost ~Lz/na + ovh, (T-Ta)*nb of cost ~Lz/nb + ovh; longest first, each onto the
+            // least-loaded SM
+            const long long sum = (long long)Ta * (Lz + (long long)na * ovh) + (long long)(T - Ta) * (Lz + (long long)nb * ovh);
+            std::fill(hist.begin(), hist.end(), 0);
+            int longest = 0;
+            add_lengths(na, Ta, longest);
+            add_lengths(nb, T - Ta, longest);
+            const long long lb = std::max((sum + nsm - 1) / nsm, (long long)longest);
+            if (best >= 0.0 && (double)lb >= best) return (double)lb;      // cannot be strictly better
+            std::priority_queue<long long, std::vector<long long>, std::greater<long long>> pq(std::greater<long long>(), load);
             long long mk = 0;
-            for (int c : cost) { long long l = pq.top() + c; pq.pop(); pq.push(l); if (l > mk) mk = l; }
+            for (int c = longest; c >= 0; --c)
+                for (int k = 0; k < hist[c]; ++k) { long long l = pq.top() + c; pq.pop(); pq.push(l); if (l > mk) mk = l; }
             return (double)mk;
         };
         for (int na = n_min; na <= n_max && na <= n_min + 24; ++na)

@@ -122,6 +122,9 @@ class DistComm:
             from_lo.copy_(to_hi)
             from_hi.copy_(to_lo)
             return
+        # gloo matches by tag; NCCL ignores tags and matches the sends and receives of a pair of ranks in issue order.
+        # With two ranks both neighbours are the same peer: the order below pairs my first send (low face) with its
+        # first receive (its high ghost) and my second send with its second receive, which is what is wanted.
         ops = [d.P2POp(d.isend, to_lo, lo, tag=0), d.P2POp(d.isend, to_hi, hi, tag=1),
                d.P2POp(d.irecv, from_hi, hi, tag=0), d.P2POp(d.irecv, from_lo, lo, tag=1)]
         for w in d.batch_isend_irecv(ops):

@@ -105,3 +105,25 @@ def test_rank_per_process_vs_oracle_and_group_driver(name, world, integrator, or
         assert np.array_equal(q[:, obj], c["q"][:, obj]) and np.abs(v[:, obj]).max(initial=0.0) == 0.0
     for x in ctxs:
         lq.lq_destroy(x)
+
+
+def test_bench_decomp_one_rank_nccl():
+    """bench.py --decomp with one rank: the same driver with staging="device" -- NCCL process group, device halo
+    packages, all_gather of the row, everything on the context's stream -- on the one GPU (the slab is the whole
+    lattice and its halo wraps onto itself).  Checks the JSON contract of the decomposed arm."""
+    import json
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    env = dict(os.environ, MASTER_ADDR="127.0.0.1", MASTER_PORT=str(_free_port()))
+    for k in ("RANK", "WORLD_SIZE", "LOCAL_RANK"):
+        env.pop(k, None)
+    out = subprocess.run([sys.executable, os.path.join(root, "bench.py"), "--decomp", "--workload", "2", "--steps", "40",
+                          "--warmup", "3", "--no-cpu-baseline", "--no-e2e", "--sustained-s", "0.2"],
+                         capture_output=True, text=True, timeout=600, env=env, cwd=root)
+    assert out.returncode == 0, out.stderr[-2000:]
+    line = json.loads(out.stdout.strip().splitlines()[-1])
+    assert line["config"]["multi_gpu"] == "z-slabs" and line["scaling"] == "strong" and line["n_gpus"] == 1
+    assert line["steps"] == 40 and line["value"] > 0 and line["gpu_launches"] >= 40
+    assert line["config"]["n_simulated"] == 980000
+    assert line["roofline"]["sustained"]["steps"] >= 40 and line["roofline"]["sustained"]["frac"] > 0

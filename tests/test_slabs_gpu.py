@@ -145,6 +145,16 @@ def test_slabs_converge_and_stop(lq, oracle_mod):
     rep = lq.lq_slabs_fire_minimize(ctxs, 10, 1e-9, c["fire"])
     assert rep["converged"] == 1 and rep["steps"] == 0
     assert np.array_equal(parallel.gather(lq.lq_get_Q, ctxs), qu)
+    # the sweep count of the step-wise protocol is only defined while a run is open
+    with pytest.raises(lq.LqError) as ei:
+        lq.lq_get_info(ctxs[0], "fire_sweeps_total")
+    assert ei.value.code == lq.LQ_ERR_STATE
+    lq.lq_fire_begin(ctxs[0], 7, 0.0, c["fire"])
+    assert lq.lq_get_info(ctxs[0], "fire_sweeps_total") == 7 and lq.lq_get_info(ctxs[0], "stored_force") == 0
+    lq.lq_fire_end(ctxs[0])
+    lq.lq_fire_begin(ctxs[0], 7, 0.0, dict(c["fire"], integrator=1))
+    assert lq.lq_get_info(ctxs[0], "fire_sweeps_total") == 8
+    lq.lq_fire_end(ctxs[0])
     # misuse: a sub-domain context refuses the single-domain minimisers
     with pytest.raises(lq.LqError) as ei:
         lq.lq_fire_minimize(ctxs[0], 1, 0.0, c["fire"])

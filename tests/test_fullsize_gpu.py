@@ -9,7 +9,7 @@ the full 100 steps against the oracle in the SAME launch configuration as the 51
 waves of CTAs).  north_star's converged-energy gate (rel 1e-6): config 2 at full size against the oracle and the
 closed form 980000 f0; configs 3, 5, 5' on their declared replicas (the full-size runs need 5000 /
 30000 steps of a 16M-site oracle).  The oracle leg of the config-2 convergence run (7.3 min) is opt-in:
-LQ_FULL_PARITY=1; its passing log is kept in profiles/r02_parity_fullsize.txt.  Also at full size: gradient descent and
+LQ_FULL_PARITY=1; its passing logs are kept in profiles/r02_parity_fullsize.txt and r03_parity_fullsize.txt.  Also at full size: gradient descent and
 Nesterov on configs 5 and 3, the analysis kernel at 512^3 on sampled sites, and config 3's lattice with every energy
 term switched on (chiral, cubic, both fields).
 """
@@ -168,7 +168,7 @@ def test_config2_converged_energy_full_size(lq, oracle_mod):
     assert rep["converged"] == 1 and rep["Fmax"] < c["tol"]
     assert abs(rep["energy"] - 980000 * f0) <= TOL_ECONV * abs(980000 * f0)
     if not FULL:
-        # the oracle leg takes 7.3 min on the GPU box's 16 cores (measured; passing log: profiles/r02_parity_fullsize.txt):
+        # the oracle leg takes 7.3 min on the GPU box's 16 cores (measured; passing logs: profiles/r02_parity_fullsize.txt, r03_parity_fullsize.txt):
         # opt in with LQ_FULL_PARITY=1 so that the default -m gpu suite stays near ten minutes
         lq.lq_destroy(ctx)
         return
@@ -206,7 +206,7 @@ def test_full_size_descent(lq, oracle_mod, name):
     kernel (opt-in, LQ_FULL_PARITY=1: 72 s of oracle; test_full_size_every_term_on runs the same kernels on the same
     lattice by default)."""
     if name == "3" and not FULL:
-        pytest.skip("config 3 leg is opt-in (LQ_FULL_PARITY=1); passing log: profiles/r02_parity_fullsize.txt")
+        pytest.skip("config 3 leg is opt-in (LQ_FULL_PARITY=1); passing logs: profiles/r02_parity_fullsize.txt, profiles/r03_parity_fullsize.txt")
     c = wl.make_config(name)
     ctx = lq.create_from_config(c)
     o = make_oracle(oracle_mod, c)
